@@ -1,0 +1,180 @@
+/*
+ * dc.h -- C ABI of libdc: the direct-cut hole-cutting pass on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (PAPER.md = arxiv 1711.07663; line numbers of /root/reference/PAPER.md):
+ *   "rather than searching for all elements which intersect a cutting boundary, we instead have
+ *    all elements calculate the (signed) minimum distance to the boundary ... to directly
+ *    determine whether each element is inside, outside, or intersecting with the boundary"
+ *   (section 4.2).  For every element e of ONE grid of 27-node quadratic hexahedra
+ *   (tensor-product Lagrange map, Eq. 1, K = 2) and ONE closed, outward-oriented cutting
+ *   surface of 9-node quadratic quadrilateral faces (L171-L175, L215):
+ *       d_e   = min over faces f, boundary patches k of e, and (u,v),(s,t) in [-1,1]^2 of
+ *               |P_{e,k}(u,v) - Q_f(s,t)|
+ *       label = DC_CUT    if d_e <= tau_cut     (L151; A.3 L719/L773-L777, A.4 L815-L837)
+ *               DC_HOLE   if (p* - q*) . n(q*) < 0 at the closest pair, n = Q_s x Q_t  (L151, L215)
+ *               DC_NORMAL otherwise
+ *       sdist = 0 for CUT, else +-min(d_e, d_band), + for NORMAL.
+ *   Elements farther than d_band from the surface take their label from a flood fill over the
+ *   face adjacency of non-CUT elements (the classical paint-fill, L143, Fig. 5), seeded by the
+ *   elements inside the band.
+ *
+ * Conventions (paper silent; readings A1/A2):
+ *   hex node  m = i + 3 j + 9 k  (xi fastest), reference nodes {-1, 0, +1};  quad node m = i + 3 j;
+ *   element faces k = 0..5 <-> xi=-1, xi=+1, eta=-1, eta=+1, zeta=-1, zeta=+1;
+ *   adj6[e][k] = element across face k, or -1.
+ *
+ * Memory: every pointer marked "dev" is a CUDA device pointer OWNED BY THE CALLER (allocated
+ * e.g. with torch); "host" pointers are host memory (pinned for asynchronous copies).  The
+ * library never allocates device memory: all scratch lives in the caller's workspace.
+ * The context borrows xyz / conn27 / adj6 / workspace until dc_destroy and the face buffer
+ * until the next dc_set_cut_surface.
+ *
+ * Errors: every call returns 0 (DC_OK) or a negative code; no exceptions, no global state.
+ * dc_set_cut_surface / dc_classify only enqueue work on `stream` (a cudaStream_t passed as
+ * void*) and never synchronise; conditions found on the device (pair-list overflow, ...)
+ * are latched into dc_stats.status and returned by dc_get_stats, which synchronises.
+ */
+#ifndef DC_H_
+#define DC_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* labels (int8).  0/1 follow the usual iblank hole/field convention; the paper's hole map uses
+ * the same three values (L169). */
+#define DC_HOLE 0
+#define DC_NORMAL 1
+#define DC_CUT 2
+
+/* return codes */
+#define DC_OK 0
+#define DC_ERR_ARG (-1)         /* NULL / negative / inconsistent argument */
+#define DC_ERR_WORKSPACE (-2)   /* workspace too small, or a device-side list overflowed */
+#define DC_ERR_UNSUPPORTED (-3) /* device is not sm_100, or input violates a documented precondition */
+#define DC_ERR_CUDA (-4)        /* a CUDA runtime call failed */
+#define DC_ERR_STATE (-5)       /* call order: dc_classify before dc_set_cut_surface, ... */
+
+/* dc_stats.status bits (device-side conditions) */
+#define DC_STATUS_PAIR_OVERFLOW 1   /* candidate pair list exceeded max_pairs: results invalid */
+#define DC_STATUS_QUEUE_OVERFLOW 2  /* narrow-phase work queue spill area exhausted: results invalid */
+#define DC_STATUS_FILL_CONFLICT 4   /* a flood-fill component has seeds of both signs */
+#define DC_STATUS_SEEDLESS_OVERFLOW 8 /* more seedless components than DC_MAX_SEEDLESS */
+
+/* dc_params.flags */
+#define DC_FLAG_RECOMPUTE_BOXES 1   /* redo step S2 (element boxes from raw nodes) inside dc_classify
+                                       instead of using the boxes cached by dc_create_grid */
+
+typedef struct dc_ctx dc_ctx;
+
+typedef struct {
+    double tau_cut_rel; /* CUT threshold / L_ref; <= 0: default 1e-7 (A.3 L719; reading A3) */
+    double d_band;      /* exact-distance band; <= 0: auto = max element Bezier-box diagonal (A5) */
+    double l_ref;       /* reference length; <= 0: auto = longest edge of the surface-node AABB */
+    double theta_leaf;  /* subdivision stops when (patch size) x (curvature) <= theta; <= 0: 0.125 */
+    int max_level;      /* subdivision bound per patch, 1..12; <= 0: default 12 */
+    int flags;          /* DC_FLAG_* */
+} dc_params;
+
+typedef struct {
+    long long n_elem, n_face;
+    long long n_active;          /* elements that reached candidate generation (S4) */
+    long long n_box_tests;       /* element-box vs face-box tests in S4 ("broad" pair tests) */
+    long long n_pairs;           /* candidate (element, face) pairs = narrow-phase pair tests */
+    long long n_bnb_nodes;       /* sub-pairs bounded in S5 */
+    long long n_newton;          /* Newton solves in S5 */
+    long long n_newton_iters;
+    long long n_newton_fail;     /* solves that hit the iteration cap unconverged */
+    long long n_depth_exceeded;  /* leaves forced by max_level */
+    long long n_cut, n_hole, n_normal;
+    long long n_ambiguous;       /* elements with |d_e - tau_cut| <= 1e-9 L_ref */
+    long long n_sign_ambiguous;  /* elements whose tied nearest faces disagree in sign */
+    long long n_seedless_components;
+    long long n_fill_conflicts;
+    long long pairs_needed;      /* pair slots S4 wanted (> max_pairs on overflow) */
+    long long queue_peak;        /* max narrow-phase queue depth seen (items) */
+    double l_ref, tau_cut, d_band;
+    float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
+                                    4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface, 7 unused */
+    int status;                  /* DC_STATUS_* bits */
+    int reserved;
+} dc_stats;
+
+/* Bytes of device scratch dc_create_grid needs for a grid of this size, up to max_faces
+ * surface faces and max_pairs candidate pairs.  Returns 0 on bad arguments. */
+size_t dc_workspace_bytes(long long n_nodes, long long n_elem, long long max_faces, long long max_pairs);
+
+/*
+ * Register the element grid ("each partition contains a unique subset of a single
+ * grid"; L233: structures that depend on the grid only are built once).  Runs S2 (conservative
+ * element boxes from the Bezier control nets) and, if adj6_dev is NULL, derives the face
+ * adjacency from shared face-centre nodes.
+ *   xyz_dev    [n_nodes][3] f64 dev      node coordinates
+ *   conn27_dev [n_elem][27] i32 dev      node ids, m = i + 3 j + 9 k
+ *   adj6_dev   [n_elem][6]  i32 dev      or NULL
+ *   workspace_dev, workspace_bytes       >= dc_workspace_bytes(...), 256-byte aligned
+ * Enqueues on `stream`; the context is usable once the stream has drained (later calls on the
+ * same stream are ordered correctly without a sync).
+ */
+int dc_create_grid(dc_ctx **out, int device,
+                   long long n_nodes, const double *xyz_dev,
+                   long long n_elem, const int *conn27_dev, const int *adj6_dev,
+                   void *workspace_dev, size_t workspace_bytes,
+                   long long max_faces, long long max_pairs, void *stream);
+
+/*
+ * Set the cutting surface (L171-L175: "each partition gathers all of its potential cutting
+ * surfaces"; L215 "outward-oriented normal").  Runs S1 (face Bezier boxes, monomial
+ * coefficients, surface AABB -> L_ref) and S3 (Morton-ordered uniform face bins).
+ *   face_nodes_dev [n_face][9][3] f64 dev, m = i + 3 j, normal x_s cross x_t points OUT of the body.
+ */
+int dc_set_cut_surface(dc_ctx *ctx, long long n_face, const double *face_nodes_dev, void *stream);
+
+/*
+ * One direct cut (S4 candidate pairs, S5 narrow phase, S6 decide, S7 flood fill; S2 too with
+ * DC_FLAG_RECOMPUTE_BOXES).  params may be NULL (all defaults).
+ *   labels_dev [n_elem] int8 dev  out    DC_HOLE / DC_NORMAL / DC_CUT   (L217 "blanking status ... saved to memory")
+ *   sdist_dev  [n_elem] f64  dev  out    signed min distance, clamped to +-d_band, 0 for CUT
+ */
+int dc_classify(dc_ctx *ctx, const dc_params *params, signed char *labels_dev, double *sdist_dev,
+                void *stream);
+
+/*
+ * End-to-end variant with HOST buffers: copies the face nodes host->device, runs
+ * dc_set_cut_surface + dc_classify, copies labels and sdist device->host, and synchronises
+ * `stream` before returning.  Host buffers should be pinned.
+ */
+int dc_classify_host(dc_ctx *ctx, const dc_params *params, long long n_face,
+                     const double *face_nodes_host, signed char *labels_host, double *sdist_host,
+                     void *stream);
+
+/* Element boxes computed by S2: copies [n_elem][6] (min xyz, max xyz) to out_dev.  For tests. */
+int dc_get_element_boxes(dc_ctx *ctx, double *out_dev, void *stream);
+
+/* Face adjacency in use (given or derived): copies [n_elem][6] i32 to out_dev.  For tests. */
+int dc_get_adjacency(dc_ctx *ctx, int *out_dev, void *stream);
+
+/* Candidate pairs of the last dc_classify: element ids and ORIGINAL face ids, up to cap pairs.
+ * Synchronises.  Returns the number of pairs (or a negative error).  For tests. */
+long long dc_get_pairs(dc_ctx *ctx, int *elem_host, int *face_host, long long cap);
+
+/* Synchronises the stream of the last call and fills *host_out. */
+int dc_get_stats(dc_ctx *ctx, dc_stats *host_out);
+
+void dc_destroy(dc_ctx *ctx);
+
+const char *dc_error_string(int code);
+
+/* FP64 FMA peak microbenchmark (register-resident DFMA chains on every SM): returns measured
+ * TFLOP/s (2 flop per FMA) or a negative error.  Used by bench.py for the "alu" roofline. */
+double dc_measure_fp64_tflops(int device, int iters);
+
+/* Library/ABI version. */
+int dc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DC_H_ */

@@ -1,0 +1,1368 @@
+// dc_kernels.cu -- libdc: direct-cut hole cutting on B200 (sm_100a).  Kernels S1..S7 + C ABI.
+//
+// Step names follow SURVEY.md 8(a) / DESIGN.md:
+//   S1 face prep      k_face_boxes, k_setup_surface
+//   S3 face bins      k_face_hist, k_cell_scan, k_face_scatter        (Morton-ordered uniform bins)
+//   S2 element boxes  k_elem_boxes                                    (HBM-bound stream)
+//   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
+//   S5 narrow phase   k_narrow (persistent CTAs, shared-memory work queues, FP64)
+//   S6 decide         fused at the end of each k_narrow batch
+//   S7 flood fill     k_uf_union, k_uf_seed, k_uf_collect, k_seedless, k_uf_assign
+//
+// PAPER.md citations are given where an operation is defined; the kernel design itself is new
+// (the paper's A.1-A.4 kernels were written for Kepler K80 and are prior art, not the blueprint).
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+
+#include "../../include/dc.h"
+#include "dc_geom.cuh"
+
+using namespace dcg;
+
+#define DC_MAX_SEEDLESS 32
+#define DC_GRID_MAX 64              /* face-bin cells per axis (Morton code: 6 bits per axis) */
+#define DC_NCELL (DC_GRID_MAX * DC_GRID_MAX * DC_GRID_MAX)
+
+// ------------------------------------------------------------------------------------------
+// device-resident scalars and counters
+struct DcScalars {
+    // reductions over the surface (ordered-uint encodings), reset by dc_set_cut_surface
+    unsigned long long node_min[3], node_max[3];   // AABB of the surface NODES -> L_ref
+    unsigned long long fbox_min[3], fbox_max[3];   // AABB of the face Bezier boxes
+    unsigned long long max_face_edge;              // max face-box edge
+    unsigned long long grid_max_diag2;             // max element-box diagonal^2 (set by S2)
+    // derived by k_setup_surface
+    double l_ref_auto;
+    double smin[3], smax[3];
+    double origin[3], cell, inv_cell, fhalf;
+    int dims[3];
+    int n_face;
+    // derived by k_setup_classify
+    double l_ref, tau, tau_exit, t_tie, d_band, reach, theta, tol_d, amb;
+    int max_level;
+    int pad0;
+    // work state
+    int n_active;
+    int work_counter;
+    int n_seedless;
+    int status;
+    unsigned long long n_pairs;
+    int seedless_elem[DC_MAX_SEEDLESS];
+    // counters
+    unsigned long long c_box_tests, c_bnb_nodes, c_newton, c_newton_iters, c_newton_fail,
+        c_depth_exceeded, c_cut, c_hole, c_normal, c_ambiguous, c_sign_ambiguous,
+        c_fill_conflicts, c_queue_peak, c_seedless_total;
+};
+
+__device__ __forceinline__ void atomic_min_d(unsigned long long *addr, double v) { atomicMin(addr, enc_ord(v)); }
+__device__ __forceinline__ void atomic_max_d(unsigned long long *addr, double v) { atomicMax(addr, enc_ord(v)); }
+
+__device__ __forceinline__ unsigned morton3(unsigned x, unsigned y, unsigned z)
+{
+    auto spread = [](unsigned v) {
+        v &= 0x3ffu;
+        v = (v | (v << 16)) & 0x030000ffu;
+        v = (v | (v << 8)) & 0x0300f00fu;
+        v = (v | (v << 4)) & 0x030c30c3u;
+        v = (v | (v << 2)) & 0x09249249u;
+        return v;
+    };
+    return spread(x) | (spread(y) << 1) | (spread(z) << 2);
+}
+
+// Bezier control values of a 1-D quadratic through nodes (-1,0,1): b0 = x0, b1 = 2 x1 - (x0+x2)/2,
+// b2 = x2 (convex-hull property => conservative boxes; Lagrange NODES do not bound the patch).
+__device__ __forceinline__ double bez_mid(double x0, double x1, double x2) { return 2.0 * x1 - 0.5 * (x0 + x2); }
+
+// ------------------------------------------------------------------------------------------
+// S1: per-face Bezier box + surface reductions.  face_nodes [n_face][9][3].
+__global__ void k_face_boxes(DcScalars *S, const double *__restrict__ face_nodes, int n_face,
+                             double *__restrict__ fbox_orig /*[n_face][6]*/)
+{
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    double lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
+    double nlo[3] = { INFINITY, INFINITY, INFINITY }, nhi[3] = { -INFINITY, -INFINITY, -INFINITY };
+    double edge = 0.0;
+    if (f < n_face) {
+        const double *X = face_nodes + (size_t)f * 27;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double x[9], b[9];
+#pragma unroll
+            for (int m = 0; m < 9; ++m) { x[m] = __ldg(X + 3 * m + c); nlo[c] = fmin(nlo[c], x[m]); nhi[c] = fmax(nhi[c], x[m]); }
+#pragma unroll
+            for (int j = 0; j < 3; ++j) { b[3*j] = x[3*j]; b[3*j+1] = bez_mid(x[3*j], x[3*j+1], x[3*j+2]); b[3*j+2] = x[3*j+2]; }
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { const double m1 = bez_mid(b[i], b[i+3], b[i+6]); b[i+3] = m1; }
+#pragma unroll
+            for (int m = 0; m < 9; ++m) { lo[c] = fmin(lo[c], b[m]); hi[c] = fmax(hi[c], b[m]); }
+            fbox_orig[(size_t)f * 6 + c] = lo[c];
+            fbox_orig[(size_t)f * 6 + 3 + c] = hi[c];
+            edge = fmax(edge, hi[c] - lo[c]);
+        }
+    }
+    // warp reduce then one atomic per warp
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            lo[c] = fmin(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o));
+            hi[c] = fmax(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
+            nlo[c] = fmin(nlo[c], __shfl_xor_sync(0xffffffffu, nlo[c], o));
+            nhi[c] = fmax(nhi[c], __shfl_xor_sync(0xffffffffu, nhi[c], o));
+        }
+        edge = fmax(edge, __shfl_xor_sync(0xffffffffu, edge, o));
+    }
+    if ((threadIdx.x & 31) == 0 && lo[0] != INFINITY) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            atomic_min_d(&S->fbox_min[c], lo[c]); atomic_max_d(&S->fbox_max[c], hi[c]);
+            atomic_min_d(&S->node_min[c], nlo[c]); atomic_max_d(&S->node_max[c], nhi[c]);
+        }
+        atomic_max_d(&S->max_face_edge, edge);
+    }
+}
+
+__global__ void k_reset_surface(DcScalars *S)
+{
+    for (int c = 0; c < 3; ++c) {
+        S->node_min[c] = S->fbox_min[c] = ~0ull;
+        S->node_max[c] = S->fbox_max[c] = 0ull;
+    }
+    S->max_face_edge = 0ull;
+}
+
+__global__ void k_setup_surface(DcScalars *S, int n_face)
+{
+    double ext = 0.0, lref = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        S->smin[c] = dec_ord(S->fbox_min[c]); S->smax[c] = dec_ord(S->fbox_max[c]);
+        ext = fmax(ext, S->smax[c] - S->smin[c]);
+        lref = fmax(lref, dec_ord(S->node_max[c]) - dec_ord(S->node_min[c]));
+    }
+    S->l_ref_auto = lref;
+    const double edge = dec_ord(S->max_face_edge);
+    double cell = fmax(edge, ext / DC_GRID_MAX) * (1.0 + 1e-9);
+    if (!(cell > 0.0)) cell = 1.0;
+    S->cell = cell; S->inv_cell = 1.0 / cell; S->fhalf = 0.5 * edge;
+    for (int c = 0; c < 3; ++c) {
+        S->origin[c] = S->smin[c];
+        int d = (int)floor((S->smax[c] - S->smin[c]) * S->inv_cell) + 1;
+        S->dims[c] = d < 1 ? 1 : (d > DC_GRID_MAX ? DC_GRID_MAX : d);
+    }
+    S->n_face = n_face;
+}
+
+__device__ __forceinline__ int cell_coord(const DcScalars *S, double x, int c)
+{
+    int i = (int)floor((x - S->origin[c]) * S->inv_cell);
+    return i < 0 ? 0 : (i >= S->dims[c] ? S->dims[c] - 1 : i);
+}
+
+// S3: histogram of faces over cells keyed by the Morton code of the box-centre cell
+__global__ void k_face_hist(const DcScalars *S, const double *__restrict__ fbox_orig, int n_face,
+                            int *__restrict__ fcell, int *cell_count)
+{
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_face) return;
+    int ic[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        ic[c] = cell_coord(S, 0.5 * (fbox_orig[(size_t)f * 6 + c] + fbox_orig[(size_t)f * 6 + 3 + c]), c);
+    const int code = (int)morton3(ic[0], ic[1], ic[2]);
+    fcell[f] = code;
+    atomicAdd(&cell_count[code], 1);
+}
+
+// exclusive scan over DC_NCELL cells by one CTA of 1024 threads (256 cells per thread)
+__global__ void __launch_bounds__(1024) k_cell_scan(const int *__restrict__ cell_count, int *__restrict__ cell_start)
+{
+    __shared__ int s_part[1024];
+    const int per = DC_NCELL / 1024;
+    const int t = threadIdx.x;
+    int sum = 0;
+    for (int i = 0; i < per; ++i) sum += cell_count[t * per + i];
+    s_part[t] = sum;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+        int v = t >= o ? s_part[t - o] : 0;
+        __syncthreads();
+        s_part[t] += v;
+        __syncthreads();
+    }
+    int run = s_part[t] - sum;
+    for (int i = 0; i < per; ++i) { cell_start[t * per + i] = run; run += cell_count[t * per + i]; }
+    if (t == 1023) cell_start[DC_NCELL] = run;
+}
+
+// scatter faces into cell order; write sorted boxes and monomial coefficients (stride 28 doubles)
+__global__ void k_face_scatter(const double *__restrict__ face_nodes, const double *__restrict__ fbox_orig,
+                               const int *__restrict__ fcell, const int *__restrict__ cell_start,
+                               int *cell_fill, int n_face, int *__restrict__ fperm,
+                               double *__restrict__ fbox, double *__restrict__ fcoef)
+{
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_face) return;
+    const int code = fcell[f];
+    const int pos = cell_start[code] + atomicAdd(&cell_fill[code], 1);
+    fperm[pos] = f;
+#pragma unroll
+    for (int m = 0; m < 6; ++m) fbox[(size_t)pos * 6 + m] = fbox_orig[(size_t)f * 6 + m];
+    const double *X = face_nodes + (size_t)f * 27;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double x[9], a[9];
+#pragma unroll
+        for (int m = 0; m < 9; ++m) x[m] = __ldg(X + 3 * m + c);
+        nodes_to_mono9(x, a);
+#pragma unroll
+        for (int m = 0; m < 9; ++m) fcoef[(size_t)pos * 28 + c * 9 + m] = a[m];
+    }
+    fcoef[(size_t)pos * 28 + 27] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------
+// S2: conservative element boxes from the 26 boundary control points of the Bezier net.
+// One thread per element; conn rows are staged through shared memory so the global reads
+// are fully coalesced.  ebox is SoA: ebox[c*n_elem + e] (c = 0..5: min xyz, max xyz).
+#define EB_THREADS 128
+__global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const double *__restrict__ xyz,
+                                                           const int *__restrict__ conn, long long n_elem,
+                                                           double *__restrict__ ebox)
+{
+    __shared__ int s_conn[EB_THREADS * 27];
+    const long long e0 = (long long)blockIdx.x * EB_THREADS;
+    const int nloc = (int)min((long long)EB_THREADS, n_elem - e0);
+    for (int i = threadIdx.x; i < nloc * 27; i += EB_THREADS) s_conn[i] = __ldg(conn + e0 * 27 + i);
+    __syncthreads();
+    double diag2 = 0.0;
+    if (threadIdx.x < nloc) {
+        const long long e = e0 + threadIdx.x;
+        const int *cn = s_conn + threadIdx.x * 27;
+        double ext2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double b[27];
+#pragma unroll
+            for (int m = 0; m < 27; ++m) b[m] = __ldg(xyz + (size_t)cn[m] * 3 + c);
+            // Lagrange -> Bezier along i, then j, then k (only the middle layer of each line changes)
+#pragma unroll
+            for (int m = 0; m < 9; ++m) b[3*m+1] = bez_mid(b[3*m], b[3*m+1], b[3*m+2]);
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+#pragma unroll
+                for (int i = 0; i < 3; ++i) b[i+3+9*k] = bez_mid(b[i+9*k], b[i+3+9*k], b[i+6+9*k]);
+#pragma unroll
+            for (int m = 0; m < 9; ++m) b[m+9] = bez_mid(b[m], b[m+9], b[m+18]);
+            double lo = INFINITY, hi = -INFINITY;
+#pragma unroll
+            for (int m = 0; m < 27; ++m) if (m != 13) { lo = fmin(lo, b[m]); hi = fmax(hi, b[m]); }
+            ebox[(size_t)c * n_elem + e] = lo;
+            ebox[(size_t)(3 + c) * n_elem + e] = hi;
+            ext2 = fma(hi - lo, hi - lo, ext2);
+        }
+        diag2 = ext2;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) diag2 = fmax(diag2, __shfl_xor_sync(0xffffffffu, diag2, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(&S->grid_max_diag2, (unsigned long long)__double_as_longlong(diag2));
+}
+
+// ------------------------------------------------------------------------------------------
+// adjacency from shared face-centre nodes (only when the caller passes adj6 = NULL)
+__constant__ int c_face_centre[6] = { 12, 14, 10, 16, 4, 22 };
+__global__ void k_adj_pass1(const int *__restrict__ conn, long long n_elem, int *first, int *second)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_elem * 6) return;
+    const long long e = t / 6; const int k = (int)(t % 6);
+    const int c = conn[e * 27 + c_face_centre[k]];
+    const int code = (int)t;
+    const int old = atomicCAS(&first[c], -1, code);
+    if (old != -1) second[c] = code;
+}
+__global__ void k_adj_pass2(const int *__restrict__ conn, long long n_elem, const int *__restrict__ first,
+                            const int *__restrict__ second, int *__restrict__ adj)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_elem * 6) return;
+    const long long e = t / 6; const int k = (int)(t % 6);
+    const int c = conn[e * 27 + c_face_centre[k]];
+    const int a = first[c], b = second[c];
+    const int other = (a == (int)t) ? b : a;
+    adj[t] = other < 0 ? -1 : other / 6;
+}
+
+// ------------------------------------------------------------------------------------------
+// per-classify scalar setup
+__global__ void k_setup_classify(DcScalars *S, dc_params P)
+{
+    const double lref = P.l_ref > 0.0 ? P.l_ref : S->l_ref_auto;
+    S->l_ref = lref;
+    S->tau = (P.tau_cut_rel > 0.0 ? P.tau_cut_rel : 1e-7) * lref;
+    S->amb = 1e-9 * lref;
+    S->tau_exit = S->tau - S->amb;
+    S->t_tie = 1e-9 * lref;
+    S->tol_d = 1e-13 * lref;
+    S->d_band = P.d_band > 0.0 ? P.d_band : sqrt(__longlong_as_double((long long)S->grid_max_diag2));
+    S->reach = S->d_band + 2.0 * S->tau + S->t_tie;
+    S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.125;
+    S->max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
+    S->n_active = 0; S->work_counter = 0; S->n_seedless = 0; S->status = 0; S->n_pairs = 0ull;
+    S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
+    S->c_depth_exceeded = S->c_cut = S->c_hole = S->c_normal = S->c_ambiguous = 0ull;
+    S->c_sign_ambiguous = S->c_fill_conflicts = S->c_queue_peak = S->c_seedless_total = 0ull;
+}
+
+// ------------------------------------------------------------------------------------------
+// S4a: one thread per element.  Initialises the per-element state of this cut and appends the
+// elements whose inflated box overlaps a non-empty face cell to the active list
+// (warp-aggregated atomic append).
+__global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
+                         signed char *__restrict__ labels, int *__restrict__ parent,
+                         unsigned char *__restrict__ comp, const int *__restrict__ cell_count,
+                         int *__restrict__ act_elem)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    bool active = false;
+    if (e < n_elem) {
+        labels[e] = -1; parent[e] = (int)e; comp[e] = 0;
+        double lo[3], hi[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e]; }
+        double d2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double g = fmax(0.0, fmax(S->smin[c] - hi[c], lo[c] - S->smax[c]));
+            d2 = fma(g, g, d2);
+        }
+        const double reach = S->reach;
+        if (d2 <= reach * reach) {
+            const double pad = reach + S->fhalf;
+            int i0[3], i1[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c); }
+            for (int z = i0[2]; z <= i1[2] && !active; ++z)
+                for (int y = i0[1]; y <= i1[1] && !active; ++y)
+                    for (int x = i0[0]; x <= i1[0]; ++x)
+                        if (__ldg(cell_count + morton3(x, y, z)) > 0) { active = true; break; }
+        }
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, active);
+    if (m) {
+        const int lane = threadIdx.x & 31;
+        int base = 0;
+        if (lane == (__ffs(m) - 1)) base = atomicAdd(&S->n_active, __popc(m));
+        base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+        if (active) act_elem[base + __popc(m & ((1u << lane) - 1))] = (int)e;
+    }
+}
+
+// S4b: one warp per active element: box test (Algorithm A.2) against the
+// faces of the cells its inflated box overlaps; count, reserve a contiguous segment with one
+// atomic per element, then write.  pair_key is initialised to +inf for S5.
+__device__ __forceinline__ bool box_within(const double *lo, const double *hi, const double *fb, double reach2)
+{
+    double d2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double g = fmax(0.0, fmax(fb[c] - hi[c], lo[c] - fb[3 + c]));
+        d2 = fma(g, g, d2);
+    }
+    return d2 <= reach2;
+}
+
+__global__ void __launch_bounds__(256) k_pairs(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
+                                               const int *__restrict__ act_elem, const int *__restrict__ cell_start,
+                                               const double *__restrict__ fbox, long long max_pairs,
+                                               long long *__restrict__ act_start, int *__restrict__ act_cnt,
+                                               int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int n_active = S->n_active;
+    const double reach = S->reach, reach2 = reach * reach, pad = reach + S->fhalf;
+    unsigned long long tests = 0;
+    for (int a = warp; a < n_active; a += nwarps) {
+        const long long e = act_elem[a];
+        double lo[3], hi[3];
+        int i0[3], i1[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e];
+            i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c);
+        }
+        const int nx = i1[0] - i0[0] + 1, ny = i1[1] - i0[1] + 1, nz = i1[2] - i0[2] + 1;
+        const int ncell = nx * ny * nz;
+        long long base = 0;
+        int my_off = 0;
+        for (int pass = 0; pass < 2; ++pass) {
+            int cnt = 0;
+            for (int ci = lane; ci < ncell; ci += 32) {
+                const int x = i0[0] + ci % nx, y = i0[1] + (ci / nx) % ny, z = i0[2] + ci / (nx * ny);
+                const unsigned code = morton3(x, y, z);
+                const int s = __ldg(cell_start + code), t = __ldg(cell_start + code + 1);
+                for (int p = s; p < t; ++p) {
+                    double fb[6];
+#pragma unroll
+                    for (int m = 0; m < 6; ++m) fb[m] = __ldg(fbox + (size_t)p * 6 + m);
+                    if (pass == 0) ++tests;
+                    if (box_within(lo, hi, fb, reach2)) {
+                        if (pass == 1) {
+                            pair_face[base + my_off + cnt] = p;
+                            pair_key[base + my_off + cnt] = 0x7ff0000000000000ull;
+                        }
+                        ++cnt;
+                    }
+                }
+            }
+            if (pass == 0) {
+                // warp exclusive scan of cnt
+                int incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+                const int total = __shfl_sync(0xffffffffu, incl, 31);
+                my_off = incl - cnt;
+                if (lane == 0) {
+                    long long b = (long long)atomicAdd(&S->n_pairs, (unsigned long long)total);
+                    if (b + total > max_pairs) { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
+                    act_start[a] = b < 0 ? 0 : b;
+                    act_cnt[a] = b < 0 ? 0 : total;
+                    base = b;
+                }
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (base < 0 || total == 0) break;
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(0xffffffffu, tests, o);
+    if (lane == 0 && tests) atomicAdd(&S->c_box_tests, tests);
+}
+
+// ------------------------------------------------------------------------------------------
+// S5 + S6: narrow phase.
+#define NP_THREADS 128
+#define NP_BE 16            /* elements per batch */
+#define NP_QCAP 2048        /* shared-memory stack items */
+#define NP_NQCAP 384        /* Newton queue items (< 2 * NP_THREADS always) */
+#define NP_SPILL 8192       /* global spill items per CTA */
+#define NP_NEWTON_ITERS 40
+
+struct __align__(16) Item { unsigned f, w1, w2, w3; };
+// w1: slot(5) | k(3)<<5 | pair_local(24)<<8
+// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20
+// w3: is(12) | it(12)<<12 | flags(8)<<24      flags bit0: seed solve (no re-split on failure)
+
+__constant__ int c_face_node[6][9] = {
+    { 0, 3, 6, 9, 12, 15, 18, 21, 24 },      // xi = -1 : (a,b) = (j,k)
+    { 2, 5, 8, 11, 14, 17, 20, 23, 26 },     // xi = +1
+    { 0, 1, 2, 9, 10, 11, 18, 19, 20 },      // eta = -1 : (a,b) = (i,k)
+    { 6, 7, 8, 15, 16, 17, 24, 25, 26 },     // eta = +1
+    { 0, 1, 2, 3, 4, 5, 6, 7, 8 },           // zeta = -1 : (a,b) = (i,j)
+    { 18, 19, 20, 21, 22, 23, 24, 25, 26 },  // zeta = +1
+};
+
+struct NarrowShared {
+    double ecoef[NP_BE][6][27];
+    double nodes[NP_THREADS / 32][27 * 3];
+    Item stack[NP_QCAP];
+    Item newton[NP_NQCAP];
+    unsigned long long best[NP_BE], dmin[NP_BE], seed[NP_BE];
+    long long pstart[NP_BE];
+    int elem[NP_BE], pcnt[NP_BE], poff[NP_BE + 1], cut[NP_BE];
+    int top, ntop, batch, nslots, peak;
+};
+
+struct Cnt { unsigned nodes, newton, iters, fail, depth; };
+
+__device__ __forceinline__ double u2d(unsigned long long b) { return __longlong_as_double((long long)b); }
+__device__ __forceinline__ unsigned long long d2u(double d) { return (unsigned long long)__double_as_longlong(d); }
+
+__device__ __forceinline__ void stack_push(NarrowShared &sh, Item *spill, DcScalars *S, const Item *it, int n)
+{
+    const int idx = atomicAdd(&sh.top, n);
+    for (int i = 0; i < n; ++i) {
+        const int j = idx + i;
+        if (j < NP_QCAP) sh.stack[j] = it[i];
+        else if (j - NP_QCAP < NP_SPILL) spill[j - NP_QCAP] = it[i];
+        else atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW);
+    }
+}
+
+__device__ __forceinline__ void item_box(const Item &it, double &uc, double &vc, double &hP,
+                                         double &sc, double &tc, double &hQ)
+{
+    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+    const int iu = (it.w2 >> 8) & 0xfff, iv = (it.w2 >> 20) & 0xfff;
+    const int is = it.w3 & 0xfff, itt = (it.w3 >> 12) & 0xfff;
+    hP = __longlong_as_double((long long)(1023 - lP) << 52);
+    hQ = __longlong_as_double((long long)(1023 - lQ) << 52);
+    uc = fma((double)(2 * iu + 1), hP, -1.0); vc = fma((double)(2 * iv + 1), hP, -1.0);
+    sc = fma((double)(2 * is + 1), hQ, -1.0); tc = fma((double)(2 * itt + 1), hQ, -1.0);
+}
+
+__device__ __forceinline__ void make_children(const Item &it, bool splitP, Item *ch)
+{
+    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+    const int iu = (it.w2 >> 8) & 0xfff, iv = (it.w2 >> 20) & 0xfff;
+    const int is = it.w3 & 0xfff, itt = (it.w3 >> 12) & 0xfff;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        ch[c].f = it.f; ch[c].w1 = it.w1;
+        if (splitP) {
+            ch[c].w2 = (unsigned)(lP + 1) | ((unsigned)lQ << 4) | ((unsigned)(2 * iu + (c & 1)) << 8) | ((unsigned)(2 * iv + (c >> 1)) << 20);
+            ch[c].w3 = it.w3 & 0x00ffffffu;
+        } else {
+            ch[c].w2 = (unsigned)lP | ((unsigned)(lQ + 1) << 4) | ((unsigned)iu << 8) | ((unsigned)iv << 20);
+            ch[c].w3 = (unsigned)(2 * is + (c & 1)) | ((unsigned)(2 * itt + (c >> 1)) << 12);
+        }
+    }
+}
+
+// one branch-and-bound node: bound, prune / split / hand over to Newton
+__device__ __forceinline__ void bnb_process(NarrowShared &sh, Item *spill, DcScalars *S, const double *__restrict__ fcoef,
+                                            const Item &it, Cnt &cnt, double t_tie, double tau_exit, double theta, int max_level)
+{
+    const int slot = it.w1 & 31, k = (it.w1 >> 5) & 7;
+    if (sh.cut[slot]) return;
+    double uc, vc, hP, sc, tc, hQ;
+    item_box(it, uc, vc, hP, sc, tc, hQ);
+    const double *AP = &sh.ecoef[slot][k][0];
+    const double *AQ = fcoef + (size_t)it.f * 28;
+    const NodeBound nb = bound_subpair([&](int m) { return AP[m]; }, [&](int m) { return __ldg(AQ + m); },
+                                       uc, vc, hP, sc, tc, hQ);
+    cnt.nodes++;
+    double best = u2d(sh.best[slot]);
+    if (nb.dist_c < best) { atomicMin(&sh.best[slot], d2u(nb.dist_c)); best = nb.dist_c; }
+    if (nb.dist_c <= tau_exit) { sh.cut[slot] = 1; return; }
+    if (nb.lb > best + t_tie) return;
+    const double kP = nb.s1P > 0.0 ? nb.s2P / (nb.s1P * nb.s1P) : 0.0;
+    const double kQ = nb.s1Q > 0.0 ? nb.s2Q / (nb.s1Q * nb.s1Q) : 0.0;
+    bool leaf = fmax(kP, kQ) * fmax(nb.s1P, nb.s1Q) <= theta;
+    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+    bool splitP = nb.s1P >= nb.s1Q;
+    if (!leaf) {
+        if (splitP && lP >= max_level) splitP = false;
+        if (!splitP && lQ >= max_level) {
+            if (lP < max_level) splitP = true;
+            else { leaf = true; cnt.depth++; }
+        }
+    }
+    if (leaf) {
+        const int idx = atomicAdd(&sh.ntop, 1);
+        sh.newton[idx] = it;
+    } else {
+        Item ch[4];
+        make_children(it, splitP, ch);
+        stack_push(sh, spill, S, ch, 4);
+    }
+}
+
+__device__ __forceinline__ void newton_process(NarrowShared &sh, Item *spill, DcScalars *S, const double *__restrict__ fcoef,
+                                               unsigned long long *__restrict__ pair_key, const Item &it, Cnt &cnt,
+                                               double tol_d, double tau_exit, int max_level)
+{
+    const int slot = it.w1 & 31, k = (it.w1 >> 5) & 7;
+    if (sh.cut[slot]) return;
+    double uc, vc, hP, sc, tc, hQ;
+    item_box(it, uc, vc, hP, sc, tc, hQ);
+    double CP[27], CQ[27];
+    const double *AP = &sh.ecoef[slot][k][0];
+    const double *AQ = fcoef + (size_t)it.f * 28;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double A[9];
+#pragma unroll
+        for (int m = 0; m < 9; ++m) A[m] = AP[c * 9 + m];
+        recentre9(A, uc, vc, hP, hP, CP + 9 * c);
+#pragma unroll
+        for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
+        recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
+    }
+    const NewtonOut o = newton_leaf(CP, CQ, tol_d, tau_exit, NP_NEWTON_ITERS);
+    cnt.newton++; cnt.iters += o.iters;
+    if (o.dist <= tau_exit) { sh.cut[slot] = 1; return; }
+    atomicMin(&sh.best[slot], d2u(o.dist));
+    atomicMin(&sh.dmin[slot], d2u(o.dist));
+    const unsigned long long key = (d2u(o.dist) & ~0xffull) | (unsigned long long)cos_code(o.cosv);
+    atomicMin(&pair_key[sh.pstart[slot] + (it.w1 >> 8)], key);
+    if (!o.converged) {
+        const bool seed = (it.w3 >> 24) & 1;
+        const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+        if (!seed) {
+            cnt.fail++;
+            bool splitP = hP >= hQ;
+            if (splitP && lP >= max_level) splitP = false;
+            if (!splitP && lQ >= max_level) { if (lP < max_level) splitP = true; else return; }
+            Item ch[4];
+            make_children(it, splitP, ch);
+            stack_push(sh, spill, S, ch, 4);
+        }
+    }
+}
+
+__device__ __forceinline__ Item stack_get(NarrowShared &sh, const Item *spill, int j)
+{
+    return j < NP_QCAP ? sh.stack[j] : spill[j - NP_QCAP];
+}
+
+__global__ void __launch_bounds__(NP_THREADS) k_narrow(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
+                                                       const int *__restrict__ act_elem, const long long *__restrict__ act_start,
+                                                       const int *__restrict__ act_cnt, const int *__restrict__ pair_face,
+                                                       unsigned long long *__restrict__ pair_key, const double *__restrict__ fcoef,
+                                                       Item *__restrict__ spill_all, signed char *__restrict__ labels,
+                                                       double *__restrict__ sdist)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    NarrowShared &sh = *reinterpret_cast<NarrowShared *>(smem_raw);
+    Item *spill = spill_all + (size_t)blockIdx.x * NP_SPILL;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_active = S->n_active;
+    const double t_tie = S->t_tie, tau = S->tau, tau_exit = S->tau_exit, theta = S->theta, tol_d = S->tol_d;
+    const double d_band = S->d_band, amb = S->amb;
+    const int max_level = S->max_level;
+    const double init_best = S->reach;
+    Cnt cnt = { 0, 0, 0, 0, 0 };
+    unsigned n_amb = 0, n_samb = 0;
+    if (tid == 0) sh.peak = 0;
+
+    // drain both queues (bulk-synchronous rounds; Newton rounds when a full round is available)
+    auto drain = [&]() {
+        while (true) {
+            __syncthreads();
+            const int nt = sh.ntop, bt = sh.top;
+            if (nt == 0 && bt == 0) break;
+            const bool do_newton = (nt >= NP_THREADS) || (bt == 0);
+            __syncthreads();
+            Item it; bool have = false;
+            if (do_newton) {
+                const int take = min(nt, NP_THREADS);
+                if (tid < take) { it = sh.newton[nt - take + tid]; have = true; }
+                if (tid == 0) sh.ntop = nt - take;
+            } else {
+                const int take = min(bt, NP_THREADS);
+                if (tid < take) { it = stack_get(sh, spill, bt - take + tid); have = true; }
+                if (tid == 0) { sh.top = bt - take; if (bt > sh.peak) sh.peak = bt; }
+            }
+            __syncthreads();
+            if (have) {
+                if (do_newton) newton_process(sh, spill, S, fcoef, pair_key, it, cnt, tol_d, tau_exit, max_level);
+                else bnb_process(sh, spill, S, fcoef, it, cnt, t_tie, tau_exit, theta, max_level);
+            }
+        }
+    };
+
+    while (true) {
+        __syncthreads();
+        if (tid == 0) {
+            sh.batch = atomicAdd(&S->work_counter, 1);
+            sh.top = 0; sh.ntop = 0;
+        }
+        __syncthreads();
+        const int first = sh.batch * NP_BE;
+        if (first >= n_active) break;
+        const int nslots = min(NP_BE, n_active - first);
+        // ---- stage the batch: conn row (coalesced), nodes, monomial coefficients of the 6 boundary patches
+        for (int slot = warp; slot < nslots; slot += NP_THREADS / 32) {
+            const int e = act_elem[first + slot];
+            double *nd = sh.nodes[warp];
+            if (lane < 27) {
+                const int id = __ldg(conn + (size_t)e * 27 + lane);
+                const double *p = xyz + (size_t)id * 3;
+                nd[lane * 3 + 0] = __ldg(p); nd[lane * 3 + 1] = __ldg(p + 1); nd[lane * 3 + 2] = __ldg(p + 2);
+            }
+            __syncwarp();
+            if (lane < 18) {
+                const int k = lane / 3, c = lane % 3;
+                double x[9], a[9];
+#pragma unroll
+                for (int m = 0; m < 9; ++m) x[m] = nd[c_face_node[k][m] * 3 + c];
+                nodes_to_mono9(x, a);
+#pragma unroll
+                for (int m = 0; m < 9; ++m) sh.ecoef[slot][k][c * 9 + m] = a[m];
+            }
+            if (lane == 0) {
+                sh.elem[slot] = e; sh.pstart[slot] = act_start[first + slot]; sh.pcnt[slot] = act_cnt[first + slot];
+                sh.best[slot] = d2u(init_best); sh.dmin[slot] = 0x7ff0000000000000ull; sh.seed[slot] = ~0ull; sh.cut[slot] = 0;
+            }
+            __syncwarp();
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int run = 0;
+            for (int s = 0; s < nslots; ++s) { sh.poff[s] = run; run += sh.pcnt[s]; }
+            sh.poff[nslots] = run; sh.nslots = nslots;
+        }
+        __syncthreads();
+        const int total = sh.poff[nslots] * 6;
+        // ---- seeding: centre-centre distances (attained) -> first upper bound, best (pair,k) per element
+        for (int t = tid; t < total; t += NP_THREADS) {
+            const int pl = t / 6, k = t - pl * 6;
+            int slot = 0;
+            while (pl >= sh.poff[slot + 1]) ++slot;
+            const int f = pair_face[sh.pstart[slot] + (pl - sh.poff[slot])];
+            const double *AP = &sh.ecoef[slot][k][0];
+            const double *AQ = fcoef + (size_t)f * 28;
+            const double dx = AP[0] - __ldg(AQ), dy = AP[9] - __ldg(AQ + 9), dz = AP[18] - __ldg(AQ + 18);
+            const double d = sqrt(dx * dx + dy * dy + dz * dz);
+            atomicMin(&sh.best[slot], d2u(d));
+            const unsigned long long sk = ((unsigned long long)__float_as_uint((float)d) << 32) | (unsigned)t;
+            atomicMin(&sh.seed[slot], sk);
+        }
+        __syncthreads();
+        if (tid < nslots && sh.seed[tid] != ~0ull) {
+            const int t = (int)(sh.seed[tid] & 0xffffffffu);
+            const int pl = t / 6, k = t - pl * 6;
+            Item it;
+            it.f = (unsigned)pair_face[sh.pstart[tid] + (pl - sh.poff[tid])];
+            it.w1 = (unsigned)tid | ((unsigned)k << 5) | ((unsigned)(pl - sh.poff[tid]) << 8);
+            it.w2 = 0; it.w3 = 1u << 24;
+            const int idx = atomicAdd(&sh.ntop, 1);
+            sh.newton[idx] = it;
+        }
+        drain();
+        // ---- roots: every (pair, boundary patch) is bounded; survivors enter the queues
+        for (int base = 0; base < total; base += NP_THREADS) {
+            const int t = base + tid;
+            if (t < total) {
+                const int pl = t / 6, k = t - pl * 6;
+                int slot = 0;
+                while (pl >= sh.poff[slot + 1]) ++slot;
+                Item it;
+                it.f = (unsigned)pair_face[sh.pstart[slot] + (pl - sh.poff[slot])];
+                it.w1 = (unsigned)slot | ((unsigned)k << 5) | ((unsigned)(pl - sh.poff[slot]) << 8);
+                it.w2 = 0; it.w3 = 0;
+                bnb_process(sh, spill, S, fcoef, it, cnt, t_tie, tau_exit, theta, max_level);
+            }
+            __syncthreads();
+            if (sh.top > NP_QCAP / 2 || sh.ntop >= NP_THREADS) drain();
+        }
+        drain();
+        // ---- S6: decide (nearest face, dot with its outward normal; ties L294)
+        if (tid < nslots) {
+            const int slot = tid;
+            const int e = sh.elem[slot];
+            const double dmin = u2d(sh.dmin[slot]);
+            if (sh.cut[slot]) { labels[e] = DC_CUT; sdist[e] = 0.0; }
+            else if (dmin <= tau) { labels[e] = DC_CUT; sdist[e] = 0.0; if (dmin >= tau - amb) ++n_amb; }
+            else if (dmin < INFINITY) {
+                if (dmin <= tau + amb) ++n_amb;
+                int bestmag = -1, neg = 0, npos = 0, nneg = 0;
+                const long long p0 = sh.pstart[slot];
+                for (int p = 0; p < sh.pcnt[slot]; ++p) {
+                    const unsigned long long key = __ldcg(pair_key + p0 + p);
+                    const double dk = u2d(key & ~0xffull);
+                    if (dk <= dmin + t_tie) {
+                        const int code = (int)(key & 0xff), mag = code & 0x7f, ng = code >> 7;
+                        if (ng) ++nneg; else ++npos;
+                        if (mag > bestmag) { bestmag = mag; neg = ng; }
+                    }
+                }
+                if (npos && nneg) ++n_samb;
+                labels[e] = neg ? DC_HOLE : DC_NORMAL;
+                const double d = fmin(dmin, d_band);
+                sdist[e] = neg ? -d : d;
+            }
+        }
+    }
+    // ---- counters
+    unsigned v[7] = { cnt.nodes, cnt.newton, cnt.iters, cnt.fail, cnt.depth, n_amb, n_samb };
+#pragma unroll
+    for (int i = 0; i < 7; ++i)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    if (lane == 0) {
+        if (v[0]) atomicAdd(&S->c_bnb_nodes, (unsigned long long)v[0]);
+        if (v[1]) atomicAdd(&S->c_newton, (unsigned long long)v[1]);
+        if (v[2]) atomicAdd(&S->c_newton_iters, (unsigned long long)v[2]);
+        if (v[3]) atomicAdd(&S->c_newton_fail, (unsigned long long)v[3]);
+        if (v[4]) atomicAdd(&S->c_depth_exceeded, (unsigned long long)v[4]);
+        if (v[5]) atomicAdd(&S->c_ambiguous, (unsigned long long)v[5]);
+        if (v[6]) atomicAdd(&S->c_sign_ambiguous, (unsigned long long)v[6]);
+    }
+    __syncthreads();
+    if (tid == 0) atomicMax(&S->c_queue_peak, (unsigned long long)sh.peak);
+}
+
+// ------------------------------------------------------------------------------------------
+// S7: flood fill = connected components of the face-adjacency graph of non-CUT elements
+// (lock-free union-find), seeded by the signs found in S5/S6 (the classical paint-fill,
+// PAPER.md L143 / Fig. 5c, without its O(diameter) sweeps).
+__device__ __forceinline__ int uf_find(int *parent, int x)
+{
+    volatile int *P = parent;
+    while (true) {
+        const int p = P[x];
+        if (p == x) return x;
+        const int gp = P[p];
+        if (gp != p) P[x] = gp;   // path halving (benign race: always points to an ancestor)
+        x = p;
+    }
+}
+__device__ __forceinline__ void uf_union(int *parent, int a, int b)
+{
+    while (true) {
+        a = uf_find(parent, a); b = uf_find(parent, b);
+        if (a == b) return;
+        if (a < b) { const int t = a; a = b; b = t; }
+        if (atomicCAS(&parent[a], a, b) == a) return;   // hook the larger root under the smaller
+    }
+}
+
+__global__ void k_uf_union(const signed char *__restrict__ labels, const int *__restrict__ adj, long long n_elem, int *parent)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elem || labels[e] == DC_CUT) return;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const int nb = __ldg(adj + e * 6 + k);
+        if (nb >= 0 && nb < e && labels[nb] != DC_CUT) uf_union(parent, (int)e, nb);
+    }
+}
+
+__global__ void k_uf_seed(const signed char *__restrict__ labels, long long n_elem, int *parent, unsigned char *comp)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elem) return;
+    const int lab = labels[e];
+    if (lab == DC_CUT) return;
+    const int r = uf_find(parent, (int)e);
+    parent[e] = r;
+    if (lab == DC_HOLE || lab == DC_NORMAL) {
+        // byte-wide OR through a 32-bit atomic
+        unsigned *w = reinterpret_cast<unsigned *>(comp + (r & ~3));
+        atomicOr(w, (unsigned)(lab == DC_HOLE ? 1 : 2) << (8 * (r & 3)));
+    }
+}
+
+__global__ void k_uf_collect(DcScalars *S, const signed char *__restrict__ labels, long long n_elem,
+                             const int *__restrict__ parent, const unsigned char *__restrict__ comp)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elem) return;
+    if (labels[e] != DC_CUT && parent[e] == (int)e && comp[e] == 0) {
+        const int i = atomicAdd(&S->n_seedless, 1);
+        if (i < DC_MAX_SEEDLESS) S->seedless_elem[i] = (int)e;
+        else atomicOr(&S->status, DC_STATUS_SEEDLESS_OVERFLOW);
+    }
+}
+
+// A component no band element touches (surface misses the grid, or a pocket cut off by the grid
+// boundary): one exhaustive nearest-face query for its representative element (SURVEY 8(a) note iii).
+// One CTA per component; each thread runs a private depth-first branch and bound per (face, patch).
+#define SL_THREADS 256
+__global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
+                                                         const double *__restrict__ fcoef, int n_face, unsigned char *comp)
+{
+    __shared__ double s_ecoef[6][27];
+    __shared__ double s_nodes[81];
+    __shared__ unsigned long long s_best;
+    __shared__ double s_d[SL_THREADS], s_c[SL_THREADS];
+    const int ns = min(S->n_seedless, DC_MAX_SEEDLESS);
+    if ((int)blockIdx.x >= ns) return;
+    const int e = S->seedless_elem[blockIdx.x];
+    const int tid = threadIdx.x;
+    if (tid < 27) {
+        const int id = conn[(size_t)e * 27 + tid];
+        for (int c = 0; c < 3; ++c) s_nodes[tid * 3 + c] = xyz[(size_t)id * 3 + c];
+    }
+    if (tid == 0) s_best = 0x7ff0000000000000ull;
+    __syncthreads();
+    if (tid < 18) {
+        const int k = tid / 3, c = tid % 3;
+        double x[9], a[9];
+        for (int m = 0; m < 9; ++m) x[m] = s_nodes[c_face_node[k][m] * 3 + c];
+        nodes_to_mono9(x, a);
+        for (int m = 0; m < 9; ++m) s_ecoef[k][c * 9 + m] = a[m];
+    }
+    __syncthreads();
+    const double t_tie = S->t_tie, theta = S->theta, tol_d = S->tol_d;
+    const int max_level = S->max_level;
+    double my_d = INFINITY, my_c = 0.0;
+    for (int f = tid; f < n_face; f += SL_THREADS) {
+        const double *AQ = fcoef + (size_t)f * 28;
+        for (int k = 0; k < 6; ++k) {
+            const double *AP = s_ecoef[k];
+            Item st[80];
+            int top = 0;
+            st[top].f = f; st[top].w1 = 0; st[top].w2 = 0; st[top].w3 = 0; ++top;
+            while (top > 0) {
+                const Item it = st[--top];
+                double uc, vc, hP, sc, tc, hQ;
+                item_box(it, uc, vc, hP, sc, tc, hQ);
+                const NodeBound nb = bound_subpair([&](int m) { return AP[m]; }, [&](int m) { return __ldg(AQ + m); },
+                                                   uc, vc, hP, sc, tc, hQ);
+                double best = u2d(s_best);
+                if (nb.dist_c < best) { atomicMin(&s_best, d2u(nb.dist_c)); best = nb.dist_c; }
+                if (nb.lb > best + t_tie) continue;
+                const double kP = nb.s1P > 0.0 ? nb.s2P / (nb.s1P * nb.s1P) : 0.0;
+                const double kQ = nb.s1Q > 0.0 ? nb.s2Q / (nb.s1Q * nb.s1Q) : 0.0;
+                bool leaf = fmax(kP, kQ) * fmax(nb.s1P, nb.s1Q) <= theta;
+                const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+                bool splitP = nb.s1P >= nb.s1Q;
+                if (!leaf) {
+                    if (splitP && lP >= max_level) splitP = false;
+                    if (!splitP && lQ >= max_level) { if (lP < max_level) splitP = true; else leaf = true; }
+                }
+                if (leaf || top + 4 > 80) {
+                    double CP[27], CQ[27];
+                    for (int c = 0; c < 3; ++c) {
+                        double A[9];
+                        for (int m = 0; m < 9; ++m) A[m] = AP[c * 9 + m];
+                        recentre9(A, uc, vc, hP, hP, CP + 9 * c);
+                        for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
+                        recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
+                    }
+                    const NewtonOut o = newton_leaf(CP, CQ, tol_d, -1.0, NP_NEWTON_ITERS);
+                    atomicMin(&s_best, d2u(o.dist));
+                    if (o.dist < my_d - t_tie || (o.dist <= my_d + t_tie && fabs(o.cosv) > fabs(my_c))) {
+                        my_d = fmin(my_d, o.dist); my_c = o.cosv;
+                    }
+                } else {
+                    make_children(it, splitP, st + top);
+                    top += 4;
+                }
+            }
+        }
+    }
+    s_d[tid] = my_d; s_c[tid] = my_c;
+    __syncthreads();
+    if (tid == 0) {
+        double dmin = INFINITY;
+        for (int i = 0; i < SL_THREADS; ++i) dmin = fmin(dmin, s_d[i]);
+        double bc = 0.0;
+        for (int i = 0; i < SL_THREADS; ++i) if (s_d[i] <= dmin + t_tie && fabs(s_c[i]) > fabs(bc)) bc = s_c[i];
+        comp[e] = bc < 0.0 ? 1 : 2;
+        atomicAdd(&S->c_seedless_total, 1ull);
+    }
+}
+
+__global__ void k_uf_assign(DcScalars *S, long long n_elem, const int *__restrict__ parent,
+                            const unsigned char *__restrict__ comp, signed char *__restrict__ labels,
+                            double *__restrict__ sdist)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int lab = -2;
+    bool conflict = false;
+    if (e < n_elem) {
+        lab = labels[e];
+        if (lab != DC_CUT) {
+            const int bits = comp[parent[e]];
+            if (lab < 0) {
+                conflict = bits == 3;
+                lab = (bits == 1) ? DC_HOLE : DC_NORMAL;
+                labels[e] = (signed char)lab;
+                sdist[e] = lab == DC_HOLE ? -S->d_band : S->d_band;
+            } else if (bits == 3) conflict = true;
+        }
+    }
+    const unsigned mc = __ballot_sync(0xffffffffu, lab == DC_CUT);
+    const unsigned mh = __ballot_sync(0xffffffffu, lab == DC_HOLE);
+    const unsigned mn = __ballot_sync(0xffffffffu, lab == DC_NORMAL);
+    const unsigned mf = __ballot_sync(0xffffffffu, conflict);
+    if ((threadIdx.x & 31) == 0) {
+        if (mc) atomicAdd(&S->c_cut, (unsigned long long)__popc(mc));
+        if (mh) atomicAdd(&S->c_hole, (unsigned long long)__popc(mh));
+        if (mn) atomicAdd(&S->c_normal, (unsigned long long)__popc(mn));
+        if (mf) { atomicAdd(&S->c_fill_conflicts, (unsigned long long)__popc(mf)); atomicOr(&S->status, DC_STATUS_FILL_CONFLICT); }
+    }
+}
+
+// small helpers
+__global__ void k_boxes_to_aos(const double *__restrict__ ebox, long long n_elem, double *__restrict__ out)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elem) return;
+    for (int c = 0; c < 6; ++c) out[e * 6 + c] = ebox[(size_t)c * n_elem + e];
+}
+
+// FP64 FMA peak: 8 independent register-resident chains per thread
+__global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, double a, double b)
+{
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// ==========================================================================================
+// host side
+// ==========================================================================================
+struct dc_ctx {
+    int device, num_sms, narrow_blocks;
+    long long n_nodes, n_elem, max_faces, max_pairs, n_face;
+    const double *xyz; const int *conn; const int *adj;
+    const double *face_nodes;
+    // workspace partition
+    unsigned char *ws; size_t ws_bytes;
+    DcScalars *S;
+    double *ebox;             // [6][n_elem]
+    int *adj_own;             // [n_elem][6] (derived) or NULL
+    int *parent; unsigned char *comp;
+    int *act_elem; long long *act_start; int *act_cnt;
+    int *pair_face; unsigned long long *pair_key;
+    double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
+    int *cell_count, *cell_start, *cell_fill;
+    Item *spill;
+    double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
+    cudaEvent_t ev[10];
+    cudaStream_t last_stream;
+    bool have_surface, have_cut;
+    DcScalars *S_host;        // pinned
+};
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct WsLayout {
+    size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_act_elem, off_act_start, off_act_cnt,
+        off_pair_face, off_pair_key, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
+        off_cell_count, off_cell_start, off_cell_fill, off_spill, off_hfaces, off_hlabels, off_hsdist, total;
+};
+
+#define DC_MAX_NARROW_BLOCKS (148 * 4)
+
+static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_faces, long long max_pairs)
+{
+    WsLayout L; size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
+    L.off_S = take(sizeof(DcScalars));
+    L.off_ebox = take((size_t)n_elem * 6 * 8);
+    L.off_adj = take((size_t)n_elem * 6 * 4);
+    L.off_parent = take((size_t)n_elem * 4);
+    L.off_comp = take((size_t)n_elem + 4);
+    L.off_act_elem = take((size_t)n_elem * 4);
+    L.off_act_start = take((size_t)n_elem * 8);
+    L.off_act_cnt = take((size_t)n_elem * 4);
+    // pair arrays double as the scratch of the adjacency derivation (2 x n_nodes ints)
+    size_t pf = (size_t)max_pairs * 4, pk = (size_t)max_pairs * 8;
+    size_t need_adj = (size_t)n_nodes * 8;
+    if (pf + pk < need_adj) pk = need_adj - pf;
+    L.off_pair_face = take(pf);
+    L.off_pair_key = take(pk);
+    L.off_fbox_orig = take((size_t)max_faces * 6 * 8);
+    L.off_fbox = take((size_t)max_faces * 6 * 8);
+    L.off_fcoef = take((size_t)max_faces * 28 * 8);
+    L.off_fcell = take((size_t)max_faces * 4);
+    L.off_fperm = take((size_t)max_faces * 4);
+    L.off_cell_count = take((size_t)(DC_NCELL + 1) * 4);
+    L.off_cell_start = take((size_t)(DC_NCELL + 1) * 4);
+    L.off_cell_fill = take((size_t)(DC_NCELL + 1) * 4);
+    L.off_spill = take((size_t)DC_MAX_NARROW_BLOCKS * NP_SPILL * sizeof(Item));
+    L.off_hfaces = take((size_t)max_faces * 27 * 8);
+    L.off_hlabels = take((size_t)n_elem);
+    L.off_hsdist = take((size_t)n_elem * 8);
+    L.total = o;
+    return L;
+}
+
+extern "C" size_t dc_workspace_bytes(long long n_nodes, long long n_elem, long long max_faces, long long max_pairs)
+{
+    if (n_nodes <= 0 || n_elem <= 0 || max_faces <= 0 || max_pairs <= 0) return 0;
+    if (n_elem > 300000000LL || n_nodes > 2000000000LL) return 0;
+    return ws_layout(n_nodes, n_elem, max_faces, max_pairs).total;
+}
+
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    fprintf(stderr, "libdc: %s failed: %s (%s:%d)\n", #call, cudaGetErrorString(e_), __FILE__, __LINE__); return DC_ERR_CUDA; } } while (0)
+
+static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+static int run_elem_boxes(dc_ctx *c, cudaStream_t st)
+{
+    CK(cudaMemsetAsync(&c->S->grid_max_diag2, 0, 8, st));
+    k_elem_boxes<<<nblk(c->n_elem, EB_THREADS), EB_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->n_elem, c->ebox);
+    CK(cudaGetLastError());
+    return DC_OK;
+}
+
+extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const double *xyz_dev,
+                              long long n_elem, const int *conn27_dev, const int *adj6_dev,
+                              void *workspace_dev, size_t workspace_bytes,
+                              long long max_faces, long long max_pairs, void *stream)
+{
+    if (!out || !xyz_dev || !conn27_dev || !workspace_dev) return DC_ERR_ARG;
+    const size_t need = dc_workspace_bytes(n_nodes, n_elem, max_faces, max_pairs);
+    if (need == 0) return DC_ERR_ARG;
+    if (workspace_bytes < need) return DC_ERR_WORKSPACE;
+    if (((uintptr_t)workspace_dev & 255) != 0) return DC_ERR_ARG;
+    CK(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return DC_ERR_UNSUPPORTED;   // sm_100a only: no fallback path exists
+    dc_ctx *c = new (std::nothrow) dc_ctx();
+    if (!c) return DC_ERR_ARG;
+    memset(c, 0, sizeof *c);
+    c->device = device; c->num_sms = prop.multiProcessorCount;
+    c->n_nodes = n_nodes; c->n_elem = n_elem; c->max_faces = max_faces; c->max_pairs = max_pairs;
+    c->xyz = xyz_dev; c->conn = conn27_dev;
+    c->ws = (unsigned char *)workspace_dev; c->ws_bytes = workspace_bytes;
+    const WsLayout L = ws_layout(n_nodes, n_elem, max_faces, max_pairs);
+    c->S = (DcScalars *)(c->ws + L.off_S);
+    c->ebox = (double *)(c->ws + L.off_ebox);
+    c->adj_own = (int *)(c->ws + L.off_adj);
+    c->parent = (int *)(c->ws + L.off_parent);
+    c->comp = c->ws + L.off_comp;
+    c->act_elem = (int *)(c->ws + L.off_act_elem);
+    c->act_start = (long long *)(c->ws + L.off_act_start);
+    c->act_cnt = (int *)(c->ws + L.off_act_cnt);
+    c->pair_face = (int *)(c->ws + L.off_pair_face);
+    c->pair_key = (unsigned long long *)(c->ws + L.off_pair_key);
+    c->fbox_orig = (double *)(c->ws + L.off_fbox_orig);
+    c->fbox = (double *)(c->ws + L.off_fbox);
+    c->fcoef = (double *)(c->ws + L.off_fcoef);
+    c->fcell = (int *)(c->ws + L.off_fcell);
+    c->fperm = (int *)(c->ws + L.off_fperm);
+    c->cell_count = (int *)(c->ws + L.off_cell_count);
+    c->cell_start = (int *)(c->ws + L.off_cell_start);
+    c->cell_fill = (int *)(c->ws + L.off_cell_fill);
+    c->spill = (Item *)(c->ws + L.off_spill);
+    c->h_faces_dev = (double *)(c->ws + L.off_hfaces);
+    c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
+    c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->ev[i]));
+    CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
+    CK(cudaFuncSetAttribute(k_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NarrowShared)));
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_narrow, NP_THREADS, sizeof(NarrowShared)));
+    if (occ < 1) occ = 1;
+    c->narrow_blocks = c->num_sms * occ;
+    if (c->narrow_blocks > DC_MAX_NARROW_BLOCKS) c->narrow_blocks = DC_MAX_NARROW_BLOCKS;
+    CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
+    int rc = run_elem_boxes(c, st);
+    if (rc != DC_OK) { delete c; return rc; }
+    if (adj6_dev) c->adj = adj6_dev;
+    else {
+        int *first = (int *)(c->ws + L.off_pair_face);
+        int *second = first + n_nodes;
+        CK(cudaMemsetAsync(first, 0xff, (size_t)n_nodes * 8, st));
+        k_adj_pass1<<<nblk(n_elem * 6, 256), 256, 0, st>>>(c->conn, n_elem, first, second);
+        k_adj_pass2<<<nblk(n_elem * 6, 256), 256, 0, st>>>(c->conn, n_elem, first, second, c->adj_own);
+        CK(cudaGetLastError());
+        c->adj = c->adj_own;
+    }
+    *out = c;
+    return DC_OK;
+}
+
+extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *face_nodes_dev, void *stream)
+{
+    if (!c || !face_nodes_dev || n_face <= 0) return DC_ERR_ARG;
+    if (n_face > c->max_faces) return DC_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    CK(cudaSetDevice(c->device));
+    CK(cudaEventRecord(c->ev[8], st));
+    c->face_nodes = face_nodes_dev; c->n_face = n_face;
+    const int nf = (int)n_face;
+    k_reset_surface<<<1, 1, 0, st>>>(c->S);
+    k_face_boxes<<<nblk(nf, 128), 128, 0, st>>>(c->S, face_nodes_dev, nf, c->fbox_orig);
+    k_setup_surface<<<1, 1, 0, st>>>(c->S, nf);
+    CK(cudaMemsetAsync(c->cell_count, 0, (size_t)(DC_NCELL + 1) * 4, st));
+    CK(cudaMemsetAsync(c->cell_fill, 0, (size_t)(DC_NCELL + 1) * 4, st));
+    k_face_hist<<<nblk(nf, 128), 128, 0, st>>>(c->S, c->fbox_orig, nf, c->fcell, c->cell_count);
+    k_cell_scan<<<1, 1024, 0, st>>>(c->cell_count, c->cell_start);
+    k_face_scatter<<<nblk(nf, 128), 128, 0, st>>>(face_nodes_dev, c->fbox_orig, c->fcell, c->cell_start, c->cell_fill,
+                                                   nf, c->fperm, c->fbox, c->fcoef);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(c->ev[9], st));
+    c->have_surface = true;
+    return DC_OK;
+}
+
+extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labels_dev, double *sdist_dev, void *stream)
+{
+    if (!c || !labels_dev || !sdist_dev) return DC_ERR_ARG;
+    if (!c->have_surface) return DC_ERR_STATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    CK(cudaSetDevice(c->device));
+    dc_params P; memset(&P, 0, sizeof P);
+    if (params) P = *params;
+    const long long ne = c->n_elem;
+    CK(cudaEventRecord(c->ev[0], st));
+    if (P.flags & DC_FLAG_RECOMPUTE_BOXES) { int rc = run_elem_boxes(c, st); if (rc) return rc; }
+    CK(cudaEventRecord(c->ev[1], st));
+    k_setup_classify<<<1, 1, 0, st>>>(c->S, P);
+    k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_count, c->act_elem);
+    k_pairs<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
+                                           c->act_start, c->act_cnt, c->pair_face, c->pair_key);
+    CK(cudaEventRecord(c->ev[2], st));
+    k_narrow<<<c->narrow_blocks, NP_THREADS, sizeof(NarrowShared), st>>>(c->S, c->xyz, c->conn, c->act_elem, c->act_start,
+                                                                         c->act_cnt, c->pair_face, c->pair_key, c->fcoef,
+                                                                         c->spill, labels_dev, sdist_dev);
+    CK(cudaEventRecord(c->ev[3], st));
+    k_uf_union<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, c->adj, ne, c->parent);
+    k_uf_seed<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, ne, c->parent, c->comp);
+    k_uf_collect<<<nblk(ne, 256), 256, 0, st>>>(c->S, labels_dev, ne, c->parent, c->comp);
+    k_seedless<<<DC_MAX_SEEDLESS, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
+    k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(c->ev[4], st));
+    c->have_cut = true;
+    return DC_OK;
+}
+
+extern "C" int dc_classify_host(dc_ctx *c, const dc_params *params, long long n_face, const double *face_nodes_host,
+                                signed char *labels_host, double *sdist_host, void *stream)
+{
+    if (!c || !face_nodes_host || !labels_host || !sdist_host || n_face <= 0) return DC_ERR_ARG;
+    if (n_face > c->max_faces) return DC_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(c->device));
+    CK(cudaMemcpyAsync(c->h_faces_dev, face_nodes_host, (size_t)n_face * 27 * 8, cudaMemcpyHostToDevice, st));
+    int rc = dc_set_cut_surface(c, n_face, c->h_faces_dev, stream);
+    if (rc) return rc;
+    rc = dc_classify(c, params, c->h_labels_dev, c->h_sdist_dev, stream);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(labels_host, c->h_labels_dev, (size_t)c->n_elem, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(sdist_host, c->h_sdist_dev, (size_t)c->n_elem * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return DC_OK;
+}
+
+extern "C" int dc_get_element_boxes(dc_ctx *c, double *out_dev, void *stream)
+{
+    if (!c || !out_dev) return DC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    k_boxes_to_aos<<<nblk(c->n_elem, 256), 256, 0, st>>>(c->ebox, c->n_elem, out_dev);
+    CK(cudaGetLastError());
+    return DC_OK;
+}
+
+extern "C" int dc_get_adjacency(dc_ctx *c, int *out_dev, void *stream)
+{
+    if (!c || !out_dev) return DC_ERR_ARG;
+    CK(cudaMemcpyAsync(out_dev, c->adj, (size_t)c->n_elem * 6 * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return DC_OK;
+}
+
+extern "C" long long dc_get_pairs(dc_ctx *c, int *elem_host, int *face_host, long long cap)
+{
+    if (!c || !elem_host || !face_host) return DC_ERR_ARG;
+    if (!c->have_cut) return DC_ERR_STATE;
+    CK(cudaStreamSynchronize(c->last_stream));
+    CK(cudaMemcpy(c->S_host, c->S, sizeof(DcScalars), cudaMemcpyDeviceToHost));
+    const int na = c->S_host->n_active;
+    int *ae = new int[na > 0 ? na : 1]; long long *as = new long long[na > 0 ? na : 1]; int *ac = new int[na > 0 ? na : 1];
+    int *perm = new int[c->n_face];
+    cudaMemcpy(ae, c->act_elem, (size_t)na * 4, cudaMemcpyDeviceToHost);
+    cudaMemcpy(as, c->act_start, (size_t)na * 8, cudaMemcpyDeviceToHost);
+    cudaMemcpy(ac, c->act_cnt, (size_t)na * 4, cudaMemcpyDeviceToHost);
+    cudaMemcpy(perm, c->fperm, (size_t)c->n_face * 4, cudaMemcpyDeviceToHost);
+    long long np = (long long)c->S_host->n_pairs; if (np > c->max_pairs) np = c->max_pairs;
+    int *pf = new int[np > 0 ? np : 1];
+    cudaMemcpy(pf, c->pair_face, (size_t)np * 4, cudaMemcpyDeviceToHost);
+    long long n = 0;
+    for (int a = 0; a < na; ++a)
+        for (int i = 0; i < ac[a]; ++i) {
+            if (n < cap) { elem_host[n] = ae[a]; face_host[n] = perm[pf[as[a] + i]]; }
+            ++n;
+        }
+    delete[] ae; delete[] as; delete[] ac; delete[] perm; delete[] pf;
+    return n;
+}
+
+extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
+{
+    if (!c || !o) return DC_ERR_ARG;
+    CK(cudaSetDevice(c->device));
+    CK(cudaStreamSynchronize(c->last_stream));
+    CK(cudaMemcpy(c->S_host, c->S, sizeof(DcScalars), cudaMemcpyDeviceToHost));
+    const DcScalars &S = *c->S_host;
+    memset(o, 0, sizeof *o);
+    o->n_elem = c->n_elem; o->n_face = c->n_face;
+    o->n_active = S.n_active; o->n_box_tests = (long long)S.c_box_tests;
+    o->n_pairs = (long long)S.n_pairs > c->max_pairs ? c->max_pairs : (long long)S.n_pairs;
+    o->pairs_needed = (long long)S.n_pairs;
+    o->n_bnb_nodes = (long long)S.c_bnb_nodes; o->n_newton = (long long)S.c_newton;
+    o->n_newton_iters = (long long)S.c_newton_iters; o->n_newton_fail = (long long)S.c_newton_fail;
+    o->n_depth_exceeded = (long long)S.c_depth_exceeded;
+    o->n_cut = (long long)S.c_cut; o->n_hole = (long long)S.c_hole; o->n_normal = (long long)S.c_normal;
+    o->n_ambiguous = (long long)S.c_ambiguous; o->n_sign_ambiguous = (long long)S.c_sign_ambiguous;
+    o->n_seedless_components = S.n_seedless; o->n_fill_conflicts = (long long)S.c_fill_conflicts;
+    o->queue_peak = (long long)S.c_queue_peak;
+    o->l_ref = S.l_ref; o->tau_cut = S.tau; o->d_band = S.d_band;
+    o->status = S.status;
+    if (c->have_cut) {
+        float ms;
+        if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) == cudaSuccess) o->ms_stage[1] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[1], c->ev[2]) == cudaSuccess) o->ms_stage[2] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[2], c->ev[3]) == cudaSuccess) o->ms_stage[3] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[3], c->ev[4]) == cudaSuccess) o->ms_stage[4] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[4]) == cudaSuccess) o->ms_stage[5] = ms;
+    }
+    if (c->have_surface) {
+        float ms;
+        if (cudaEventElapsedTime(&ms, c->ev[8], c->ev[9]) == cudaSuccess) { o->ms_stage[0] = ms; o->ms_stage[6] = ms; }
+    }
+    (void)cudaGetLastError();
+    if (S.status & (DC_STATUS_PAIR_OVERFLOW | DC_STATUS_QUEUE_OVERFLOW)) return DC_ERR_WORKSPACE;
+    return DC_OK;
+}
+
+extern "C" void dc_destroy(dc_ctx *c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    if (c->last_stream || true) cudaStreamSynchronize(c->last_stream);
+    for (int i = 0; i < 10; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    if (c->S_host) cudaFreeHost(c->S_host);
+    delete c;
+}
+
+extern "C" const char *dc_error_string(int code)
+{
+    switch (code) {
+    case DC_OK: return "ok";
+    case DC_ERR_ARG: return "bad argument";
+    case DC_ERR_WORKSPACE: return "workspace too small or device-side list overflow";
+    case DC_ERR_UNSUPPORTED: return "unsupported device or input (libdc needs an sm_100 GPU)";
+    case DC_ERR_CUDA: return "CUDA runtime error";
+    case DC_ERR_STATE: return "call order error";
+    default: return "unknown error";
+    }
+}
+
+extern "C" double dc_measure_fp64_tflops(int device, int iters)
+{
+    if (cudaSetDevice(device) != cudaSuccess) return -1.0;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return -1.0;
+    const int blocks = prop.multiProcessorCount * 8, threads = 256;
+    double *out = nullptr;
+    if (cudaMalloc(&out, (size_t)blocks * threads * 8) != cudaSuccess) return -1.0;
+    cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+    if (iters <= 0) iters = 2000;
+    k_dfma_peak<<<blocks, threads>>>(out, iters / 10 + 1, 1.0000001, 1e-9);
+    cudaDeviceSynchronize();
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(a);
+        k_dfma_peak<<<blocks, threads>>>(out, iters, 1.0000001, 1e-9);
+        cudaEventRecord(b);
+        cudaEventSynchronize(b);
+        float ms = 0; cudaEventElapsedTime(&ms, a, b);
+        const double flop = 2.0 * 8 * 16 * (double)iters * blocks * threads;
+        const double tf = flop / (ms * 1e-3) / 1e12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(out);
+    if (cudaGetLastError() != cudaSuccess) return -1.0;
+    return best;
+}
+
+extern "C" int dc_version(void) { return 1; }
