@@ -99,7 +99,7 @@ typedef struct {
     float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
                                     4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface, 7 unused */
     int status;                  /* DC_STATUS_* bits */
-    int reserved;
+    int n_launches;              /* kernels launched by the last dc_set_cut_surface + dc_classify */
 } dc_stats;
 
 /* Bytes of device scratch dc_create_grid needs for a grid of this size, up to max_faces

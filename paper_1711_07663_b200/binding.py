@@ -37,7 +37,7 @@ class dc_stats(C.Structure):
                 ("n_seedless_components", C.c_longlong), ("n_fill_conflicts", C.c_longlong),
                 ("pairs_needed", C.c_longlong), ("queue_peak", C.c_longlong),
                 ("l_ref", C.c_double), ("tau_cut", C.c_double), ("d_band", C.c_double),
-                ("ms_stage", C.c_float * 8), ("status", C.c_int), ("reserved", C.c_int)]
+                ("ms_stage", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int)]
 
     def as_dict(self) -> dict:
         d = {}

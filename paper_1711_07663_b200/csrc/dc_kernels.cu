@@ -1020,6 +1020,7 @@ struct dc_ctx {
     cudaEvent_t ev[10];
     cudaStream_t last_stream;
     bool have_surface, have_cut;
+    int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
     DcScalars *S_host;        // pinned
 };
 
@@ -1179,6 +1180,7 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
                                                    nf, c->fperm, c->fbox, c->fcoef);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[9], st));
+    c->launches_surface = 6;
     c->have_surface = true;
     return DC_OK;
 }
@@ -1212,6 +1214,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
+    c->launches_classify = 9 + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }
@@ -1297,6 +1300,7 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
     o->queue_peak = (long long)S.c_queue_peak;
     o->l_ref = S.l_ref; o->tau_cut = S.tau; o->d_band = S.d_band;
     o->status = S.status;
+    o->n_launches = (c->have_surface ? c->launches_surface : 0) + (c->have_cut ? c->launches_classify : 0);
     if (c->have_cut) {
         float ms;
         if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) == cudaSuccess) o->ms_stage[1] = ms;

@@ -1,0 +1,113 @@
+"""-m gpu: BASELINE.json's FULL-SIZE configs in the launch configuration bench.py times
+(dc_set_cut_surface + dc_classify with DC_FLAG_RECOMPUTE_BOXES on a warm context):
+
+* sampled outputs the oracle computes one by one (elements chosen from the ANALYTIC shape only:
+  half near the surface, half uniformly at random), labels bit-exact off the oracle's ambiguous
+  band and signed distance within 1e-10 L_ref;
+* properties that hold at any size: P7 no HOLE element face-adjacent to a NORMAL one, P8 HOLE u CUT
+  covers every centroid inside the analytic body (and NORMAL u CUT every one outside), census
+  adds up, no fill conflicts, no sign ambiguity;
+* config 3 = config 2's grid re-cut by the rotated surface on the same context.
+"""
+import numpy as np
+import pytest
+
+from oracle import dc_oracle as O
+from workloads import make_config, rotation_about_axis
+
+pytestmark = pytest.mark.gpu
+HOLE, NORMAL, CUT = 0, 1, 2
+TOL_REL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1711_07663_b200._build import build_lib
+    build_lib()
+    from paper_1711_07663_b200 import binding
+    return binding
+
+
+def centroids(w):
+    return w.xyz[w.conn27[:, 13]]          # the centre node IS the image of (0,0,0)
+
+
+def pick_sample(w, cen, n_near, n_rand, seed):
+    rng = np.random.default_rng(seed)
+    h = 2.0 / w.N
+    # cheap analytic pre-filter so the margin (336 dimples / 8 ellipsoids) is evaluated on few points
+    cand = rng.choice(w.n_elem, size=min(w.n_elem, 400000), replace=False)
+    mar = w.surf_margin(cen[cand])
+    near = cand[mar < 1.5 * h]
+    ids = np.concatenate([rng.choice(near, size=min(n_near, near.size), replace=False),
+                          rng.choice(w.n_elem, size=n_rand, replace=False)])
+    return np.unique(ids)
+
+
+def check_invariants(w, cen, labels, st, eps_margin):
+    assert st.status == 0 and st.n_fill_conflicts == 0 and st.n_depth_exceeded == 0
+    assert st.n_cut + st.n_hole + st.n_normal == w.n_elem
+    assert (np.bincount(labels, minlength=3)[:3] == [st.n_hole, st.n_normal, st.n_cut]).all()
+    for k in range(6):
+        nb = w.adj6[:, k]; m = nb >= 0
+        a, b = labels[m], labels[nb[m]]
+        assert not ((a == HOLE) & (b == NORMAL)).any() and not ((a == NORMAL) & (b == HOLE)).any()
+    # P8 on a large random subset (the analytic margin is costly for the dimpled sphere)
+    rng = np.random.default_rng(8)
+    sub = rng.choice(w.n_elem, size=min(w.n_elem, 300000), replace=False)
+    ins, mar = w.inside(cen[sub]), w.surf_margin(cen[sub])
+    sure = mar > eps_margin
+    assert np.isin(labels[sub][sure & ins], (HOLE, CUT)).all()
+    assert np.isin(labels[sub][sure & ~ins], (NORMAL, CUT)).all()
+    assert (labels[sub][ins] != NORMAL).sum() > 0
+
+
+def check_sample(w, faces, ids, labels, sdist, st, nproc, zero_amb):
+    d_band = O.auto_d_band(w.xyz, w.conn27, faces)       # the oracle's own (never the GPU's value)
+    assert abs(st.d_band - d_band) <= 1e-14
+    ref = O.classify(w.xyz, w.conn27, faces, elem_ids=ids, nproc=nproc, d_band=d_band)
+    L = ref.stats["l_ref"]
+    amb = (ref.flags & O.FLAG_AMBIGUOUS) != 0
+    if zero_amb:
+        assert amb.sum() == 0 and st.n_ambiguous == 0
+    assert ref.stats["n_depth_exceeded"] == 0
+    bad = (labels[ids] != ref.labels) & ~amb
+    assert bad.sum() == 0, "label mismatches at elements %s" % ids[bad][:10]
+    err = np.abs(sdist[ids] - ref.sdist)[~amb]
+    assert err.max() <= TOL_REL * L, "max |dsdist| %.3e" % err.max()
+    assert (ref.labels == CUT).sum() > 20 and (ref.labels == HOLE).sum() > 5
+    return ref
+
+
+@pytest.mark.parametrize("config", [1, 2, 4])
+def test_fullsize_sampled_parity_and_invariants(B, nproc, config):
+    w = make_config(config)
+    cen = centroids(w)
+    dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face)
+    p = B.dc_params(); p.flags = B.DC_FLAG_RECOMPUTE_BOXES
+    dcut.set_cut_surface(w.faces)
+    dcut.classify(p)                                      # warm context, as bench.py times it
+    dcut.set_cut_surface(w.faces)
+    labels, sdist = dcut.classify(p)
+    st = dcut.stats()
+    labels, sdist = labels.cpu().numpy().copy(), sdist.cpu().numpy().copy()
+    check_invariants(w, cen, labels, st, eps_margin=1e-3)
+    assert st.n_sign_ambiguous == 0
+    ids = pick_sample(w, cen, 500 if config != 4 else 300, 500 if config != 4 else 300, seed=config)
+    check_sample(w, w.faces, ids, labels, sdist, st, nproc, zero_amb=(config == 1))
+    if config == 2:
+        # config 3: the same grid re-cut by the surface rotated 32 degrees about the seeded axis
+        faces = w.spin_faces(32)
+        dcut.set_cut_surface(faces)
+        labels, sdist = dcut.classify(p)
+        st = dcut.stats()
+        labels, sdist = labels.cpu().numpy().copy(), sdist.cpu().numpy().copy()
+        assert st.status == 0 and st.n_fill_conflicts == 0
+        Rm = rotation_about_axis(w.meta["spin_axis"], np.deg2rad(32.0))     # faces = w.faces @ Rm.T
+        cen_back = cen @ Rm                                                 # centroids in the body frame
+        mar = w.surf_margin(cen_back[ids]); h = 2.0 / w.N
+        ids3 = ids[(mar < 1.5 * h) | (np.arange(ids.size) % 3 == 0)][:600]
+        check_sample(w, faces, ids3, labels, sdist, st, nproc, zero_amb=False)
+    dcut.close()
