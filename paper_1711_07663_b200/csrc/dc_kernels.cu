@@ -5,8 +5,8 @@
 //   S3 face bins      k_face_hist, k_cell_scan, k_face_scatter        (Morton-ordered uniform bins)
 //   S2 element boxes  k_elem_boxes                                    (HBM-bound stream)
 //   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
-//   S5 narrow phase   k_narrow (persistent CTAs, shared-memory work queues, FP64)
-//   S6 decide         fused at the end of each k_narrow batch
+//   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound (wavefront of uniform kernels, FP64)
+//   S6 decide         k_np_decide
 //   S7 flood fill     k_uf_union, k_uf_seed, k_uf_collect, k_seedless, k_uf_assign
 //
 // PAPER.md citations are given where an operation is defined; the kernel design itself is new
@@ -26,6 +26,7 @@ using namespace dcg;
 #define DC_MAX_SEEDLESS 32
 #define DC_GRID_MAX 64              /* face-bin cells per axis (Morton code: 6 bits per axis) */
 #define DC_NCELL (DC_GRID_MAX * DC_GRID_MAX * DC_GRID_MAX)
+#define DC_NQN 28                   /* >= DC_MAX_ROUNDS + 2 */
 
 // ------------------------------------------------------------------------------------------
 // device-resident scalars and counters
@@ -47,9 +48,12 @@ struct DcScalars {
     int pad0;
     // work state
     int n_active;
-    int work_counter;
+    int n_band;                     // elements with >= 1 candidate pair (the narrow-phase band)
+    int max_band;                   // capacity of the per-band-element arrays
     int n_seedless;
     int status;
+    int qn[DC_NQN];                 // items of round r (children queue, ping-pong buffers)
+    int nn[DC_NQN];                 // leaves of round r (Newton queue)
     unsigned long long n_pairs;
     int seedless_elem[DC_MAX_SEEDLESS];
     // counters
@@ -213,16 +217,17 @@ __global__ void k_face_scatter(const double *__restrict__ face_nodes, const doub
 #pragma unroll
     for (int m = 0; m < 6; ++m) fbox[(size_t)pos * 6 + m] = fbox_orig[(size_t)f * 6 + m];
     const double *X = face_nodes + (size_t)f * 27;
+    double A[27];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        double x[9], a[9];
+        double x[9];
 #pragma unroll
         for (int m = 0; m < 9; ++m) x[m] = __ldg(X + 3 * m + c);
-        nodes_to_mono9(x, a);
+        nodes_to_mono9(x, A + 9 * c);
 #pragma unroll
-        for (int m = 0; m < 9; ++m) fcoef[(size_t)pos * 28 + c * 9 + m] = a[m];
+        for (int m = 0; m < 9; ++m) fcoef[(size_t)pos * 28 + c * 9 + m] = A[9 * c + m];
     }
-    fcoef[(size_t)pos * 28 + 27] = 0.0;
+    fcoef[(size_t)pos * 28 + 27] = higher_order_const(A);   // slot 27: see dc_geom.cuh bound_node
 }
 
 // ------------------------------------------------------------------------------------------
@@ -299,8 +304,9 @@ __global__ void k_adj_pass2(const int *__restrict__ conn, long long n_elem, cons
 
 // ------------------------------------------------------------------------------------------
 // per-classify scalar setup
-__global__ void k_setup_classify(DcScalars *S, dc_params P)
+__global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
 {
+    S->max_band = max_band;
     const double lref = P.l_ref > 0.0 ? P.l_ref : S->l_ref_auto;
     S->l_ref = lref;
     S->tau = (P.tau_cut_rel > 0.0 ? P.tau_cut_rel : 1e-7) * lref;
@@ -312,7 +318,8 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P)
     S->reach = S->d_band + 2.0 * S->tau + S->t_tie;
     S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.125;
     S->max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
-    S->n_active = 0; S->work_counter = 0; S->n_seedless = 0; S->status = 0; S->n_pairs = 0ull;
+    S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->status = 0; S->n_pairs = 0ull;
+    for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; }
     S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
     S->c_depth_exceeded = S->c_cut = S->c_hole = S->c_normal = S->c_ambiguous = 0ull;
     S->c_sign_ambiguous = S->c_fill_conflicts = S->c_queue_peak = S->c_seedless_total = 0ull;
@@ -379,7 +386,8 @@ __device__ __forceinline__ bool box_within(const double *lo, const double *hi, c
 __global__ void __launch_bounds__(256) k_pairs(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
                                                const int *__restrict__ act_elem, const int *__restrict__ cell_start,
                                                const double *__restrict__ fbox, long long max_pairs,
-                                               long long *__restrict__ act_start, int *__restrict__ act_cnt,
+                                               int *__restrict__ band_elem, long long *__restrict__ band_start,
+                                               int *__restrict__ band_cnt,
                                                int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key)
 {
     const int lane = threadIdx.x & 31;
@@ -431,8 +439,11 @@ __global__ void __launch_bounds__(256) k_pairs(DcScalars *S, const double *__res
                 if (lane == 0) {
                     long long b = (long long)atomicAdd(&S->n_pairs, (unsigned long long)total);
                     if (b + total > max_pairs) { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
-                    act_start[a] = b < 0 ? 0 : b;
-                    act_cnt[a] = b < 0 ? 0 : total;
+                    if (b >= 0 && total > 0) {
+                        const int slot = atomicAdd(&S->n_band, 1);
+                        if (slot < S->max_band) { band_elem[slot] = (int)e; band_start[slot] = b; band_cnt[slot] = total; }
+                        else atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW);
+                    }
                     base = b;
                 }
                 base = __shfl_sync(0xffffffffu, base, 0);
@@ -446,18 +457,11 @@ __global__ void __launch_bounds__(256) k_pairs(DcScalars *S, const double *__res
 }
 
 // ------------------------------------------------------------------------------------------
-// S5 + S6: narrow phase.
-#define NP_THREADS 128
-#define NP_BE 16            /* elements per batch */
-#define NP_QCAP 2048        /* shared-memory stack items */
-#define NP_NQCAP 384        /* Newton queue items (< 2 * NP_THREADS always) */
-#define NP_SPILL 8192       /* global spill items per CTA */
-#define NP_NEWTON_ITERS 40
-
+// S5 + S6: narrow phase -> dc_narrow.cuh (wavefront kernels).  Item / item_box / make_children below
+// serve k_seedless only.
+#define NP_NEWTON_ITERS_SL 40
 struct __align__(16) Item { unsigned f, w1, w2, w3; };
-// w1: slot(5) | k(3)<<5 | pair_local(24)<<8
-// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20
-// w3: is(12) | it(12)<<12 | flags(8)<<24      flags bit0: seed solve (no re-split on failure)
+// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20      w3: is(12) | it(12)<<12
 
 __constant__ int c_face_node[6][9] = {
     { 0, 3, 6, 9, 12, 15, 18, 21, 24 },      // xi = -1 : (a,b) = (j,k)
@@ -467,33 +471,6 @@ __constant__ int c_face_node[6][9] = {
     { 0, 1, 2, 3, 4, 5, 6, 7, 8 },           // zeta = -1 : (a,b) = (i,j)
     { 18, 19, 20, 21, 22, 23, 24, 25, 26 },  // zeta = +1
 };
-
-struct NarrowShared {
-    double ecoef[NP_BE][6][27];
-    double nodes[NP_THREADS / 32][27 * 3];
-    Item stack[NP_QCAP];
-    Item newton[NP_NQCAP];
-    unsigned long long best[NP_BE], dmin[NP_BE], seed[NP_BE];
-    long long pstart[NP_BE];
-    int elem[NP_BE], pcnt[NP_BE], poff[NP_BE + 1], cut[NP_BE];
-    int top, ntop, batch, nslots, peak;
-};
-
-struct Cnt { unsigned nodes, newton, iters, fail, depth; };
-
-__device__ __forceinline__ double u2d(unsigned long long b) { return __longlong_as_double((long long)b); }
-__device__ __forceinline__ unsigned long long d2u(double d) { return (unsigned long long)__double_as_longlong(d); }
-
-__device__ __forceinline__ void stack_push(NarrowShared &sh, Item *spill, DcScalars *S, const Item *it, int n)
-{
-    const int idx = atomicAdd(&sh.top, n);
-    for (int i = 0; i < n; ++i) {
-        const int j = idx + i;
-        if (j < NP_QCAP) sh.stack[j] = it[i];
-        else if (j - NP_QCAP < NP_SPILL) spill[j - NP_QCAP] = it[i];
-        else atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW);
-    }
-}
 
 __device__ __forceinline__ void item_box(const Item &it, double &uc, double &vc, double &hP,
                                          double &sc, double &tc, double &hQ)
@@ -525,270 +502,7 @@ __device__ __forceinline__ void make_children(const Item &it, bool splitP, Item 
     }
 }
 
-// one branch-and-bound node: bound, prune / split / hand over to Newton
-__device__ __forceinline__ void bnb_process(NarrowShared &sh, Item *spill, DcScalars *S, const double *__restrict__ fcoef,
-                                            const Item &it, Cnt &cnt, double t_tie, double tau_exit, double theta, int max_level)
-{
-    const int slot = it.w1 & 31, k = (it.w1 >> 5) & 7;
-    if (sh.cut[slot]) return;
-    double uc, vc, hP, sc, tc, hQ;
-    item_box(it, uc, vc, hP, sc, tc, hQ);
-    const double *AP = &sh.ecoef[slot][k][0];
-    const double *AQ = fcoef + (size_t)it.f * 28;
-    const NodeBound nb = bound_subpair([&](int m) { return AP[m]; }, [&](int m) { return __ldg(AQ + m); },
-                                       uc, vc, hP, sc, tc, hQ);
-    cnt.nodes++;
-    double best = u2d(sh.best[slot]);
-    if (nb.dist_c < best) { atomicMin(&sh.best[slot], d2u(nb.dist_c)); best = nb.dist_c; }
-    if (nb.dist_c <= tau_exit) { sh.cut[slot] = 1; return; }
-    if (nb.lb > best + t_tie) return;
-    const double kP = nb.s1P > 0.0 ? nb.s2P / (nb.s1P * nb.s1P) : 0.0;
-    const double kQ = nb.s1Q > 0.0 ? nb.s2Q / (nb.s1Q * nb.s1Q) : 0.0;
-    bool leaf = fmax(kP, kQ) * fmax(nb.s1P, nb.s1Q) <= theta;
-    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
-    bool splitP = nb.s1P >= nb.s1Q;
-    if (!leaf) {
-        if (splitP && lP >= max_level) splitP = false;
-        if (!splitP && lQ >= max_level) {
-            if (lP < max_level) splitP = true;
-            else { leaf = true; cnt.depth++; }
-        }
-    }
-    if (leaf) {
-        const int idx = atomicAdd(&sh.ntop, 1);
-        sh.newton[idx] = it;
-    } else {
-        Item ch[4];
-        make_children(it, splitP, ch);
-        stack_push(sh, spill, S, ch, 4);
-    }
-}
-
-__device__ __forceinline__ void newton_process(NarrowShared &sh, Item *spill, DcScalars *S, const double *__restrict__ fcoef,
-                                               unsigned long long *__restrict__ pair_key, const Item &it, Cnt &cnt,
-                                               double tol_d, double tau_exit, int max_level)
-{
-    const int slot = it.w1 & 31, k = (it.w1 >> 5) & 7;
-    if (sh.cut[slot]) return;
-    double uc, vc, hP, sc, tc, hQ;
-    item_box(it, uc, vc, hP, sc, tc, hQ);
-    double CP[27], CQ[27];
-    const double *AP = &sh.ecoef[slot][k][0];
-    const double *AQ = fcoef + (size_t)it.f * 28;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        double A[9];
-#pragma unroll
-        for (int m = 0; m < 9; ++m) A[m] = AP[c * 9 + m];
-        recentre9(A, uc, vc, hP, hP, CP + 9 * c);
-#pragma unroll
-        for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
-        recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
-    }
-    const NewtonOut o = newton_leaf(CP, CQ, tol_d, tau_exit, NP_NEWTON_ITERS);
-    cnt.newton++; cnt.iters += o.iters;
-    if (o.dist <= tau_exit) { sh.cut[slot] = 1; return; }
-    atomicMin(&sh.best[slot], d2u(o.dist));
-    atomicMin(&sh.dmin[slot], d2u(o.dist));
-    const unsigned long long key = (d2u(o.dist) & ~0xffull) | (unsigned long long)cos_code(o.cosv);
-    atomicMin(&pair_key[sh.pstart[slot] + (it.w1 >> 8)], key);
-    if (!o.converged) {
-        const bool seed = (it.w3 >> 24) & 1;
-        const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
-        if (!seed) {
-            cnt.fail++;
-            bool splitP = hP >= hQ;
-            if (splitP && lP >= max_level) splitP = false;
-            if (!splitP && lQ >= max_level) { if (lP < max_level) splitP = true; else return; }
-            Item ch[4];
-            make_children(it, splitP, ch);
-            stack_push(sh, spill, S, ch, 4);
-        }
-    }
-}
-
-__device__ __forceinline__ Item stack_get(NarrowShared &sh, const Item *spill, int j)
-{
-    return j < NP_QCAP ? sh.stack[j] : spill[j - NP_QCAP];
-}
-
-__global__ void __launch_bounds__(NP_THREADS) k_narrow(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
-                                                       const int *__restrict__ act_elem, const long long *__restrict__ act_start,
-                                                       const int *__restrict__ act_cnt, const int *__restrict__ pair_face,
-                                                       unsigned long long *__restrict__ pair_key, const double *__restrict__ fcoef,
-                                                       Item *__restrict__ spill_all, signed char *__restrict__ labels,
-                                                       double *__restrict__ sdist)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    NarrowShared &sh = *reinterpret_cast<NarrowShared *>(smem_raw);
-    Item *spill = spill_all + (size_t)blockIdx.x * NP_SPILL;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int n_active = S->n_active;
-    const double t_tie = S->t_tie, tau = S->tau, tau_exit = S->tau_exit, theta = S->theta, tol_d = S->tol_d;
-    const double d_band = S->d_band, amb = S->amb;
-    const int max_level = S->max_level;
-    const double init_best = S->reach;
-    Cnt cnt = { 0, 0, 0, 0, 0 };
-    unsigned n_amb = 0, n_samb = 0;
-    if (tid == 0) sh.peak = 0;
-
-    // drain both queues (bulk-synchronous rounds; Newton rounds when a full round is available)
-    auto drain = [&]() {
-        while (true) {
-            __syncthreads();
-            const int nt = sh.ntop, bt = sh.top;
-            if (nt == 0 && bt == 0) break;
-            const bool do_newton = (nt >= NP_THREADS) || (bt == 0);
-            __syncthreads();
-            Item it; bool have = false;
-            if (do_newton) {
-                const int take = min(nt, NP_THREADS);
-                if (tid < take) { it = sh.newton[nt - take + tid]; have = true; }
-                if (tid == 0) sh.ntop = nt - take;
-            } else {
-                const int take = min(bt, NP_THREADS);
-                if (tid < take) { it = stack_get(sh, spill, bt - take + tid); have = true; }
-                if (tid == 0) { sh.top = bt - take; if (bt > sh.peak) sh.peak = bt; }
-            }
-            __syncthreads();
-            if (have) {
-                if (do_newton) newton_process(sh, spill, S, fcoef, pair_key, it, cnt, tol_d, tau_exit, max_level);
-                else bnb_process(sh, spill, S, fcoef, it, cnt, t_tie, tau_exit, theta, max_level);
-            }
-        }
-    };
-
-    while (true) {
-        __syncthreads();
-        if (tid == 0) {
-            sh.batch = atomicAdd(&S->work_counter, 1);
-            sh.top = 0; sh.ntop = 0;
-        }
-        __syncthreads();
-        const int first = sh.batch * NP_BE;
-        if (first >= n_active) break;
-        const int nslots = min(NP_BE, n_active - first);
-        // ---- stage the batch: conn row (coalesced), nodes, monomial coefficients of the 6 boundary patches
-        for (int slot = warp; slot < nslots; slot += NP_THREADS / 32) {
-            const int e = act_elem[first + slot];
-            double *nd = sh.nodes[warp];
-            if (lane < 27) {
-                const int id = __ldg(conn + (size_t)e * 27 + lane);
-                const double *p = xyz + (size_t)id * 3;
-                nd[lane * 3 + 0] = __ldg(p); nd[lane * 3 + 1] = __ldg(p + 1); nd[lane * 3 + 2] = __ldg(p + 2);
-            }
-            __syncwarp();
-            if (lane < 18) {
-                const int k = lane / 3, c = lane % 3;
-                double x[9], a[9];
-#pragma unroll
-                for (int m = 0; m < 9; ++m) x[m] = nd[c_face_node[k][m] * 3 + c];
-                nodes_to_mono9(x, a);
-#pragma unroll
-                for (int m = 0; m < 9; ++m) sh.ecoef[slot][k][c * 9 + m] = a[m];
-            }
-            if (lane == 0) {
-                sh.elem[slot] = e; sh.pstart[slot] = act_start[first + slot]; sh.pcnt[slot] = act_cnt[first + slot];
-                sh.best[slot] = d2u(init_best); sh.dmin[slot] = 0x7ff0000000000000ull; sh.seed[slot] = ~0ull; sh.cut[slot] = 0;
-            }
-            __syncwarp();
-        }
-        __syncthreads();
-        if (tid == 0) {
-            int run = 0;
-            for (int s = 0; s < nslots; ++s) { sh.poff[s] = run; run += sh.pcnt[s]; }
-            sh.poff[nslots] = run; sh.nslots = nslots;
-        }
-        __syncthreads();
-        const int total = sh.poff[nslots] * 6;
-        // ---- seeding: centre-centre distances (attained) -> first upper bound, best (pair,k) per element
-        for (int t = tid; t < total; t += NP_THREADS) {
-            const int pl = t / 6, k = t - pl * 6;
-            int slot = 0;
-            while (pl >= sh.poff[slot + 1]) ++slot;
-            const int f = pair_face[sh.pstart[slot] + (pl - sh.poff[slot])];
-            const double *AP = &sh.ecoef[slot][k][0];
-            const double *AQ = fcoef + (size_t)f * 28;
-            const double dx = AP[0] - __ldg(AQ), dy = AP[9] - __ldg(AQ + 9), dz = AP[18] - __ldg(AQ + 18);
-            const double d = sqrt(dx * dx + dy * dy + dz * dz);
-            atomicMin(&sh.best[slot], d2u(d));
-            const unsigned long long sk = ((unsigned long long)__float_as_uint((float)d) << 32) | (unsigned)t;
-            atomicMin(&sh.seed[slot], sk);
-        }
-        __syncthreads();
-        if (tid < nslots && sh.seed[tid] != ~0ull) {
-            const int t = (int)(sh.seed[tid] & 0xffffffffu);
-            const int pl = t / 6, k = t - pl * 6;
-            Item it;
-            it.f = (unsigned)pair_face[sh.pstart[tid] + (pl - sh.poff[tid])];
-            it.w1 = (unsigned)tid | ((unsigned)k << 5) | ((unsigned)(pl - sh.poff[tid]) << 8);
-            it.w2 = 0; it.w3 = 1u << 24;
-            const int idx = atomicAdd(&sh.ntop, 1);
-            sh.newton[idx] = it;
-        }
-        drain();
-        // ---- roots: every (pair, boundary patch) is bounded; survivors enter the queues
-        for (int base = 0; base < total; base += NP_THREADS) {
-            const int t = base + tid;
-            if (t < total) {
-                const int pl = t / 6, k = t - pl * 6;
-                int slot = 0;
-                while (pl >= sh.poff[slot + 1]) ++slot;
-                Item it;
-                it.f = (unsigned)pair_face[sh.pstart[slot] + (pl - sh.poff[slot])];
-                it.w1 = (unsigned)slot | ((unsigned)k << 5) | ((unsigned)(pl - sh.poff[slot]) << 8);
-                it.w2 = 0; it.w3 = 0;
-                bnb_process(sh, spill, S, fcoef, it, cnt, t_tie, tau_exit, theta, max_level);
-            }
-            __syncthreads();
-            if (sh.top > NP_QCAP / 2 || sh.ntop >= NP_THREADS) drain();
-        }
-        drain();
-        // ---- S6: decide (nearest face, dot with its outward normal; ties L294)
-        if (tid < nslots) {
-            const int slot = tid;
-            const int e = sh.elem[slot];
-            const double dmin = u2d(sh.dmin[slot]);
-            if (sh.cut[slot]) { labels[e] = DC_CUT; sdist[e] = 0.0; }
-            else if (dmin <= tau) { labels[e] = DC_CUT; sdist[e] = 0.0; if (dmin >= tau - amb) ++n_amb; }
-            else if (dmin < INFINITY) {
-                if (dmin <= tau + amb) ++n_amb;
-                int bestmag = -1, neg = 0, npos = 0, nneg = 0;
-                const long long p0 = sh.pstart[slot];
-                for (int p = 0; p < sh.pcnt[slot]; ++p) {
-                    const unsigned long long key = __ldcg(pair_key + p0 + p);
-                    const double dk = u2d(key & ~0xffull);
-                    if (dk <= dmin + t_tie) {
-                        const int code = (int)(key & 0xff), mag = code & 0x7f, ng = code >> 7;
-                        if (ng) ++nneg; else ++npos;
-                        if (mag > bestmag) { bestmag = mag; neg = ng; }
-                    }
-                }
-                if (npos && nneg) ++n_samb;
-                labels[e] = neg ? DC_HOLE : DC_NORMAL;
-                const double d = fmin(dmin, d_band);
-                sdist[e] = neg ? -d : d;
-            }
-        }
-    }
-    // ---- counters
-    unsigned v[7] = { cnt.nodes, cnt.newton, cnt.iters, cnt.fail, cnt.depth, n_amb, n_samb };
-#pragma unroll
-    for (int i = 0; i < 7; ++i)
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
-    if (lane == 0) {
-        if (v[0]) atomicAdd(&S->c_bnb_nodes, (unsigned long long)v[0]);
-        if (v[1]) atomicAdd(&S->c_newton, (unsigned long long)v[1]);
-        if (v[2]) atomicAdd(&S->c_newton_iters, (unsigned long long)v[2]);
-        if (v[3]) atomicAdd(&S->c_newton_fail, (unsigned long long)v[3]);
-        if (v[4]) atomicAdd(&S->c_depth_exceeded, (unsigned long long)v[4]);
-        if (v[5]) atomicAdd(&S->c_ambiguous, (unsigned long long)v[5]);
-        if (v[6]) atomicAdd(&S->c_sign_ambiguous, (unsigned long long)v[6]);
-    }
-    __syncthreads();
-    if (tid == 0) atomicMax(&S->c_queue_peak, (unsigned long long)sh.peak);
-}
+#include "dc_narrow.cuh"
 
 // ------------------------------------------------------------------------------------------
 // S7: flood fill = connected components of the face-adjacency graph of non-CUT elements
@@ -919,7 +633,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                         for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
                         recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
                     }
-                    const NewtonOut o = newton_leaf(CP, CQ, tol_d, -1.0, NP_NEWTON_ITERS);
+                    const NewtonOut o = newton_leaf(CP, CQ, tol_d, -1.0, NP_NEWTON_ITERS_SL);
                     atomicMin(&s_best, d2u(o.dist));
                     if (o.dist < my_d - t_tie || (o.dist <= my_d + t_tie && fabs(o.cosv) > fabs(my_c))) {
                         my_d = fmin(my_d, o.dist); my_c = o.cosv;
@@ -1001,8 +715,8 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, doubl
 // host side
 // ==========================================================================================
 struct dc_ctx {
-    int device, num_sms, narrow_blocks;
-    long long n_nodes, n_elem, max_faces, max_pairs, n_face;
+    int device, num_sms;
+    long long n_nodes, n_elem, max_faces, max_pairs, n_face, max_band, qcap;
     const double *xyz; const int *conn; const int *adj;
     const double *face_nodes;
     // workspace partition
@@ -1011,11 +725,13 @@ struct dc_ctx {
     double *ebox;             // [6][n_elem]
     int *adj_own;             // [n_elem][6] (derived) or NULL
     int *parent; unsigned char *comp;
-    int *act_elem; long long *act_start; int *act_cnt;
+    int *act_elem;
+    int *band_elem; long long *band_start; int *band_cnt;
+    double *ecoef, *pbox; unsigned long long *best, *dmin;
+    NItem *q[2], *nq;
     int *pair_face; unsigned long long *pair_key;
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
     int *cell_count, *cell_start, *cell_fill;
-    Item *spill;
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
     cudaEvent_t ev[10];
     cudaStream_t last_stream;
@@ -1027,12 +743,20 @@ struct dc_ctx {
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_act_elem, off_act_start, off_act_cnt,
+    size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
+        off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq,
         off_pair_face, off_pair_key, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
-        off_cell_count, off_cell_start, off_cell_fill, off_spill, off_hfaces, off_hlabels, off_hsdist, total;
+        off_cell_count, off_cell_start, off_cell_fill, off_hfaces, off_hlabels, off_hsdist, total;
+    long long max_band, qcap;
 };
 
-#define DC_MAX_NARROW_BLOCKS (148 * 4)
+// capacities derived from max_pairs: band elements (each has >= 1 pair, ~25 in the configs) and
+// narrow-phase queue items per round
+static long long band_capacity(long long n_elem, long long max_pairs)
+{
+    long long b = max_pairs / 8; if (b < 65536) b = 65536; if (b > n_elem) b = n_elem; return b;
+}
+static long long queue_capacity(long long max_pairs) { return max_pairs < (1LL << 20) ? (1LL << 20) : max_pairs; }
 
 static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_faces, long long max_pairs)
 {
@@ -1044,8 +768,18 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_parent = take((size_t)n_elem * 4);
     L.off_comp = take((size_t)n_elem + 4);
     L.off_act_elem = take((size_t)n_elem * 4);
-    L.off_act_start = take((size_t)n_elem * 8);
-    L.off_act_cnt = take((size_t)n_elem * 4);
+    L.max_band = band_capacity(n_elem, max_pairs);
+    L.qcap = queue_capacity(max_pairs);
+    L.off_band_elem = take((size_t)L.max_band * 4);
+    L.off_band_start = take((size_t)L.max_band * 8);
+    L.off_band_cnt = take((size_t)L.max_band * 4);
+    L.off_ecoef = take((size_t)L.max_band * 6 * 28 * 8);
+    L.off_pbox = take((size_t)L.max_band * 36 * 8);
+    L.off_best = take((size_t)L.max_band * 8);
+    L.off_dmin = take((size_t)L.max_band * 8);
+    L.off_q0 = take((size_t)L.qcap * sizeof(NItem));
+    L.off_q1 = take((size_t)L.qcap * sizeof(NItem));
+    L.off_nq = take((size_t)(L.qcap > L.max_band ? L.qcap : L.max_band) * sizeof(NItem));
     // pair arrays double as the scratch of the adjacency derivation (2 x n_nodes ints)
     size_t pf = (size_t)max_pairs * 4, pk = (size_t)max_pairs * 8;
     size_t need_adj = (size_t)n_nodes * 8;
@@ -1060,7 +794,6 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_cell_count = take((size_t)(DC_NCELL + 1) * 4);
     L.off_cell_start = take((size_t)(DC_NCELL + 1) * 4);
     L.off_cell_fill = take((size_t)(DC_NCELL + 1) * 4);
-    L.off_spill = take((size_t)DC_MAX_NARROW_BLOCKS * NP_SPILL * sizeof(Item));
     L.off_hfaces = take((size_t)max_faces * 27 * 8);
     L.off_hlabels = take((size_t)n_elem);
     L.off_hsdist = take((size_t)n_elem * 8);
@@ -1116,8 +849,17 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->parent = (int *)(c->ws + L.off_parent);
     c->comp = c->ws + L.off_comp;
     c->act_elem = (int *)(c->ws + L.off_act_elem);
-    c->act_start = (long long *)(c->ws + L.off_act_start);
-    c->act_cnt = (int *)(c->ws + L.off_act_cnt);
+    c->max_band = L.max_band; c->qcap = L.qcap;
+    c->band_elem = (int *)(c->ws + L.off_band_elem);
+    c->band_start = (long long *)(c->ws + L.off_band_start);
+    c->band_cnt = (int *)(c->ws + L.off_band_cnt);
+    c->ecoef = (double *)(c->ws + L.off_ecoef);
+    c->pbox = (double *)(c->ws + L.off_pbox);
+    c->best = (unsigned long long *)(c->ws + L.off_best);
+    c->dmin = (unsigned long long *)(c->ws + L.off_dmin);
+    c->q[0] = (NItem *)(c->ws + L.off_q0);
+    c->q[1] = (NItem *)(c->ws + L.off_q1);
+    c->nq = (NItem *)(c->ws + L.off_nq);
     c->pair_face = (int *)(c->ws + L.off_pair_face);
     c->pair_key = (unsigned long long *)(c->ws + L.off_pair_key);
     c->fbox_orig = (double *)(c->ws + L.off_fbox_orig);
@@ -1128,7 +870,6 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->cell_count = (int *)(c->ws + L.off_cell_count);
     c->cell_start = (int *)(c->ws + L.off_cell_start);
     c->cell_fill = (int *)(c->ws + L.off_cell_fill);
-    c->spill = (Item *)(c->ws + L.off_spill);
     c->h_faces_dev = (double *)(c->ws + L.off_hfaces);
     c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
     c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
@@ -1136,12 +877,6 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->last_stream = st;
     for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->ev[i]));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
-    CK(cudaFuncSetAttribute(k_narrow, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NarrowShared)));
-    int occ = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_narrow, NP_THREADS, sizeof(NarrowShared)));
-    if (occ < 1) occ = 1;
-    c->narrow_blocks = c->num_sms * occ;
-    if (c->narrow_blocks > DC_MAX_NARROW_BLOCKS) c->narrow_blocks = DC_MAX_NARROW_BLOCKS;
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
     int rc = run_elem_boxes(c, st);
     if (rc != DC_OK) { delete c; return rc; }
@@ -1198,14 +933,31 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     CK(cudaEventRecord(c->ev[0], st));
     if (P.flags & DC_FLAG_RECOMPUTE_BOXES) { int rc = run_elem_boxes(c, st); if (rc) return rc; }
     CK(cudaEventRecord(c->ev[1], st));
-    k_setup_classify<<<1, 1, 0, st>>>(c->S, P);
+    k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
     k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_count, c->act_elem);
     k_pairs<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
-                                           c->act_start, c->act_cnt, c->pair_face, c->pair_key);
+                                           c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key);
     CK(cudaEventRecord(c->ev[2], st));
-    k_narrow<<<c->narrow_blocks, NP_THREADS, sizeof(NarrowShared), st>>>(c->S, c->xyz, c->conn, c->act_elem, c->act_start,
-                                                                         c->act_cnt, c->pair_face, c->pair_key, c->fcoef,
-                                                                         c->spill, labels_dev, sdist_dev);
+    // ---- S5: wavefront narrow phase (dc_narrow.cuh)
+    const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
+    DcScalars *S = c->S;
+    k_np_stage<<<gw, NPW_THREADS, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fcoef,
+                                           c->ecoef, c->pbox, c->best, c->dmin, c->nq);
+    // seed solves: one per band element, queue = nq[0 .. n_band); failures are never re-split
+    k_np_newton<<<gw, NPW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
+                                            c->q[0], &S->qn[0], c->qcap);
+    k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
+                                           c->q[0], &S->qn[0], c->qcap);
+    const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
+    const int rounds = 2 * max_level + 1;
+    for (int r = 0; r < rounds; ++r) {
+        k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, &S->nn[r], c->qcap);
+        k_np_newton<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[r], c->qcap, c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
+                                                c->q[(r + 1) & 1], &S->qn[r + 1], c->qcap);
+    }
+    k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
+                                                                              c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
     k_uf_union<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, c->adj, ne, c->parent);
     k_uf_seed<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, ne, c->parent, c->comp);
@@ -1214,7 +966,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
-    c->launches_classify = 9 + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
+    c->launches_classify = 12 + 2 * rounds + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }
@@ -1259,12 +1011,12 @@ extern "C" long long dc_get_pairs(dc_ctx *c, int *elem_host, int *face_host, lon
     if (!c->have_cut) return DC_ERR_STATE;
     CK(cudaStreamSynchronize(c->last_stream));
     CK(cudaMemcpy(c->S_host, c->S, sizeof(DcScalars), cudaMemcpyDeviceToHost));
-    const int na = c->S_host->n_active;
+    const int na = c->S_host->n_band < (int)c->max_band ? c->S_host->n_band : (int)c->max_band;
     int *ae = new int[na > 0 ? na : 1]; long long *as = new long long[na > 0 ? na : 1]; int *ac = new int[na > 0 ? na : 1];
     int *perm = new int[c->n_face];
-    cudaMemcpy(ae, c->act_elem, (size_t)na * 4, cudaMemcpyDeviceToHost);
-    cudaMemcpy(as, c->act_start, (size_t)na * 8, cudaMemcpyDeviceToHost);
-    cudaMemcpy(ac, c->act_cnt, (size_t)na * 4, cudaMemcpyDeviceToHost);
+    cudaMemcpy(ae, c->band_elem, (size_t)na * 4, cudaMemcpyDeviceToHost);
+    cudaMemcpy(as, c->band_start, (size_t)na * 8, cudaMemcpyDeviceToHost);
+    cudaMemcpy(ac, c->band_cnt, (size_t)na * 4, cudaMemcpyDeviceToHost);
     cudaMemcpy(perm, c->fperm, (size_t)c->n_face * 4, cudaMemcpyDeviceToHost);
     long long np = (long long)c->S_host->n_pairs; if (np > c->max_pairs) np = c->max_pairs;
     int *pf = new int[np > 0 ? np : 1];

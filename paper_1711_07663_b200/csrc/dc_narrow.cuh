@@ -1,0 +1,411 @@
+// dc_narrow.cuh -- S5 (narrow phase) and S6 (decide) as a WAVEFRONT of small uniform kernels.
+//
+// Every kernel does one operation on one item per thread and compacts its output into a global
+// queue (warp-aggregated atomics), so warps stay full and no kernel carries another's registers:
+//
+//   k_np_stage   warp / band element : gather the 27 nodes (coalesced conn row), monomial coefficients
+//                                      and Bezier boxes of the 6 boundary patches -> ecoef, pbox;
+//                                      centre-centre distances of all (pair, patch) -> first upper
+//                                      bound best[b] and ONE seed item per element
+//   k_np_newton  thread / item       : projected Newton (Eq. 3-5 L256-L270 generalised to two patches,
+//                                      clamp L272-L278) on a leaf; min into best/dmin/pair_key;
+//                                      an unconverged non-seed leaf is re-split
+//   k_np_roots   warp / band element : (pair, patch) whose boxes are within best + t_tie (A.2,
+//                                      L689-L709) become root items
+//   k_np_bound   thread / item       : bound_node -> prune / 4 children / leaf
+//   k_np_decide  thread / band elem  : S6 (L215 nearest face and its normal; tie rule L294)
+//
+// Round r = k_np_bound(r) + k_np_newton(r): every item of round r has lP + lQ = r, so 2 max_level + 1
+// rounds always terminate the branch and bound; empty rounds exit at once.
+#pragma once
+
+#define NPW_THREADS 128
+#define NP_NEWTON_ITERS 40
+#define DC_MAX_ROUNDS 25            /* 2 * 12 + 1 */
+
+struct __align__(16) NItem { unsigned p, ak, w2, w3; };
+// p : global pair index (face = pair_face[p], key slot = pair_key[p])
+// ak: band index b (29 bits) | boundary patch k << 29
+// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20
+// w3: is(12) | it(12)<<12 | flags(8)<<24      flags bit0: seed solve (no re-split on failure)
+
+struct NpCounters { unsigned nodes, newton, iters, fail, depth; };
+
+__device__ __forceinline__ double u2d(unsigned long long b) { return __longlong_as_double((long long)b); }
+__device__ __forceinline__ unsigned long long d2u(double d) { return (unsigned long long)__double_as_longlong(d); }
+
+__device__ __forceinline__ void nitem_box(const NItem &it, double &uc, double &vc, double &hP,
+                                          double &sc, double &tc, double &hQ)
+{
+    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+    const int iu = (it.w2 >> 8) & 0xfff, iv = (it.w2 >> 20) & 0xfff;
+    const int is = it.w3 & 0xfff, itt = (it.w3 >> 12) & 0xfff;
+    hP = __longlong_as_double((long long)(1023 - lP) << 52);
+    hQ = __longlong_as_double((long long)(1023 - lQ) << 52);
+    uc = fma((double)(2 * iu + 1), hP, -1.0); vc = fma((double)(2 * iv + 1), hP, -1.0);
+    sc = fma((double)(2 * is + 1), hQ, -1.0); tc = fma((double)(2 * itt + 1), hQ, -1.0);
+}
+
+__device__ __forceinline__ NItem nitem_child(const NItem &it, bool splitP, int c)
+{
+    const unsigned lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+    const unsigned iu = (it.w2 >> 8) & 0xfff, iv = (it.w2 >> 20) & 0xfff;
+    const unsigned is = it.w3 & 0xfff, itt = (it.w3 >> 12) & 0xfff;
+    NItem ch; ch.p = it.p; ch.ak = it.ak;
+    if (splitP) {
+        ch.w2 = (lP + 1) | (lQ << 4) | ((2 * iu + (c & 1)) << 8) | ((2 * iv + (c >> 1)) << 20);
+        ch.w3 = it.w3 & 0x00ffffffu;
+    } else {
+        ch.w2 = lP | ((lQ + 1) << 4) | (iu << 8) | (iv << 20);
+        ch.w3 = (2 * is + (c & 1)) | ((2 * itt + (c >> 1)) << 12);
+    }
+    return ch;
+}
+
+// choose which patch a node splits (never beyond max_level); false = nothing left to split
+__device__ __forceinline__ bool choose_split(const NItem &it, bool wantP, int max_level, bool &splitP)
+{
+    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
+    splitP = wantP;
+    if (splitP && lP >= max_level) splitP = false;
+    if (!splitP && lQ >= max_level) {
+        if (lP < max_level) splitP = true;
+        else return false;
+    }
+    return true;
+}
+
+// warp-aggregated append of `n_mine` (0 or `per`) items per lane; returns this lane's first slot or -1
+__device__ __forceinline__ long long warp_reserve(int *counter, bool mine, int per, long long cap, int *status)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, mine);
+    if (!m) return -1;
+    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(counter, __popc(m) * per);
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (!mine) return -1;
+    const long long slot = (long long)base + (long long)__popc(m & ((1u << lane) - 1)) * per;
+    if (slot + per > cap) { atomicOr(status, DC_STATUS_QUEUE_OVERFLOW); return -1; }
+    return slot;
+}
+
+__device__ __forceinline__ void np_flush_counters(DcScalars *S, const NpCounters &c)
+{
+    unsigned v[5] = { c.nodes, c.newton, c.iters, c.fail, c.depth };
+#pragma unroll
+    for (int i = 0; i < 5; ++i)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    if ((threadIdx.x & 31) == 0) {
+        if (v[0]) atomicAdd(&S->c_bnb_nodes, (unsigned long long)v[0]);
+        if (v[1]) atomicAdd(&S->c_newton, (unsigned long long)v[1]);
+        if (v[2]) atomicAdd(&S->c_newton_iters, (unsigned long long)v[2]);
+        if (v[3]) atomicAdd(&S->c_newton_fail, (unsigned long long)v[3]);
+        if (v[4]) atomicAdd(&S->c_depth_exceeded, (unsigned long long)v[4]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Stage: one warp per band element.  ecoef [b][6][28] (27 monomial coefficients [coord][9] + the
+// higher-order constant K), pbox [b][6][6] (Bezier box of each boundary patch).
+#define ST_WARPS (NPW_THREADS / 32)
+__global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
+                                                          const int *__restrict__ band_elem, const long long *__restrict__ band_start,
+                                                          const int *__restrict__ band_cnt, const int *__restrict__ pair_face,
+                                                          const double *__restrict__ fcoef, double *__restrict__ ecoef,
+                                                          double *__restrict__ pbox, unsigned long long *__restrict__ best,
+                                                          unsigned long long *__restrict__ dmin, NItem *__restrict__ nq)
+{
+    __shared__ double s_nodes[ST_WARPS][81];
+    __shared__ double s_coef[ST_WARPS][6 * 28];
+    __shared__ double s_box[ST_WARPS][36];
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int n_band = min(S->n_band, S->max_band);
+    const double reach = S->reach;
+    double *nd = s_nodes[wl], *cf = s_coef[wl], *bx = s_box[wl];
+    for (int b = warp; b < n_band; b += nwarps) {
+        const int e = band_elem[b];
+        if (lane < 27) {
+            const int id = __ldg(conn + (size_t)e * 27 + lane);
+            const double *p = xyz + (size_t)id * 3;
+            nd[lane * 3 + 0] = __ldg(p); nd[lane * 3 + 1] = __ldg(p + 1); nd[lane * 3 + 2] = __ldg(p + 2);
+        }
+        __syncwarp();
+        if (lane < 18) {
+            const int k = lane / 3, c = lane % 3;
+            double x[9], a[9];
+#pragma unroll
+            for (int m = 0; m < 9; ++m) x[m] = nd[c_face_node[k][m] * 3 + c];
+            nodes_to_mono9(x, a);
+#pragma unroll
+            for (int m = 0; m < 9; ++m) cf[k * 28 + c * 9 + m] = a[m];
+            // Bezier box of the patch (convex-hull property)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) x[3 * j + 1] = bez_mid(x[3 * j], x[3 * j + 1], x[3 * j + 2]);
+#pragma unroll
+            for (int i = 0; i < 3; ++i) x[i + 3] = bez_mid(x[i], x[i + 3], x[i + 6]);
+            double lo = x[0], hi = x[0];
+#pragma unroll
+            for (int m = 1; m < 9; ++m) { lo = fmin(lo, x[m]); hi = fmax(hi, x[m]); }
+            bx[k * 6 + c] = lo; bx[k * 6 + 3 + c] = hi;
+        }
+        __syncwarp();
+        if (lane < 6) cf[lane * 28 + 27] = higher_order_const(cf + lane * 28);
+        __syncwarp();
+        for (int i = lane; i < 6 * 28; i += 32) ecoef[(size_t)b * (6 * 28) + i] = cf[i];
+        for (int i = lane; i < 36; i += 32) pbox[(size_t)b * 36 + i] = bx[i];
+        // centre-centre distances of every (pair, patch): attained => upper bound; the smallest seeds Newton
+        const long long p0 = band_start[b];
+        const int total = band_cnt[b] * 6;
+        unsigned long long key = ~0ull;
+        for (int t = lane; t < total; t += 32) {
+            const int pl = t / 6, k = t - pl * 6;
+            const int f = __ldg(pair_face + p0 + pl);
+            const double *AQ = fcoef + (size_t)f * 28;
+            const double dx = cf[k * 28] - __ldg(AQ), dy = cf[k * 28 + 9] - __ldg(AQ + 9), dz = cf[k * 28 + 18] - __ldg(AQ + 18);
+            const double d = sqrt(dx * dx + dy * dy + dz * dz);
+            const unsigned long long kk = (d2u(d) & ~0xfffffull) | (unsigned long long)min(t, 0xfffff);
+            key = kk < key ? kk : key;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, key, o); key = v < key ? v : key; }
+        if (lane == 0) {
+            // the truncated key distance is <= the attained one: round up to stay an upper bound
+            const double dkey = u2d((key & ~0xfffffull) + 0x100000ull);
+            best[b] = d2u(fmin(reach, dkey));
+            dmin[b] = 0x7ff0000000000000ull;
+            const int t = (int)(key & 0xfffffull);
+            const int pl = t / 6, k = t - pl * 6;
+            NItem it; it.p = (unsigned)(p0 + pl); it.ak = (unsigned)b | ((unsigned)k << 29); it.w2 = 0; it.w3 = 1u << 24;
+            nq[b] = it;
+        }
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Newton: one thread per leaf item of queue nq[0 .. *n_items).
+__global__ void __launch_bounds__(NPW_THREADS) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, const NItem *__restrict__ nq,
+                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                                           unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
+                                                           NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
+{
+    const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
+    if (n == 0) return;
+    const double tol_d = S->tol_d, tau_exit = S->tau_exit;
+    const int max_level = S->max_level;
+    NpCounters cnt = { 0, 0, 0, 0, 0 };
+    const int stride = gridDim.x * blockDim.x;
+    const int n_round = (n + 31) & ~31;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        bool resplit = false, splitP = false;
+        NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
+        if (i < n) {
+            it = nq[i];
+            const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+            if (u2d(__ldcg(best + b)) > tau_exit) {
+                double uc, vc, hP, sc, tc, hQ;
+                nitem_box(it, uc, vc, hP, sc, tc, hQ);
+                const double *AP = ecoef + ((size_t)b * 6 + k) * 28;
+                const double *AQ = fcoef + (size_t)__ldg(pair_face + it.p) * 28;
+                double CP[27], CQ[27];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    double A[9];
+#pragma unroll
+                    for (int m = 0; m < 9; ++m) A[m] = __ldg(AP + c * 9 + m);
+                    recentre9(A, uc, vc, hP, hP, CP + 9 * c);
+#pragma unroll
+                    for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
+                    recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
+                }
+                const NewtonOut o = newton_leaf(CP, CQ, tol_d, tau_exit, NP_NEWTON_ITERS);
+                cnt.newton++; cnt.iters += o.iters;
+                atomicMin(best + b, d2u(o.dist));
+                if (o.dist > tau_exit) {
+                    atomicMin(dmin + b, d2u(o.dist));
+                    const unsigned long long key = (d2u(o.dist) & ~0xffull) | (unsigned long long)cos_code(o.cosv);
+                    atomicMin(pair_key + it.p, key);
+                    if (!o.converged && !((it.w3 >> 24) & 1)) {
+                        cnt.fail++;
+                        resplit = choose_split(it, hP >= hQ, max_level, splitP);
+                    }
+                }
+            }
+        }
+        const long long slot = warp_reserve(qout_n, resplit, 4, qcap, &S->status);
+        if (slot >= 0) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) qout[slot + c] = nitem_child(it, splitP, c);
+        }
+    }
+    np_flush_counters(S, cnt);
+}
+
+// ------------------------------------------------------------------------------------------
+// Roots: one warp per band element, lanes over its pairs.  (pair, patch k) survives when the
+// box distance (Algorithm A.2) of the patch's Bezier box and the face's Bezier box is
+// within best + t_tie; survivors become the items of round 0.
+__global__ void __launch_bounds__(NPW_THREADS) k_np_roots(DcScalars *S, const long long *__restrict__ band_start,
+                                                          const int *__restrict__ band_cnt, const int *__restrict__ pair_face,
+                                                          const double *__restrict__ fbox, const double *__restrict__ pbox,
+                                                          const unsigned long long *__restrict__ best,
+                                                          NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int n_band = min(S->n_band, S->max_band);
+    const double t_tie = S->t_tie, tau_exit = S->tau_exit;
+    for (int b = warp; b < n_band; b += nwarps) {
+        const double bst = u2d(best[b]);
+        if (bst <= tau_exit) continue;                      // already CUT
+        const double cut = bst + t_tie, cut2 = cut * cut;
+        const long long p0 = band_start[b];
+        const int cnt = band_cnt[b];
+        const double *pb = pbox + (size_t)b * 36;
+        for (int base = 0; base < cnt; base += 32) {
+            const int pl = base + lane;
+            unsigned mask = 0;
+            if (pl < cnt) {
+                const int f = __ldg(pair_face + p0 + pl);
+                double fb[6];
+#pragma unroll
+                for (int m = 0; m < 6; ++m) fb[m] = __ldg(fbox + (size_t)f * 6 + m);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) {
+                    double d2 = 0.0;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        const double g = fmax(0.0, fmax(fb[c] - __ldg(pb + k * 6 + 3 + c), __ldg(pb + k * 6 + c) - fb[3 + c]));
+                        d2 = fma(g, g, d2);
+                    }
+                    if (d2 <= cut2) mask |= 1u << k;
+                }
+            }
+            const int mine = __popc(mask);
+            int incl = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            if (total == 0) continue;
+            int start = 0;
+            if (lane == 31) start = atomicAdd(qout_n, total);
+            start = __shfl_sync(0xffffffffu, start, 31);
+            long long slot = (long long)start + incl - mine;
+            if ((long long)start + total > qcap) { if (lane == 0) atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW); continue; }
+            while (mask) {
+                const int k = __ffs(mask) - 1; mask &= mask - 1;
+                NItem it; it.p = (unsigned)(p0 + pl); it.ak = (unsigned)b | ((unsigned)k << 29); it.w2 = 0; it.w3 = 0;
+                qout[slot++] = it;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Bound: one thread per item of qin[0 .. *n_in): prune, or 4 children -> qout, or leaf -> nq.
+__global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
+                                                          const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                                          const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                                          NItem *__restrict__ qout, int *__restrict__ qout_n,
+                                                          NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap)
+{
+    const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
+    if (n == 0) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
+    const double t_tie = S->t_tie, tau_exit = S->tau_exit, theta2 = S->theta * S->theta;
+    const int max_level = S->max_level;
+    NpCounters cnt = { 0, 0, 0, 0, 0 };
+    const int stride = gridDim.x * blockDim.x;
+    const int n_round = (n + 31) & ~31;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        bool split = false, leaf = false, splitP = false;
+        NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
+        if (i < n) {
+            it = qin[i];
+            const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+            double bst = u2d(__ldcg(best + b));
+            if (bst > tau_exit) {
+                double uc, vc, hP, sc, tc, hQ;
+                nitem_box(it, uc, vc, hP, sc, tc, hQ);
+                const double *APg = ecoef + ((size_t)b * 6 + k) * 28;
+                const double *AQg = fcoef + (size_t)__ldg(pair_face + it.p) * 28;
+                double AP[28], AQ[28];
+#pragma unroll
+                for (int m = 0; m < 14; ++m) {
+                    const double2 vp = __ldg(reinterpret_cast<const double2 *>(APg) + m);
+                    const double2 vq = __ldg(reinterpret_cast<const double2 *>(AQg) + m);
+                    AP[2 * m] = vp.x; AP[2 * m + 1] = vp.y; AQ[2 * m] = vq.x; AQ[2 * m + 1] = vq.y;
+                }
+                const NodeOut o = bound_node(AP, AQ, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
+                cnt.nodes++;
+                if (o.dist_c < bst) { atomicMin(best + b, d2u(o.dist_c)); bst = o.dist_c; }
+                if (o.dist_c > tau_exit && o.lb <= bst + t_tie) {
+                    leaf = o.leaf;
+                    if (!leaf) {
+                        split = choose_split(it, o.splitP, max_level, splitP);
+                        if (!split) { leaf = true; cnt.depth++; }
+                    }
+                }
+            }
+        }
+        const long long sl = warp_reserve(nq_n, leaf, 1, qcap, &S->status);
+        if (sl >= 0) nq[sl] = it;
+        const long long slot = warp_reserve(qout_n, split, 4, qcap, &S->status);
+        if (slot >= 0) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) qout[slot + c] = nitem_child(it, splitP, c);
+        }
+    }
+    np_flush_counters(S, cnt);
+}
+
+// ------------------------------------------------------------------------------------------
+// S6 decide (L215: nearest face, dot of the minimal vector with its outward normal; ties L294):
+// one thread per band element.
+__global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, const long long *__restrict__ band_start,
+                            const int *__restrict__ band_cnt, const unsigned long long *__restrict__ best,
+                            const unsigned long long *__restrict__ dmin_arr, const unsigned long long *__restrict__ pair_key,
+                            signed char *__restrict__ labels, double *__restrict__ sdist)
+{
+    const int n_band = min(S->n_band, S->max_band);
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    const double tau = S->tau, tau_exit = S->tau_exit, amb = S->amb, t_tie = S->t_tie, d_band = S->d_band;
+    unsigned n_amb = 0, n_samb = 0;
+    if (b < n_band) {
+        const int e = band_elem[b];
+        const double dmin = u2d(dmin_arr[b]);
+        if (u2d(best[b]) <= tau_exit) { labels[e] = DC_CUT; sdist[e] = 0.0; }
+        else if (dmin <= tau) { labels[e] = DC_CUT; sdist[e] = 0.0; if (dmin >= tau - amb) ++n_amb; }
+        else if (dmin < INFINITY) {
+            if (dmin <= tau + amb) ++n_amb;
+            int bestmag = -1, neg = 0, npos = 0, nneg = 0;
+            const long long p0 = band_start[b];
+            const int cnt = band_cnt[b];
+            for (int p = 0; p < cnt; ++p) {
+                const unsigned long long key = pair_key[p0 + p];
+                const double dk = u2d(key & ~0xffull);
+                if (dk <= dmin + t_tie) {
+                    const int code = (int)(key & 0xff), mag = code & 0x7f, ng = code >> 7;
+                    if (ng) ++nneg; else ++npos;
+                    if (mag > bestmag) { bestmag = mag; neg = ng; }
+                }
+            }
+            if (npos && nneg) ++n_samb;
+            labels[e] = neg ? DC_HOLE : DC_NORMAL;
+            const double d = fmin(dmin, d_band);
+            sdist[e] = neg ? -d : d;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { n_amb += __shfl_xor_sync(0xffffffffu, n_amb, o); n_samb += __shfl_xor_sync(0xffffffffu, n_samb, o); }
+    if ((threadIdx.x & 31) == 0) {
+        if (n_amb) atomicAdd(&S->c_ambiguous, (unsigned long long)n_amb);
+        if (n_samb) atomicAdd(&S->c_sign_ambiguous, (unsigned long long)n_samb);
+    }
+}
