@@ -20,6 +20,7 @@
 
 #include "../../include/dc.h"
 #include "dc_geom.cuh"
+#include "dc_newton.cuh"
 
 using namespace dcg;
 
@@ -54,6 +55,7 @@ struct DcScalars {
     int status;
     int qn[DC_NQN];                 // items of round r (children queue, ping-pong buffers)
     int nn[DC_NQN];                 // leaves of round r (Newton queue)
+    int nh[DC_NQN + 1];             // Newton queue heads: [0] seed pass, [r + 1] round r
     unsigned long long n_pairs;
     int seedless_elem[DC_MAX_SEEDLESS];
     // counters
@@ -319,7 +321,8 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
     S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.125;
     S->max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->status = 0; S->n_pairs = 0ull;
-    for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; }
+    for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; S->nh[i] = 0; }
+    S->nh[DC_NQN] = 0;
     S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
     S->c_depth_exceeded = S->c_cut = S->c_hole = S->c_normal = S->c_ambiguous = 0ull;
     S->c_sign_ambiguous = S->c_fill_conflicts = S->c_queue_peak = S->c_seedless_total = 0ull;
@@ -876,6 +879,8 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->ev[i]));
+    CK(cudaFuncSetAttribute(k_np_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, NW_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_np_newton, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
     int rc = run_elem_boxes(c, st);
@@ -944,7 +949,8 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_stage<<<gw, NPW_THREADS, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fcoef,
                                            c->ecoef, c->pbox, c->best, c->dmin, c->nq);
     // seed solves: one per band element, queue = nq[0 .. n_band); failures are never re-split
-    k_np_newton<<<gw, NPW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
+    const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
                                             c->q[0], &S->qn[0], c->qcap);
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
                                            c->q[0], &S->qn[0], c->qcap);
@@ -953,7 +959,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     for (int r = 0; r < rounds; ++r) {
         k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, &S->nn[r], c->qcap);
-        k_np_newton<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[r], c->qcap, c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
+        k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[r], c->qcap, &S->nh[r + 1], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
                                                 c->q[(r + 1) & 1], &S->qn[r + 1], c->qcap);
     }
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,

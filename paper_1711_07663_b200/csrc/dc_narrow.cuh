@@ -7,7 +7,7 @@
 //                                      and Bezier boxes of the 6 boundary patches -> ecoef, pbox;
 //                                      centre-centre distances of all (pair, patch) -> first upper
 //                                      bound best[b] and ONE seed item per element
-//   k_np_newton  thread / item       : projected Newton (Eq. 3-5 L256-L270 generalised to two patches,
+//   k_np_newton  persistent warps    : projected Newton (Eq. 3-5 L256-L270 generalised to two patches,
 //                                      clamp L272-L278) on a leaf; min into best/dmin/pair_key;
 //                                      an unconverged non-seed leaf is re-split
 //   k_np_roots   warp / band element : (pair, patch) whose boxes are within best + t_tie (A.2,
@@ -20,7 +20,6 @@
 #pragma once
 
 #define NPW_THREADS 128
-#define NP_NEWTON_ITERS 40
 #define DC_MAX_ROUNDS 25            /* 2 * 12 + 1 */
 
 struct __align__(16) NItem { unsigned p, ak, w2, w3; };
@@ -187,60 +186,121 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 }
 
 // ------------------------------------------------------------------------------------------
-// Newton: one thread per leaf item of queue nq[0 .. *n_items).
-__global__ void __launch_bounds__(NPW_THREADS) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, const NItem *__restrict__ nq,
-                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
-                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                           unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
-                                                           NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
+// Newton: PERSISTENT warps over the leaf queue nq[0 .. *n_items), one solve per lane, all lanes of a warp
+// in lockstep (dcn::iterate = exactly one value+gradient+Hessian evaluation), lanes whose solve has
+// finished are refilled from the queue (one warp-aggregated atomic on *head), so the iteration count of
+// one solve never holds up the other 31.  The two patches' 54 root monomial coefficients of every lane
+// live in shared memory, transposed (coefficient-major, lane-minor: conflict-free reads), which keeps the
+// kernel at <= 128 registers and 16 warps per SM; a refill is a warp-cooperative coalesced copy of the
+// 2 x 216 B of the new item (the odd stride makes the transposed store 2-way conflicted instead of 32).
+#define NW_THREADS 128
+#define NW_STRIDE 129
+#define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
+#define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
+
+__global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
+                                                            const NItem *__restrict__ nq,
+                                                            const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                                            const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                                            unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
+                                                            NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
 {
+    extern __shared__ double nw_sm[];
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
     if (n == 0) return;
-    const double tol_d = S->tol_d, tau_exit = S->tau_exit;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const double *slot = nw_sm + tid;
+    double *wslot = nw_sm + (tid & ~31);
+    const volatile double *vslot = slot;   // volatile: re-read in the line search instead of keeping 54 values live
+    auto cf = [&](int m) { return vslot[m * NW_STRIDE]; };
+    const double tau_exit = S->tau_exit, tol_d2 = S->tol_d * S->tol_d;
+    const double tau_exit2 = tau_exit > 0.0 ? tau_exit * tau_exit : -1.0;
     const int max_level = S->max_level;
     NpCounters cnt = { 0, 0, 0, 0, 0 };
-    const int stride = gridDim.x * blockDim.x;
-    const int n_round = (n + 31) & ~31;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
-        bool resplit = false, splitP = false;
-        NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
-        if (i < n) {
-            it = nq[i];
-            const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
-            if (u2d(__ldcg(best + b)) > tau_exit) {
-                double uc, vc, hP, sc, tc, hQ;
-                nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                const double *AP = ecoef + ((size_t)b * 6 + k) * 28;
-                const double *AQ = fcoef + (size_t)__ldg(pair_face + it.p) * 28;
-                double CP[27], CQ[27];
+    dcn::NwState s; s.phase = 0; s.iters = 0;
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    double A[9];
-#pragma unroll
-                    for (int m = 0; m < 9; ++m) A[m] = __ldg(AP + c * 9 + m);
-                    recentre9(A, uc, vc, hP, hP, CP + 9 * c);
-#pragma unroll
-                    for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
-                    recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
-                }
-                const NewtonOut o = newton_leaf(CP, CQ, tol_d, tau_exit, NP_NEWTON_ITERS);
-                cnt.newton++; cnt.iters += o.iters;
-                atomicMin(best + b, d2u(o.dist));
-                if (o.dist > tau_exit) {
-                    atomicMin(dmin + b, d2u(o.dist));
-                    const unsigned long long key = (d2u(o.dist) & ~0xffull) | (unsigned long long)cos_code(o.cosv);
-                    atomicMin(pair_key + it.p, key);
-                    if (!o.converged && !((it.w3 >> 24) & 1)) {
-                        cnt.fail++;
-                        resplit = choose_split(it, hP >= hQ, max_level, splitP);
+    for (int i = 0; i < 4; ++i) s.x[i] = 0.0;
+    NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
+    bool exhausted = false;
+    while (true) {
+        // ---- refill idle lanes
+        for (int pass = 0; pass < 4; ++pass) {
+            const bool need = s.phase == 0 && !exhausted;
+            const unsigned mneed = __ballot_sync(0xffffffffu, need);
+            const unsigned mbusy = __ballot_sync(0xffffffffu, s.phase != 0);
+            if (!mneed || (__popc(mneed) < NW_REFILL && mbusy != 0)) break;
+            const int leader = __ffs(mneed) - 1;
+            int base = 0;
+            if (lane == leader) base = atomicAdd(head, __popc(mneed));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            bool fresh = false;
+            unsigned long long pA = 0, pQ = 0;
+            if (need) {
+                const int i = base + __popc(mneed & lt_mask);
+                if (i >= n) exhausted = true;
+                else {
+                    it = nq[i];
+                    const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+                    if (u2d(__ldcg(best + b)) > tau_exit) {          // else: the element is already CUT, drop the item
+                        fresh = true;
+                        double uc, vc, hP, sc, tc, hQ;
+                        nitem_box(it, uc, vc, hP, sc, tc, hQ);
+                        s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
+                        s.iters = 0; s.phase = 1;
+                        pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
+                        pQ = (unsigned long long)(fcoef + (size_t)__ldg(pair_face + it.p) * 28);
                     }
                 }
             }
+            unsigned mf = __ballot_sync(0xffffffffu, fresh);
+            const bool dropped = __ballot_sync(0xffffffffu, need && !fresh && !exhausted) != 0;
+            while (mf) {
+                const int L = __ffs(mf) - 1; mf &= mf - 1;
+                const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
+                const double *q = (const double *)__shfl_sync(0xffffffffu, pQ, L);
+                double *dst = wslot + L;
+                dst[lane * NW_STRIDE] = lane < 27 ? __ldg(a + lane) : __ldg(q + (lane - 27));
+                if (lane < 22) dst[(lane + 32) * NW_STRIDE] = __ldg(q + (lane + 5));
+            }
+            __syncwarp();
+            if (!dropped) break;
         }
-        const long long slot = warp_reserve(qout_n, resplit, 4, qcap, &S->status);
-        if (slot >= 0) {
+        if (__ballot_sync(0xffffffffu, s.phase != 0) == 0) {
+            if (__ballot_sync(0xffffffffu, !exhausted) == 0) break;
+            continue;
+        }
+        // ---- one evaluation per busy lane
+        bool fin = false;
+        dcn::NwResult R; R.dist = 0.0; R.cosv = 0.0; R.converged = 0;
+        if (s.phase != 0) {
+            // the leaf's box (dyadic, exact) is re-derived from the item every time instead of living in registers
+            double uc, vc, hP, sc, tc, hQ;
+            nitem_box(it, uc, vc, hP, sc, tc, hQ);
+            const double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };
+            fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R);
+        }
+        // ---- results of the solves that finished (an attained distance is an upper bound whether converged or not)
+        bool resplit = false, splitP = false;
+        if (fin) {
+            const unsigned b = it.ak & 0x1fffffffu;
+            cnt.newton++; cnt.iters += s.iters;
+            s.phase = 0;
+            atomicMin(best + b, d2u(R.dist));
+            if (R.dist > tau_exit) {
+                atomicMin(dmin + b, d2u(R.dist));
+                const unsigned long long key = (d2u(R.dist) & ~0xffull) | (unsigned long long)cos_code(R.cosv);
+                atomicMin(pair_key + it.p, key);
+                if (!R.converged && !((it.w3 >> 24) & 1)) {
+                    cnt.fail++;
+                    resplit = choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP);
+                }
+            }
+        }
+        const long long sl = warp_reserve(qout_n, resplit, 4, qcap, &S->status);
+        if (sl >= 0) {
 #pragma unroll
-            for (int c = 0; c < 4; ++c) qout[slot + c] = nitem_child(it, splitP, c);
+            for (int c = 0; c < 4; ++c) qout[sl + c] = nitem_child(it, splitP, c);
         }
     }
     np_flush_counters(S, cnt);

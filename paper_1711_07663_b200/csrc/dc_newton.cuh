@@ -1,0 +1,203 @@
+// dc_newton.cuh -- one iteration of the projected Newton closest-point solve between two biquadratic
+// patches, written so that a warp can run it in LOCKSTEP (every lane does exactly one evaluation of
+// value + gradient + Hessian per call) and lanes that finish are refilled from a queue.
+//
+// The solve is the two-patch generalisation of PAPER.md Eq. 3-5 (L256-L270): minimise
+//   f(x) = 1/2 |P(u,v) - Q(s,t)|^2,   x = (u,v,s,t) in the box [lo,hi]   (a leaf of the branch and bound),
+// with the paper's clamp to the reference box (L272-L278) as a projected step: variables at a bound whose
+// gradient pushes outward are held, the rest take a Levenberg-damped Newton step, the trial point is
+// clamped and accepted only if f does not increase.
+//
+// Both patches are evaluated straight from their ROOT monomial coefficients (no re-centring): the box
+// bounds are dyadic and exactly representable, so clamped variables sit exactly on sub-patch borders.
+// Coefficients are read through an accessor `cf(m)`: m = c*9 + i + 3j for P (c = x,y,z), 27 + ... for Q.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace dcn {
+
+#ifndef DCN_HD
+#define DCN_HD __host__ __device__ __forceinline__
+#endif
+
+#ifndef NW_LAM_TRIES
+#define NW_LAM_TRIES 11
+#define NW_LAM_GROW 10.0
+#endif
+#define NW_MAXIT 16                 /* evaluations per solve before it is declared unconverged */
+
+// state of one lane's solve
+struct NwState {
+    double x[4];
+    int iters;                      // evaluations done
+    int phase;                      // 0 idle, 1 iterating, 3 last evaluation of an unconverged solve
+};
+
+struct NwResult { double dist, cosv; int converged; };
+
+// value + first + second derivatives of one coordinate of a biquadratic at (a,b); C(m) = coefficient of a^i b^j, m = i+3j
+template <class CF>
+DCN_HD void jet(CF C, double a, double b, double &p, double &pa, double &pb, double &paa, double &pab, double &pbb)
+{
+    const double c0 = C(0), c1 = C(1), c2 = C(2), c3 = C(3), c4 = C(4), c5 = C(5), c6 = C(6), c7 = C(7), c8 = C(8);
+    const double a2 = a + a, b2 = b + b;
+    const double r0 = fma(a, fma(a, c2, c1), c0);
+    const double r1 = fma(a, fma(a, c5, c4), c3);
+    const double r2 = fma(a, fma(a, c8, c7), c6);
+    const double d0 = fma(a2, c2, c1);
+    const double d1 = fma(a2, c5, c4);
+    const double d2 = fma(a2, c8, c7);
+    p = fma(b, fma(b, r2, r1), r0);
+    pb = fma(b2, r2, r1);
+    pbb = r2 + r2;
+    pa = fma(b, fma(b, d2, d1), d0);
+    pab = fma(b2, d2, d1);
+    const double e = fma(b, fma(b, c8, c5), c2);
+    paa = e + e;
+}
+
+template <class CF>
+DCN_HD double value(CF C, double a, double b)
+{
+    const double r0 = fma(a, fma(a, C(2), C(1)), C(0));
+    const double r1 = fma(a, fma(a, C(5), C(4)), C(3));
+    const double r2 = fma(a, fma(a, C(8), C(7)), C(6));
+    return fma(b, fma(b, r2, r1), r0);
+}
+
+// LDL^T solve of H p = -g for the symmetric 4x4 H (upper triangle); false if a pivot is not above `floor`
+DCN_HD bool ldl4(double h00, double h01, double h02, double h03, double h11, double h12, double h13,
+                 double h22, double h23, double h33, const double *g, double floor, double *p)
+{
+    if (!(h00 > floor)) return false;
+    const double i0 = 1.0 / h00;
+    const double l10 = h01 * i0, l20 = h02 * i0, l30 = h03 * i0;
+    const double d1 = fma(-l10, h01, h11);
+    if (!(d1 > floor)) return false;
+    const double i1 = 1.0 / d1;
+    const double t21 = fma(-l20, h01, h12), t31 = fma(-l30, h01, h13);
+    const double l21 = t21 * i1, l31 = t31 * i1;
+    const double d2 = fma(-l21, t21, fma(-l20, h02, h22));
+    if (!(d2 > floor)) return false;
+    const double i2 = 1.0 / d2;
+    const double t32 = fma(-l31, t21, fma(-l30, h02, h23));
+    const double l32 = t32 * i2;
+    const double d3 = fma(-l32, t32, fma(-l31, t31, fma(-l30, h03, h33)));
+    if (!(d3 > floor)) return false;
+    const double i3 = 1.0 / d3;
+    const double y0 = -g[0];
+    const double y1 = fma(-l10, y0, -g[1]);
+    const double y2 = fma(-l21, y1, fma(-l20, y0, -g[2]));
+    const double y3 = fma(-l32, y2, fma(-l31, y1, fma(-l30, y0, -g[3])));
+    p[3] = y3 * i3;
+    p[2] = fma(-l32, p[3], y2 * i2);
+    p[1] = fma(-l31, p[3], fma(-l21, p[2], y1 * i1));
+    p[0] = fma(-l30, p[3], fma(-l20, p[2], fma(-l10, p[1], y0 * i0)));
+    return true;
+}
+
+// One lockstep iteration (tol_d2 = tol_d^2, tau_exit2 = tau_exit^2 or negative to disable).  Returns true when the solve is finished (R filled: the distance is attained
+// at the point just evaluated, hence an upper bound of the minimum whether or not it converged).
+template <class CF>
+DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, double tol_d2, double tau_exit2, NwResult &R)
+{
+    const double u = s.x[0], v = s.x[1], sq = s.x[2], tq = s.x[3];
+    double rr = 0.0, g[4] = { 0.0, 0.0, 0.0, 0.0 };
+    double h00 = 0.0, h01 = 0.0, h02 = 0.0, h03 = 0.0, h11 = 0.0, h12 = 0.0, h13 = 0.0, h22 = 0.0, h23 = 0.0, h33 = 0.0;
+    double r[3], Qs[3], Qt[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double p, pa, pb, paa, pab, pbb, q, qa, qb, qaa, qab, qbb;
+        jet([&](int m) { return cf(9 * c + m); }, u, v, p, pa, pb, paa, pab, pbb);
+        jet([&](int m) { return cf(27 + 9 * c + m); }, sq, tq, q, qa, qb, qaa, qab, qbb);
+        const double rc = p - q;
+        r[c] = rc; Qs[c] = qa; Qt[c] = qb;
+        rr = fma(rc, rc, rr);
+        g[0] = fma(rc, pa, g[0]); g[1] = fma(rc, pb, g[1]); g[2] = fma(-rc, qa, g[2]); g[3] = fma(-rc, qb, g[3]);
+        h00 = fma(pa, pa, fma(rc, paa, h00)); h01 = fma(pa, pb, fma(rc, pab, h01));
+        h02 = fma(-pa, qa, h02); h03 = fma(-pa, qb, h03);
+        h11 = fma(pb, pb, fma(rc, pbb, h11)); h12 = fma(-pb, qa, h12); h13 = fma(-pb, qb, h13);
+        h22 = fma(qa, qa, fma(-rc, qaa, h22)); h23 = fma(qa, qb, fma(-rc, qab, h23));
+        h33 = fma(qb, qb, fma(-rc, qbb, h33));
+    }
+    s.iters++;
+    // active set (L272-L278): a variable at a bound whose gradient pushes outward is held
+    bool fx[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) fx[i] = (s.x[i] <= lo[i] && g[i] > 0.0) || (s.x[i] >= hi[i] && g[i] < 0.0);
+    const double tr = (fx[0] ? 0.0 : fabs(h00)) + (fx[1] ? 0.0 : fabs(h11)) + (fx[2] ? 0.0 : fabs(h22)) + (fx[3] ? 0.0 : fabs(h33));
+    const double gg = (fx[0] ? 0.0 : g[0] * g[0]) + (fx[1] ? 0.0 : g[1] * g[1]) + (fx[2] ? 0.0 : g[2] * g[2]) + (fx[3] ? 0.0 : g[3] * g[3]);
+    double rr_out = rr;
+    bool finished = s.phase >= 2 || rr <= tau_exit2 || gg == 0.0 || !(tr > 0.0);
+    int converged = s.phase != 3;
+    if (!finished) {
+        const double one = tr;
+        if (fx[0]) { h01 = h02 = h03 = 0.0; h00 = one; g[0] = 0.0; }
+        if (fx[1]) { h01 = h12 = h13 = 0.0; h11 = one; g[1] = 0.0; }
+        if (fx[2]) { h02 = h12 = h23 = 0.0; h22 = one; g[2] = 0.0; }
+        if (fx[3]) { h03 = h13 = h23 = 0.0; h33 = one; g[3] = 0.0; }
+        // Levenberg damping: the Gauss-Newton part J^T J (J = [P_u P_v -Q_s -Q_t], 3x4) always has a null
+        // direction, so a small multiple of the trace is always added; larger ones only if a pivot fails
+        double p[4];
+        double lam = 1e-10 * tr;
+        bool ok = false;
+#pragma unroll 1
+        for (int tries = 0; tries < NW_LAM_TRIES && !ok; ++tries) {
+            ok = ldl4(h00 + lam, h01, h02, h03, h11 + lam, h12, h13, h22 + lam, h23, h33 + lam, g, 0.25 * lam, p);
+            lam *= NW_LAM_GROW;
+        }
+        if (!ok) {
+            const double sc = 1.0 / tr;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) p[i] = -g[i] * sc;
+        }
+        const double pred = -0.5 * (g[0] * p[0] + g[1] * p[1] + g[2] * p[2] + g[3] * p[3]);
+        // projected step, backtracking on f (value-only evaluations)
+        const double f0 = 0.5 * rr;
+        double xn[4], alpha = 1.0, fn2 = rr;
+        bool dec = false;
+#pragma unroll 1
+        for (int ls = 0; ls < 6 && !dec; ++ls) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) xn[i] = fmin(hi[i], fmax(lo[i], fma(alpha, p[i], s.x[i])));
+            double fn = 0.0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double d = value([&](int m) { return cf(9 * c + m); }, xn[0], xn[1])
+                               - value([&](int m) { return cf(27 + 9 * c + m); }, xn[2], xn[3]);
+                fn = fma(d, d, fn);
+            }
+            dec = 0.5 * fn <= f0; fn2 = fn;
+            alpha *= 0.25;
+        }
+        double step = 0.0;
+        if (dec) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { step = fmax(step, fabs(xn[i] - s.x[i]) / (hi[i] - lo[i])); s.x[i] = xn[i]; }
+        }
+        if (pred <= 0.0 || pred * pred <= tol_d2 * fmax(rr, tol_d2)) {
+            // predicted decrease of the DISTANCE below tolerance: converged.  The distance reported is the
+            // one attained at the accepted trial point (value-only evaluation), the sign cosine the one here.
+            finished = true;
+            if (dec) { rr_out = fn2; }
+        } else if (!dec || step < 1e-15) {
+            finished = true; converged = 0;              // stalled at the point just evaluated
+        } else if (s.iters >= NW_MAXIT - 1) {
+            s.phase = 3;                                  // one last evaluation at the new point
+        }
+    }
+    if (finished) {
+        const double nx = Qs[1] * Qt[2] - Qs[2] * Qt[1];
+        const double ny = Qs[2] * Qt[0] - Qs[0] * Qt[2];
+        const double nz = Qs[0] * Qt[1] - Qs[1] * Qt[0];
+        const double nn = nx * nx + ny * ny + nz * nz;
+        const double den = sqrt(rr * nn);
+        R.dist = sqrt(rr_out);
+        R.cosv = den > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) / den : 0.0;
+        R.converged = converged;
+    }
+    return finished;
+}
+
+} // namespace dcn
