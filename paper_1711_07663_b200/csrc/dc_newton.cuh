@@ -14,23 +14,27 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
+#include <string.h>
 
 namespace dcn {
+
+#ifdef __CUDA_ARCH__
+#define __longlong_as_double_hd(x) __longlong_as_double(x)
+#else
+static inline double __longlong_as_double_hd(long long x) { double d; memcpy(&d, &x, 8); return d; }
+#endif
 
 #ifndef DCN_HD
 #define DCN_HD __host__ __device__ __forceinline__
 #endif
 
-#ifndef NW_LAM_TRIES
-#define NW_LAM_TRIES 11
-#define NW_LAM_GROW 10.0
-#endif
-#define NW_MAXIT 16                 /* evaluations per solve before it is declared unconverged */
+#define NW_MAXIT 24                 /* evaluations per solve before it is declared unconverged */
 
 // state of one lane's solve
 struct NwState {
     double x[4];
     int iters;                      // evaluations done
+    int ls;                         // rejected trial steps at the current point (0: none yet)
     int phase;                      // 0 idle, 1 iterating, 3 last evaluation of an unconverged solve
 };
 
@@ -66,25 +70,29 @@ DCN_HD double value(CF C, double a, double b)
     return fma(b, fma(b, r2, r1), r0);
 }
 
-// LDL^T solve of H p = -g for the symmetric 4x4 H (upper triangle); false if a pivot is not above `floor`
-DCN_HD bool ldl4(double h00, double h01, double h02, double h03, double h11, double h12, double h13,
-                 double h22, double h23, double h33, const double *g, double floor, double *p)
+// Modified LDL^T solve of H p = -g for the symmetric 4x4 H (upper triangle): a pivot d that is not safely
+// positive is replaced by max(|d|, floor) (Gill-Murray style, one pass, no retries, no branches), which
+// turns a direction of negative or vanishing curvature into a descent direction of curvature scale.
+// Returns true if any pivot had to be modified (H was not positive definite).
+DCN_HD bool ldl4_mod(double h00, double h01, double h02, double h03, double h11, double h12, double h13,
+                     double h22, double h23, double h33, const double *g, double floor, double *p)
 {
-    if (!(h00 > floor)) return false;
-    const double i0 = 1.0 / h00;
+    bool mod = !(h00 > floor);
+    const double d0 = mod ? fmax(fabs(h00), floor) : h00;
+    const double i0 = 1.0 / d0;
     const double l10 = h01 * i0, l20 = h02 * i0, l30 = h03 * i0;
-    const double d1 = fma(-l10, h01, h11);
-    if (!(d1 > floor)) return false;
+    double d1 = fma(-l10, h01, h11);
+    if (!(d1 > floor)) { mod = true; d1 = fmax(fabs(d1), floor); }
     const double i1 = 1.0 / d1;
     const double t21 = fma(-l20, h01, h12), t31 = fma(-l30, h01, h13);
     const double l21 = t21 * i1, l31 = t31 * i1;
-    const double d2 = fma(-l21, t21, fma(-l20, h02, h22));
-    if (!(d2 > floor)) return false;
+    double d2 = fma(-l21, t21, fma(-l20, h02, h22));
+    if (!(d2 > floor)) { mod = true; d2 = fmax(fabs(d2), floor); }
     const double i2 = 1.0 / d2;
     const double t32 = fma(-l31, t21, fma(-l30, h02, h23));
     const double l32 = t32 * i2;
-    const double d3 = fma(-l32, t32, fma(-l31, t31, fma(-l30, h03, h33)));
-    if (!(d3 > floor)) return false;
+    double d3 = fma(-l32, t32, fma(-l31, t31, fma(-l30, h03, h33)));
+    if (!(d3 > floor)) { mod = true; d3 = fmax(fabs(d3), floor); }
     const double i3 = 1.0 / d3;
     const double y0 = -g[0];
     const double y1 = fma(-l10, y0, -g[1]);
@@ -94,7 +102,7 @@ DCN_HD bool ldl4(double h00, double h01, double h02, double h03, double h11, dou
     p[2] = fma(-l32, p[3], y2 * i2);
     p[1] = fma(-l31, p[3], fma(-l21, p[2], y1 * i1));
     p[0] = fma(-l30, p[3], fma(-l20, p[2], fma(-l10, p[1], y0 * i0)));
-    return true;
+    return mod;
 }
 
 // One lockstep iteration (tol_d2 = tol_d^2, tau_exit2 = tau_exit^2 or negative to disable).  Returns true when the solve is finished (R filled: the distance is attained
@@ -132,59 +140,121 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
     bool finished = s.phase >= 2 || rr <= tau_exit2 || gg == 0.0 || !(tr > 0.0);
     int converged = s.phase != 3;
     if (!finished) {
-        const double one = tr;
-        if (fx[0]) { h01 = h02 = h03 = 0.0; h00 = one; g[0] = 0.0; }
-        if (fx[1]) { h01 = h12 = h13 = 0.0; h11 = one; g[1] = 0.0; }
-        if (fx[2]) { h02 = h12 = h23 = 0.0; h22 = one; g[2] = 0.0; }
-        if (fx[3]) { h03 = h13 = h23 = 0.0; h33 = one; g[3] = 0.0; }
-        // Levenberg damping: the Gauss-Newton part J^T J (J = [P_u P_v -Q_s -Q_t], 3x4) always has a null
-        // direction, so a small multiple of the trace is always added; larger ones only if a pivot fails
-        double p[4];
-        double lam = 1e-10 * tr;
-        bool ok = false;
+        // Minimise the quadratic model g.p + 1/2 p.H.p over the box by a short active-set loop (no new
+        // evaluation of the patches): solve for the free variables; every free variable the step would carry
+        // across a bound is fixed AT that bound (its move dx becomes data of the next solve); repeat.
+        // The Gauss-Newton part J^T J (J = [P_u P_v -Q_s -Q_t], 3x4) of H always has a null direction, which the
+        // curvature terms r.P_uu ... make weakly positive or negative: the factorisation repairs its pivots.
+        double p[4], p0[4], dx[4] = { 0.0, 0.0, 0.0, 0.0 };
+        const double g0[4] = { fx[0] ? 0.0 : g[0], fx[1] ? 0.0 : g[1], fx[2] ? 0.0 : g[2], fx[3] ? 0.0 : g[3] };
+        bool indefinite = false;
 #pragma unroll 1
-        for (int tries = 0; tries < NW_LAM_TRIES && !ok; ++tries) {
-            ok = ldl4(h00 + lam, h01, h02, h03, h11 + lam, h12, h13, h22 + lam, h23, h33 + lam, g, 0.25 * lam, p);
-            lam *= NW_LAM_GROW;
-        }
-        if (!ok) {
-            const double sc = 1.0 / tr;
+        for (int pass = 0; pass < 3; ++pass) {
+            const double a00 = fx[0] ? tr : h00, a11 = fx[1] ? tr : h11, a22 = fx[2] ? tr : h22, a33 = fx[3] ? tr : h33;
+            const double a01 = (fx[0] || fx[1]) ? 0.0 : h01, a02 = (fx[0] || fx[2]) ? 0.0 : h02, a03 = (fx[0] || fx[3]) ? 0.0 : h03;
+            const double a12 = (fx[1] || fx[2]) ? 0.0 : h12, a13 = (fx[1] || fx[3]) ? 0.0 : h13, a23 = (fx[2] || fx[3]) ? 0.0 : h23;
+            double rhs[4];
+            rhs[0] = fx[0] ? 0.0 : fma(h03, dx[3], fma(h02, dx[2], fma(h01, dx[1], g[0])));
+            rhs[1] = fx[1] ? 0.0 : fma(h13, dx[3], fma(h12, dx[2], fma(h01, dx[0], g[1])));
+            rhs[2] = fx[2] ? 0.0 : fma(h23, dx[3], fma(h12, dx[1], fma(h02, dx[0], g[2])));
+            rhs[3] = fx[3] ? 0.0 : fma(h23, dx[2], fma(h13, dx[1], fma(h03, dx[0], g[3])));
+            const bool mod = ldl4_mod(a00, a01, a02, a03, a11, a12, a13, a22, a23, a33, rhs, 1e-10 * tr, p);
+            if (pass == 0) {
+                indefinite = mod;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) p[i] = -g[i] * sc;
-        }
-        const double pred = -0.5 * (g[0] * p[0] + g[1] * p[1] + g[2] * p[2] + g[3] * p[3]);
-        // projected step, backtracking on f (value-only evaluations)
-        const double f0 = 0.5 * rr;
-        double xn[4], alpha = 1.0, fn2 = rr;
-        bool dec = false;
-#pragma unroll 1
-        for (int ls = 0; ls < 6 && !dec; ++ls) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) xn[i] = fmin(hi[i], fmax(lo[i], fma(alpha, p[i], s.x[i])));
-            double fn = 0.0;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const double d = value([&](int m) { return cf(9 * c + m); }, xn[0], xn[1])
-                               - value([&](int m) { return cf(27 + 9 * c + m); }, xn[2], xn[3]);
-                fn = fma(d, d, fn);
+                for (int i = 0; i < 4; ++i) p0[i] = p[i];
             }
-            dec = 0.5 * fn <= f0; fn2 = fn;
-            alpha *= 0.25;
+            bool any = false;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (fx[i]) p[i] = dx[i];
+                else {
+                    const double t = s.x[i] + p[i];
+                    if (t > hi[i] || (t == hi[i] && p[i] > 0.0 && s.x[i] == hi[i])) { fx[i] = true; dx[i] = hi[i] - s.x[i]; p[i] = dx[i]; any = true; }
+                    else if (t < lo[i] || (t == lo[i] && p[i] < 0.0 && s.x[i] == lo[i])) { fx[i] = true; dx[i] = lo[i] - s.x[i]; p[i] = dx[i]; any = true; }
+                }
+            }
+            if (!any) break;
         }
+        // predicted decrease of f: -(g.p + 1/2 p.H.p); the model gradient g + H p at the end point must push
+        // every fixed variable outward (nothing is released inside the loop above).  Otherwise fall back on the
+        // plain projected step of the first solve, whose predicted decrease -1/2 g.p0 is never negative.
+        double pred = 0.0;
+        {
+            const double Hp[4] = { fma(h03, p[3], fma(h02, p[2], fma(h01, p[1], h00 * p[0]))),
+                                   fma(h13, p[3], fma(h12, p[2], fma(h11, p[1], h01 * p[0]))),
+                                   fma(h23, p[3], fma(h22, p[2], fma(h12, p[1], h02 * p[0]))),
+                                   fma(h33, p[3], fma(h23, p[2], fma(h13, p[1], h03 * p[0]))) };
+            bool valid = true;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                pred = fma(-p[i], fma(0.5, Hp[i], g[i]), pred);
+                if (fx[i]) {
+                    const double m = g[i] + Hp[i];
+                    valid = valid && (s.x[i] + p[i] >= hi[i] ? m <= 0.0 : m >= 0.0);
+                }
+            }
+            if (!valid || !(pred >= 0.0)) {
+                pred = 0.0;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) { p[i] = p0[i]; pred = fma(-0.5 * g0[i], p0[i], pred); }
+            }
+        }
+        // Step length of THIS call's single trial (s.ls counts the rejected trials at this point).  With an
+        // indefinite H the minimum along the valley sits on the box border: the first trial stretches the
+        // step until the first free variable reaches its bound.
+        double alpha = 1.0;
+        if (indefinite || s.ls > 0) {
+            // largest multiple of p that keeps every free variable inside its bounds
+            double ahit = INFINITY;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const double room = (p[i] > 0.0 ? hi[i] : lo[i]) - s.x[i];
+                if (p[i] != 0.0 && room != 0.0) ahit = fmin(ahit, room / p[i]);   // (a variable already on the bound it is pushed against just stays clamped)
+            }
+            const bool stretch = indefinite && ahit > 1.0 && ahit < INFINITY;
+            const double q = __longlong_as_double_hd((long long)(1023 - 2 * (s.ls > 0 ? s.ls - 1 : 0)) << 52);   // 4^-(ls-1)
+            if (s.ls == 0) alpha = stretch ? ahit : 1.0;
+            // a rejected trial is followed by UNCLAMPED ones: up to the first bound (a clamped step is not a
+            // descent step when the clamped variable is coupled to the others), then quarters of that
+            else alpha = stretch ? q : (ahit < 1.0 ? ahit * q : 0.25 * q);
+        }
+        // one projected trial point, value-only evaluation; a rejected trial is retried by the NEXT call with a
+        // shorter step (the other lanes of the warp never wait for a backtracking loop)
+        double xn[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            // (a trial point within rounding of a bound is snapped onto it: the step to the first bound lands
+            // an ulp short of it as often as not, and "on the bound" is tested exactly everywhere)
+            const double t = fma(alpha, p[i], s.x[i]), w = 1e-14 * (hi[i] - lo[i]);
+            xn[i] = t >= hi[i] - w ? hi[i] : (t <= lo[i] + w ? lo[i] : t);
+        }
+        double fn = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double d = value([&](int m) { return cf(9 * c + m); }, xn[0], xn[1])
+                           - value([&](int m) { return cf(27 + 9 * c + m); }, xn[2], xn[3]);
+            fn = fma(d, d, fn);
+        }
+        const bool dec = fn <= rr;
+#ifdef NW_TRACE
+        printf("   indef %d alpha %.3e p=(%.3e %.3e %.3e %.3e) g=(%.3e %.3e %.3e %.3e) fx=%d%d%d%d pred %.3e rr %.17e fn %.17e\n",(int)indefinite,alpha,p[0],p[1],p[2],p[3],g[0],g[1],g[2],g[3],fx[0],fx[1],fx[2],fx[3],pred,rr,fn);
+#endif
         double step = 0.0;
         if (dec) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) { step = fmax(step, fabs(xn[i] - s.x[i]) / (hi[i] - lo[i])); s.x[i] = xn[i]; }
-        }
-        if (pred <= 0.0 || pred * pred <= tol_d2 * fmax(rr, tol_d2)) {
+            s.ls = 0;
+        } else s.ls++;
+        if (pred * pred <= tol_d2 * fmax(rr, tol_d2)) {
             // predicted decrease of the DISTANCE below tolerance: converged.  The distance reported is the
             // one attained at the accepted trial point (value-only evaluation), the sign cosine the one here.
             finished = true;
-            if (dec) { rr_out = fn2; }
-        } else if (!dec || step < 1e-15) {
+            if (dec) rr_out = fn;
+        } else if ((dec && step < 1e-15) || s.ls > 7) {
             finished = true; converged = 0;              // stalled at the point just evaluated
         } else if (s.iters >= NW_MAXIT - 1) {
-            s.phase = 3;                                  // one last evaluation at the new point
+            s.phase = 3;                                  // one last evaluation
         }
     }
     if (finished) {
