@@ -2,7 +2,7 @@
 //
 // Step names follow SURVEY.md 8(a) / DESIGN.md:
 //   S1 face prep      k_face_boxes, k_setup_surface
-//   S3 face bins      k_face_hist, k_cell_scan, k_face_scatter        (Morton-ordered uniform bins)
+//   S3 face bins      k_face_hist, k_scan_sums, k_scan_cells, k_face_scatter        (Morton-ordered uniform bins)
 //   S2 element boxes  k_elem_boxes                                    (HBM-bound stream)
 //   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
 //   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound (wavefront of uniform kernels, FP64)
@@ -184,25 +184,51 @@ __global__ void k_face_hist(const DcScalars *S, const double *__restrict__ fbox_
     atomicAdd(&cell_count[code], 1);
 }
 
-// exclusive scan over DC_NCELL cells by one CTA of 1024 threads (256 cells per thread)
-__global__ void __launch_bounds__(1024) k_cell_scan(const int *__restrict__ cell_count, int *__restrict__ cell_start)
+// exclusive scan over the DC_NCELL Morton-ordered cells in two coalesced passes: per-chunk sums (one CTA of
+// 256 threads per 1024 cells, int4 loads), then every CTA adds the sums of the chunks before it to a local scan.
+#define SCAN_CHUNK 1024
+#define SCAN_NCHUNK (DC_NCELL / SCAN_CHUNK)
+__device__ __forceinline__ int block_sum_256(int v, int *s_warp)
 {
-    __shared__ int s_part[1024];
-    const int per = DC_NCELL / 1024;
-    const int t = threadIdx.x;
-    int sum = 0;
-    for (int i = 0; i < per; ++i) sum += cell_count[t * per + i];
-    s_part[t] = sum;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = v;
     __syncthreads();
-    for (int o = 1; o < 1024; o <<= 1) {
-        int v = t >= o ? s_part[t - o] : 0;
-        __syncthreads();
-        s_part[t] += v;
-        __syncthreads();
-    }
-    int run = s_part[t] - sum;
-    for (int i = 0; i < per; ++i) { cell_start[t * per + i] = run; run += cell_count[t * per + i]; }
-    if (t == 1023) cell_start[DC_NCELL] = run;
+    int t = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) t += s_warp[w];
+    __syncthreads();
+    return t;
+}
+__global__ void __launch_bounds__(256) k_scan_sums(const int *__restrict__ cell_count, int *__restrict__ chunk_sum)
+{
+    __shared__ int s_warp[8];
+    const int4 v = reinterpret_cast<const int4 *>(cell_count)[blockIdx.x * 256 + threadIdx.x];
+    const int t = block_sum_256(v.x + v.y + v.z + v.w, s_warp);
+    if (threadIdx.x == 0) chunk_sum[blockIdx.x] = t;
+}
+__global__ void __launch_bounds__(256) k_scan_cells(const int *__restrict__ cell_count, const int *__restrict__ chunk_sum,
+                                                    int *__restrict__ cell_start)
+{
+    __shared__ int s_warp[8];
+    __shared__ int s_incl[8];
+    // sum of the chunks before this one (SCAN_NCHUNK = 256 values: one per thread)
+    const int before = block_sum_256((int)threadIdx.x < (int)blockIdx.x ? chunk_sum[threadIdx.x] : 0, s_warp);
+    const int4 v = reinterpret_cast<const int4 *>(cell_count)[blockIdx.x * 256 + threadIdx.x];
+    const int mine = v.x + v.y + v.z + v.w;
+    int incl = mine;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += u; }
+    if (lane == 31) s_incl[wid] = incl;
+    __syncthreads();
+    int woff = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) if (w < wid) woff += s_incl[w];
+    int4 o;
+    o.x = before + woff + incl - mine; o.y = o.x + v.x; o.z = o.y + v.y; o.w = o.z + v.z;
+    reinterpret_cast<int4 *>(cell_start)[blockIdx.x * 256 + threadIdx.x] = o;
+    if (blockIdx.x == SCAN_NCHUNK - 1 && threadIdx.x == 255) cell_start[DC_NCELL] = o.w + v.w;
 }
 
 // scatter faces into cell order; write sorted boxes and monomial coefficients (stride 28 doubles)
@@ -330,11 +356,18 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
 
 // ------------------------------------------------------------------------------------------
 // S4a: one thread per element.  Initialises the per-element state of this cut and appends the
-// elements whose inflated box overlaps a non-empty face cell to the active list
-// (warp-aggregated atomic append).
+// elements whose inflated box overlaps a non-empty 4x4x4 block of face cells to the active list
+// (warp-aggregated atomic append).  A block of 64 cells is one contiguous range of the Morton order.
+__device__ __forceinline__ int block_faces(const int *__restrict__ cell_start, int bx, int by, int bz, int &first)
+{
+    const unsigned c0 = morton3(bx, by, bz) << 6;
+    first = __ldg(cell_start + c0);
+    return __ldg(cell_start + c0 + 64) - first;
+}
+
 __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
                          signed char *__restrict__ labels, int *__restrict__ parent,
-                         unsigned char *__restrict__ comp, const int *__restrict__ cell_count,
+                         unsigned char *__restrict__ comp, const int *__restrict__ cell_start,
                          int *__restrict__ act_elem)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -353,13 +386,15 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
         const double reach = S->reach;
         if (d2 <= reach * reach) {
             const double pad = reach + S->fhalf;
-            int i0[3], i1[3];
+            int b0[3], b1[3];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c); }
-            for (int z = i0[2]; z <= i1[2] && !active; ++z)
-                for (int y = i0[1]; y <= i1[1] && !active; ++y)
-                    for (int x = i0[0]; x <= i1[0]; ++x)
-                        if (__ldg(cell_count + morton3(x, y, z)) > 0) { active = true; break; }
+            for (int c = 0; c < 3; ++c) { b0[c] = cell_coord(S, lo[c] - pad, c) >> 2; b1[c] = cell_coord(S, hi[c] + pad, c) >> 2; }
+            for (int z = b0[2]; z <= b1[2] && !active; ++z)
+                for (int y = b0[1]; y <= b1[1] && !active; ++y)
+                    for (int x = b0[0]; x <= b1[0]; ++x) {
+                        int first;
+                        if (block_faces(cell_start, x, y, z, first) > 0) { active = true; break; }
+                    }
         }
     }
     const unsigned m = __ballot_sync(0xffffffffu, active);
@@ -372,9 +407,13 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
     }
 }
 
-// S4b: one warp per active element: box test (Algorithm A.2) against the
-// faces of the cells its inflated box overlaps; count, reserve a contiguous segment with one
-// atomic per element, then write.  pair_key is initialised to +inf for S5.
+// S4b: one warp per active element.  The 4x4x4 cell blocks its inflated box overlaps (at most 27 for an
+// element smaller than a block) are one contiguous face range each in the Morton order: one lane per block
+// fetches its range, the ranges are concatenated by a warp scan, and the lanes then walk the concatenation
+// 32 faces at a time (coalesced face-box loads, every lane busy) applying the box test of Algorithm A.2
+// (PAPER.md L689-L709).  Survivors are staged in shared memory and written as ONE contiguous segment of
+// the pair list (one atomic per element); an element with more survivors than the stage holds re-walks its
+// ranges and writes directly.  pair_key is initialised to +inf for S5.
 __device__ __forceinline__ bool box_within(const double *lo, const double *hi, const double *fb, double reach2)
 {
     double d2 = 0.0;
@@ -386,73 +425,100 @@ __device__ __forceinline__ bool box_within(const double *lo, const double *hi, c
     return d2 <= reach2;
 }
 
-__global__ void __launch_bounds__(256) k_pairs(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
+#define PR_WARPS 8
+#define PR_CAP 224
+__global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
                                                const int *__restrict__ act_elem, const int *__restrict__ cell_start,
                                                const double *__restrict__ fbox, long long max_pairs,
                                                int *__restrict__ band_elem, long long *__restrict__ band_start,
                                                int *__restrict__ band_cnt,
                                                int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key)
 {
-    const int lane = threadIdx.x & 31;
+    __shared__ int s_list[PR_WARPS][PR_CAP];
+    __shared__ int s_off[PR_WARPS][33];
+    __shared__ int s_first[PR_WARPS][32];
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * blockDim.x) >> 5;
     const int n_active = S->n_active;
     const double reach = S->reach, reach2 = reach * reach, pad = reach + S->fhalf;
+    int *list = s_list[wl], *off = s_off[wl], *firsts = s_first[wl];
     unsigned long long tests = 0;
     for (int a = warp; a < n_active; a += nwarps) {
         const long long e = act_elem[a];
         double lo[3], hi[3];
-        int i0[3], i1[3];
+        int b0[3], nb[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e];
-            i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c);
+            b0[c] = cell_coord(S, lo[c] - pad, c) >> 2;
+            nb[c] = (cell_coord(S, hi[c] + pad, c) >> 2) - b0[c] + 1;
         }
-        const int nx = i1[0] - i0[0] + 1, ny = i1[1] - i0[1] + 1, nz = i1[2] - i0[2] + 1;
-        const int ncell = nx * ny * nz;
+        const int nblk = nb[0] * nb[1] * nb[2];
         long long base = 0;
-        int my_off = 0;
-        for (int pass = 0; pass < 2; ++pass) {
-            int cnt = 0;
-            for (int ci = lane; ci < ncell; ci += 32) {
-                const int x = i0[0] + ci % nx, y = i0[1] + (ci / nx) % ny, z = i0[2] + ci / (nx * ny);
-                const unsigned code = morton3(x, y, z);
-                const int s = __ldg(cell_start + code), t = __ldg(cell_start + code + 1);
-                for (int p = s; p < t; ++p) {
-                    double fb[6];
-#pragma unroll
-                    for (int m = 0; m < 6; ++m) fb[m] = __ldg(fbox + (size_t)p * 6 + m);
-                    if (pass == 0) ++tests;
-                    if (box_within(lo, hi, fb, reach2)) {
-                        if (pass == 1) {
-                            pair_face[base + my_off + cnt] = p;
-                            pair_key[base + my_off + cnt] = 0x7ff0000000000000ull;
-                        }
-                        ++cnt;
-                    }
-                }
-            }
-            if (pass == 0) {
-                // warp exclusive scan of cnt
+        int total = 0;
+        for (int phase = 0; phase < 2; ++phase) {
+            int running = 0;
+            for (int bbase = 0; bbase < nblk; bbase += 32) {
+                const int bi = bbase + lane;
+                int cnt = 0, first = 0;
+                if (bi < nblk) cnt = block_faces(cell_start, b0[0] + bi % nb[0], b0[1] + (bi / nb[0]) % nb[1], b0[2] + bi / (nb[0] * nb[1]), first);
                 int incl = cnt;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-                const int total = __shfl_sync(0xffffffffu, incl, 31);
-                my_off = incl - cnt;
-                if (lane == 0) {
-                    long long b = (long long)atomicAdd(&S->n_pairs, (unsigned long long)total);
-                    if (b + total > max_pairs) { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
-                    if (b >= 0 && total > 0) {
-                        const int slot = atomicAdd(&S->n_band, 1);
-                        if (slot < S->max_band) { band_elem[slot] = (int)e; band_start[slot] = b; band_cnt[slot] = total; }
-                        else atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW);
+                const int T = __shfl_sync(0xffffffffu, incl, 31);
+                if (lane == 0) off[0] = 0;
+                off[lane + 1] = incl; firsts[lane] = first;
+                __syncwarp();
+                for (int j0 = 0; j0 < T; j0 += 32) {
+                    const int j = j0 + lane;
+                    bool hit = false;
+                    int p = -1;
+                    if (j < T) {
+                        int L = 0;                       // largest L with off[L] <= j
+#pragma unroll
+                        for (int st = 16; st > 0; st >>= 1) if (off[L + st] <= j) L += st;
+                        p = firsts[L] + (j - off[L]);
+                        double fb[6];
+#pragma unroll
+                        for (int m = 0; m < 6; m += 2) {
+                            const double2 v = __ldg(reinterpret_cast<const double2 *>(fbox + (size_t)p * 6 + m));
+                            fb[m] = v.x; fb[m + 1] = v.y;
+                        }
+                        hit = box_within(lo, hi, fb, reach2);
+                        if (phase == 0) ++tests;
                     }
-                    base = b;
+                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    const int pos = running + __popc(m & lt_mask);
+                    if (hit) {
+                        if (phase == 0) { if (pos < PR_CAP) list[pos] = p; }
+                        else { pair_face[base + pos] = p; pair_key[base + pos] = 0x7ff0000000000000ull; }
+                    }
+                    running += __popc(m);
                 }
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (base < 0 || total == 0) break;
+                __syncwarp();
+            }
+            if (phase == 1) break;
+            total = running;
+            if (lane == 0) {
+                long long b = (long long)atomicAdd(&S->n_pairs, (unsigned long long)total);
+                if (b + total > max_pairs) { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
+                if (b >= 0 && total > 0) {
+                    const int slot = atomicAdd(&S->n_band, 1);
+                    if (slot < S->max_band) { band_elem[slot] = (int)e; band_start[slot] = b; band_cnt[slot] = total; }
+                    else atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW);
+                }
+                base = b;
+            }
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (base < 0 || total == 0) break;
+            if (total <= PR_CAP) {
+                for (int i = lane; i < total; i += 32) { pair_face[base + i] = list[i]; pair_key[base + i] = 0x7ff0000000000000ull; }
+                break;
             }
         }
+        __syncwarp();
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(0xffffffffu, tests, o);
@@ -796,7 +862,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_fperm = take((size_t)max_faces * 4);
     L.off_cell_count = take((size_t)(DC_NCELL + 1) * 4);
     L.off_cell_start = take((size_t)(DC_NCELL + 1) * 4);
-    L.off_cell_fill = take((size_t)(DC_NCELL + 1) * 4);
+    L.off_cell_fill = take((size_t)(DC_NCELL + 8 + SCAN_NCHUNK) * 4);   // + the scan's chunk sums
     L.off_hfaces = take((size_t)max_faces * 27 * 8);
     L.off_hlabels = take((size_t)n_elem);
     L.off_hsdist = take((size_t)n_elem * 8);
@@ -915,12 +981,13 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
     CK(cudaMemsetAsync(c->cell_count, 0, (size_t)(DC_NCELL + 1) * 4, st));
     CK(cudaMemsetAsync(c->cell_fill, 0, (size_t)(DC_NCELL + 1) * 4, st));
     k_face_hist<<<nblk(nf, 128), 128, 0, st>>>(c->S, c->fbox_orig, nf, c->fcell, c->cell_count);
-    k_cell_scan<<<1, 1024, 0, st>>>(c->cell_count, c->cell_start);
+    k_scan_sums<<<SCAN_NCHUNK, 256, 0, st>>>(c->cell_count, c->cell_fill + DC_NCELL + 8);
+    k_scan_cells<<<SCAN_NCHUNK, 256, 0, st>>>(c->cell_count, c->cell_fill + DC_NCELL + 8, c->cell_start);
     k_face_scatter<<<nblk(nf, 128), 128, 0, st>>>(face_nodes_dev, c->fbox_orig, c->fcell, c->cell_start, c->cell_fill,
                                                    nf, c->fperm, c->fbox, c->fcoef);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[9], st));
-    c->launches_surface = 6;
+    c->launches_surface = 7;
     c->have_surface = true;
     return DC_OK;
 }
@@ -939,7 +1006,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     if (P.flags & DC_FLAG_RECOMPUTE_BOXES) { int rc = run_elem_boxes(c, st); if (rc) return rc; }
     CK(cudaEventRecord(c->ev[1], st));
     k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
-    k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_count, c->act_elem);
+    k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->act_elem);
     k_pairs<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
                                            c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key);
     CK(cudaEventRecord(c->ev[2], st));
