@@ -7,7 +7,7 @@
 //   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
 //   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound (wavefront of uniform kernels, FP64)
 //   S6 decide         k_np_decide
-//   S7 flood fill     k_uf_union, k_uf_seed, k_uf_collect, k_seedless, k_uf_assign
+//   S7 flood fill     k_uf_local, k_uf_union, k_uf_seed, k_uf_collect, k_seedless, k_uf_assign
 //
 // PAPER.md citations are given where an operation is defined; the kernel design itself is new
 // (the paper's A.1-A.4 kernels were written for Kepler K80 and are prior art, not the blueprint).
@@ -373,7 +373,7 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     bool active = false;
     if (e < n_elem) {
-        labels[e] = -1; parent[e] = (int)e; comp[e] = 0;
+        labels[e] = -1; comp[e] = 0;       // (parent[] is initialised by k_uf_local)
         double lo[3], hi[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) { lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e]; }
@@ -598,14 +598,46 @@ __device__ __forceinline__ void uf_union(int *parent, int a, int b)
     }
 }
 
+// Pass 1: components INSIDE a tile of UF_TILE consecutive elements, in shared memory (neighbours mostly have
+// nearby ids, so most edges are settled here without touching global memory); every element then points at
+// its tile-local root.  Pass 2 (k_uf_union): only the edges that leave the tile go through the global forest.
+#define UF_TILE 1024
+__global__ void __launch_bounds__(UF_TILE) k_uf_local(const signed char *__restrict__ labels, const int *__restrict__ adj,
+                                                      long long n_elem, int *__restrict__ parent)
+{
+    __shared__ int sp[UF_TILE];
+    const int tid = threadIdx.x;
+    const long long base = (long long)blockIdx.x * UF_TILE, e = base + tid;
+    sp[tid] = tid;
+    __syncthreads();
+    if (e < n_elem && labels[e] != DC_CUT) {
+        int nbs[6];
+        const int2 *ap = reinterpret_cast<const int2 *>(adj + e * 6);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { const int2 v = __ldg(ap + k); nbs[2 * k] = v.x; nbs[2 * k + 1] = v.y; }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const int nb = nbs[k];
+            if (nb >= base && nb < e && labels[nb] != DC_CUT) uf_union(sp, tid, nb - (int)base);
+        }
+    }
+    __syncthreads();
+    if (e < n_elem) parent[e] = (int)base + uf_find(sp, tid);
+}
+
 __global__ void k_uf_union(const signed char *__restrict__ labels, const int *__restrict__ adj, long long n_elem, int *parent)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n_elem || labels[e] == DC_CUT) return;
+    const long long base = e & ~(long long)(UF_TILE - 1);
+    int nbs[6];
+    const int2 *ap = reinterpret_cast<const int2 *>(adj + e * 6);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { const int2 v = __ldg(ap + k); nbs[2 * k] = v.x; nbs[2 * k + 1] = v.y; }
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-        const int nb = __ldg(adj + e * 6 + k);
-        if (nb >= 0 && nb < e && labels[nb] != DC_CUT) uf_union(parent, (int)e, nb);
+        const int nb = nbs[k];
+        if (nb >= 0 && nb < base && labels[nb] != DC_CUT) uf_union(parent, (int)e, nb);
     }
 }
 
@@ -1032,6 +1064,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
+    k_uf_local<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(labels_dev, c->adj, ne, c->parent);
     k_uf_union<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, c->adj, ne, c->parent);
     k_uf_seed<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, ne, c->parent, c->comp);
     k_uf_collect<<<nblk(ne, 256), 256, 0, st>>>(c->S, labels_dev, ne, c->parent, c->comp);
@@ -1039,7 +1072,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
-    c->launches_classify = 12 + 2 * rounds + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
+    c->launches_classify = 13 + 2 * rounds + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }

@@ -5,8 +5,8 @@
 // The solve is the two-patch generalisation of PAPER.md Eq. 3-5 (L256-L270): minimise
 //   f(x) = 1/2 |P(u,v) - Q(s,t)|^2,   x = (u,v,s,t) in the box [lo,hi]   (a leaf of the branch and bound),
 // with the paper's clamp to the reference box (L272-L278) as a projected step: variables at a bound whose
-// gradient pushes outward are held, the rest take a Levenberg-damped Newton step, the trial point is
-// clamped and accepted only if f does not increase.
+// gradient pushes outward are held, the rest take a Newton step (LDL^T with repaired pivots), the trial
+// point is clamped and accepted only if f does not increase.
 //
 // Both patches are evaluated straight from their ROOT monomial coefficients (no re-centring): the box
 // bounds are dyadic and exactly representable, so clamped variables sit exactly on sub-patch borders.
@@ -140,66 +140,14 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
     bool finished = s.phase >= 2 || rr <= tau_exit2 || gg == 0.0 || !(tr > 0.0);
     int converged = s.phase != 3;
     if (!finished) {
-        // Minimise the quadratic model g.p + 1/2 p.H.p over the box by a short active-set loop (no new
-        // evaluation of the patches): solve for the free variables; every free variable the step would carry
-        // across a bound is fixed AT that bound (its move dx becomes data of the next solve); repeat.
-        // The Gauss-Newton part J^T J (J = [P_u P_v -Q_s -Q_t], 3x4) of H always has a null direction, which the
-        // curvature terms r.P_uu ... make weakly positive or negative: the factorisation repairs its pivots.
-        double p[4], p0[4], dx[4] = { 0.0, 0.0, 0.0, 0.0 };
-        const double g0[4] = { fx[0] ? 0.0 : g[0], fx[1] ? 0.0 : g[1], fx[2] ? 0.0 : g[2], fx[3] ? 0.0 : g[3] };
-        bool indefinite = false;
-#pragma unroll 1
-        for (int pass = 0; pass < 3; ++pass) {
-            const double a00 = fx[0] ? tr : h00, a11 = fx[1] ? tr : h11, a22 = fx[2] ? tr : h22, a33 = fx[3] ? tr : h33;
-            const double a01 = (fx[0] || fx[1]) ? 0.0 : h01, a02 = (fx[0] || fx[2]) ? 0.0 : h02, a03 = (fx[0] || fx[3]) ? 0.0 : h03;
-            const double a12 = (fx[1] || fx[2]) ? 0.0 : h12, a13 = (fx[1] || fx[3]) ? 0.0 : h13, a23 = (fx[2] || fx[3]) ? 0.0 : h23;
-            double rhs[4];
-            rhs[0] = fx[0] ? 0.0 : fma(h03, dx[3], fma(h02, dx[2], fma(h01, dx[1], g[0])));
-            rhs[1] = fx[1] ? 0.0 : fma(h13, dx[3], fma(h12, dx[2], fma(h01, dx[0], g[1])));
-            rhs[2] = fx[2] ? 0.0 : fma(h23, dx[3], fma(h12, dx[1], fma(h02, dx[0], g[2])));
-            rhs[3] = fx[3] ? 0.0 : fma(h23, dx[2], fma(h13, dx[1], fma(h03, dx[0], g[3])));
-            const bool mod = ldl4_mod(a00, a01, a02, a03, a11, a12, a13, a22, a23, a33, rhs, 1e-10 * tr, p);
-            if (pass == 0) {
-                indefinite = mod;
-#pragma unroll
-                for (int i = 0; i < 4; ++i) p0[i] = p[i];
-            }
-            bool any = false;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                if (fx[i]) p[i] = dx[i];
-                else {
-                    const double t = s.x[i] + p[i];
-                    if (t > hi[i] || (t == hi[i] && p[i] > 0.0 && s.x[i] == hi[i])) { fx[i] = true; dx[i] = hi[i] - s.x[i]; p[i] = dx[i]; any = true; }
-                    else if (t < lo[i] || (t == lo[i] && p[i] < 0.0 && s.x[i] == lo[i])) { fx[i] = true; dx[i] = lo[i] - s.x[i]; p[i] = dx[i]; any = true; }
-                }
-            }
-            if (!any) break;
-        }
-        // predicted decrease of f: -(g.p + 1/2 p.H.p); the model gradient g + H p at the end point must push
-        // every fixed variable outward (nothing is released inside the loop above).  Otherwise fall back on the
-        // plain projected step of the first solve, whose predicted decrease -1/2 g.p0 is never negative.
-        double pred = 0.0;
-        {
-            const double Hp[4] = { fma(h03, p[3], fma(h02, p[2], fma(h01, p[1], h00 * p[0]))),
-                                   fma(h13, p[3], fma(h12, p[2], fma(h11, p[1], h01 * p[0]))),
-                                   fma(h23, p[3], fma(h22, p[2], fma(h12, p[1], h02 * p[0]))),
-                                   fma(h33, p[3], fma(h23, p[2], fma(h13, p[1], h03 * p[0]))) };
-            bool valid = true;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                pred = fma(-p[i], fma(0.5, Hp[i], g[i]), pred);
-                if (fx[i]) {
-                    const double m = g[i] + Hp[i];
-                    valid = valid && (s.x[i] + p[i] >= hi[i] ? m <= 0.0 : m >= 0.0);
-                }
-            }
-            if (!valid || !(pred >= 0.0)) {
-                pred = 0.0;
-#pragma unroll
-                for (int i = 0; i < 4; ++i) { p[i] = p0[i]; pred = fma(-0.5 * g0[i], p0[i], pred); }
-            }
-        }
+        // plain projected Newton: the held variables are decoupled, the rest take the (pivot-repaired) Newton step
+        if (fx[0]) { h01 = h02 = h03 = 0.0; h00 = tr; g[0] = 0.0; }
+        if (fx[1]) { h01 = h12 = h13 = 0.0; h11 = tr; g[1] = 0.0; }
+        if (fx[2]) { h02 = h12 = h23 = 0.0; h22 = tr; g[2] = 0.0; }
+        if (fx[3]) { h03 = h13 = h23 = 0.0; h33 = tr; g[3] = 0.0; }
+        double p[4];
+        const bool indefinite = ldl4_mod(h00, h01, h02, h03, h11, h12, h13, h22, h23, h33, g, 1e-10 * tr, p);
+        const double pred = -0.5 * (g[0] * p[0] + g[1] * p[1] + g[2] * p[2] + g[3] * p[3]);
         // Step length of THIS call's single trial (s.ls counts the rejected trials at this point).  With an
         // indefinite H the minimum along the valley sits on the box border: the first trial stretches the
         // step until the first free variable reaches its bound.
