@@ -1229,12 +1229,3 @@ extern "C" double dc_measure_fp64_tflops(int device, int iters)
 
 extern "C" int dc_version(void) { return 1; }
 
-#ifdef DC_DEBUG_DUMP
-extern "C" int dc_debug_dump_set(double *ptr, int cap)
-{
-    int z = 0;
-    cudaMemcpyToSymbol(g_dump, &ptr, sizeof ptr); cudaMemcpyToSymbol(g_dump_cap, &cap, sizeof cap); cudaMemcpyToSymbol(g_dump_n, &z, sizeof z);
-    return 0;
-}
-extern "C" int dc_debug_dump_count(void) { int n = 0; cudaMemcpyFromSymbol(&n, g_dump_n, sizeof n); return n; }
-#endif

@@ -194,9 +194,6 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 // kernel at <= 128 registers and 16 warps per SM; a refill is a warp-cooperative coalesced copy of the
 // 2 x 216 B of the new item (the odd stride makes the transposed store 2-way conflicted instead of 32).
 #define NW_THREADS 128
-#ifdef DC_DEBUG_DUMP
-__device__ double *g_dump; __device__ int g_dump_n, g_dump_cap;
-#endif
 #define NW_STRIDE 129
 #define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
 #define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
@@ -296,12 +293,6 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 atomicMin(pair_key + it.p, key);
                 if (!R.converged && !((it.w3 >> 24) & 1)) {
                     cnt.fail++;
-#ifdef DC_DEBUG_DUMP
-                    { const int di = atomicAdd(&g_dump_n, 1);
-                      if (di < g_dump_cap) { double *o = g_dump + (size_t)di * 64; for (int m = 0; m < 54; ++m) o[m] = cf(m);
-                        double uc, vc, hP, sc, tc, hQ; nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                        o[54] = uc; o[55] = vc; o[56] = hP; o[57] = sc; o[58] = tc; o[59] = hQ; o[60] = R.dist; o[61] = s.iters; o[62] = u2d(best[b]); } }
-#endif
                     resplit = choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP);
                 }
             }

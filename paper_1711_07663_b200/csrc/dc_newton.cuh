@@ -185,9 +185,6 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
             fn = fma(d, d, fn);
         }
         const bool dec = fn <= rr;
-#ifdef NW_TRACE
-        printf("   indef %d alpha %.3e p=(%.3e %.3e %.3e %.3e) g=(%.3e %.3e %.3e %.3e) fx=%d%d%d%d pred %.3e rr %.17e fn %.17e\n",(int)indefinite,alpha,p[0],p[1],p[2],p[3],g[0],g[1],g[2],g[3],fx[0],fx[1],fx[2],fx[3],pred,rr,fn);
-#endif
         double step = 0.0;
         if (dec) {
 #pragma unroll
