@@ -28,6 +28,7 @@ using namespace dcg;
 #define DC_GRID_MAX 64              /* face-bin cells per axis (Morton code: 6 bits per axis) */
 #define DC_NCELL (DC_GRID_MAX * DC_GRID_MAX * DC_GRID_MAX)
 #define DC_NQN 28                   /* >= DC_MAX_ROUNDS + 2 */
+#define DC_GRID_ROUNDS 8             /* branch-and-bound rounds launched as grids; the rest run inside one CTA */
 
 // ------------------------------------------------------------------------------------------
 // device-resident scalars and counters
@@ -1049,18 +1050,24 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
                                            c->ecoef, c->pbox, c->best, c->dmin, c->nq);
     // seed solves: one per band element, queue = nq[0 .. n_band); failures are never re-split
     const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
-                                            c->q[0], &S->qn[0], c->qcap);
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, c->pair_face, c->fcoef, c->ecoef,
+                                                       c->best, c->dmin, c->pair_key);
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
                                            c->q[0], &S->qn[0], c->qcap);
+    // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
+    // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
     const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     const int rounds = 2 * max_level + 1;
-    for (int r = 0; r < rounds; ++r) {
+    const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
+    for (int r = 0; r < grid_rounds; ++r)
         k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, &S->nn[r], c->qcap);
-        k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[r], c->qcap, &S->nh[r + 1], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best, c->dmin, c->pair_key,
-                                                c->q[(r + 1) & 1], &S->qn[r + 1], c->qcap);
-    }
+                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, &S->nn[0], c->qcap);
+    if (rounds > grid_rounds)
+        k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                       c->nq, &S->nn[0], c->qcap);
+    // all leaves in one launch; an unconverged leaf is quartered and finished by the lane that held it
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->pair_face, c->fcoef, c->ecoef,
+                                                       c->best, c->dmin, c->pair_key);
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
@@ -1072,7 +1079,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
-    c->launches_classify = 13 + 2 * rounds + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
+    c->launches_classify = 14 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }

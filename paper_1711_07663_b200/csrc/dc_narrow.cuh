@@ -196,14 +196,14 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_THREADS 128
 #define NW_STRIDE 129
 #define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
+#define NW_STACK 12                 /* sub-leaves a lane may hold (3 levels of quartering) */
 #define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
 
 __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
                                                             const NItem *__restrict__ nq,
                                                             const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                             const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                            unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
-                                                            NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
+                                                            unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key)
 {
     extern __shared__ double nw_sm[];
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
@@ -223,7 +223,17 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
     for (int i = 0; i < 4; ++i) s.x[i] = 0.0;
     NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
     bool exhausted = false;
+    NItem stk[NW_STACK];            // sub-leaves of an unconverged solve, solved by the same lane (local memory, rarely touched)
+    int sp = 0;
     while (true) {
+        // ---- a lane with sub-leaves of its own goes on with those (same pair: its coefficients are already in place)
+        if (s.phase == 0 && sp > 0) {
+            it = stk[--sp];
+            double uc, vc, hP, sc, tc, hQ;
+            nitem_box(it, uc, vc, hP, sc, tc, hQ);
+            s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
+            s.iters = 0; s.ls = 0; s.phase = 1;
+        }
         // ---- refill idle lanes
         for (int pass = 0; pass < 4; ++pass) {
             const bool need = s.phase == 0 && !exhausted;
@@ -281,7 +291,6 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
             fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R);
         }
         // ---- results of the solves that finished (an attained distance is an upper bound whether converged or not)
-        bool resplit = false, splitP = false;
         if (fin) {
             const unsigned b = it.ak & 0x1fffffffu;
             cnt.newton++; cnt.iters += s.iters;
@@ -292,15 +301,16 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 const unsigned long long key = (d2u(R.dist) & ~0xffull) | (unsigned long long)cos_code(R.cosv);
                 atomicMin(pair_key + it.p, key);
                 if (!R.converged && !((it.w3 >> 24) & 1)) {
+                    // unconverged: the distance above stands as an upper bound; the leaf is quartered and the four
+                    // sub-leaves are solved by this lane (a seed solve is never split: the roots cover its pair)
                     cnt.fail++;
-                    resplit = choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP);
+                    bool splitP = false;
+                    if (sp + 4 <= NW_STACK && choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP)) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) stk[sp++] = nitem_child(it, splitP, c);
+                    } else cnt.depth++;
                 }
             }
-        }
-        const long long sl = warp_reserve(qout_n, resplit, 4, qcap, &S->status);
-        if (sl >= 0) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) qout[sl + c] = nitem_child(it, splitP, c);
         }
     }
     np_flush_counters(S, cnt);
@@ -368,26 +378,25 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_roots(DcScalars *S, const lo
 }
 
 // ------------------------------------------------------------------------------------------
-// Bound: one thread per item of qin[0 .. *n_in): prune, or 4 children -> qout, or leaf -> nq.
-__global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
-                                                          const int *__restrict__ pair_face, const double *__restrict__ fcoef,
-                                                          const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                          NItem *__restrict__ qout, int *__restrict__ qout_n,
-                                                          NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap)
+// Bound: one thread per item of qin[0 .. n): prune, or 4 children -> qout, or leaf -> the ONE leaf queue nq
+// (all rounds append to it; the Newton kernel runs once, after the last round).  Items i0, i0 + stride, ...
+__device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem *__restrict__ qin,
+                                               const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                               const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                               NItem *__restrict__ qout, int *__restrict__ qout_n,
+                                               NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap,
+                                               int i0, int stride, NpCounters &cnt)
 {
-    const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
-    if (n == 0) return;
-    if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
     const double t_tie = S->t_tie, tau_exit = S->tau_exit, theta2 = S->theta * S->theta;
     const int max_level = S->max_level;
-    NpCounters cnt = { 0, 0, 0, 0, 0 };
-    const int stride = gridDim.x * blockDim.x;
     const int n_round = (n + 31) & ~31;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+    for (int i = i0; i < n_round; i += stride) {
         bool split = false, leaf = false, splitP = false;
         NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
         if (i < n) {
-            it = qin[i];
+            // (L2 load: the tail kernel reads items the same launch wrote)
+            const uint4 w = __ldcg(reinterpret_cast<const uint4 *>(qin + i));
+            it.p = w.x; it.ak = w.y; it.w2 = w.z; it.w3 = w.w;
             const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
             double bst = u2d(__ldcg(best + b));
             if (bst > tau_exit) {
@@ -421,6 +430,41 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
 #pragma unroll
             for (int c = 0; c < 4; ++c) qout[slot + c] = nitem_child(it, splitP, c);
         }
+    }
+}
+
+__global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
+                                                          const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                                          const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                                          NItem *__restrict__ qout, int *__restrict__ qout_n,
+                                                          NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap)
+{
+    const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
+    if (n == 0) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
+    NpCounters cnt = { 0, 0, 0, 0, 0 };
+    np_bound_items(S, n, qin, pair_face, fcoef, ecoef, best, qout, qout_n, nq, nq_n, qcap,
+                   blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, cnt);
+    np_flush_counters(S, cnt);
+}
+
+// The rounds after the first few hold few items (deep levels exist only where the surface curves fast): ONE CTA
+// walks them all, round after round, until a round comes up empty -- no launch per round, no empty launches.
+#define NP_TAIL_THREADS 256
+__global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S, int r_begin, int r_end, NItem *q0, NItem *q1,
+                                                                   const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                                                   const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                                                   NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap)
+{
+    NpCounters cnt = { 0, 0, 0, 0, 0 };
+    for (int r = r_begin; r < r_end; ++r) {
+        const int n = min(*(volatile int *)&S->qn[r], (int)min(qcap, (long long)0x7fffffff));
+        if (n == 0) break;
+        if (threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
+        np_bound_items(S, n, (r & 1) ? q1 : q0, pair_face, fcoef, ecoef, best, (r & 1) ? q0 : q1, &S->qn[r + 1], nq, nq_n, qcap,
+                       threadIdx.x, NP_TAIL_THREADS, cnt);
+        __threadfence();
+        __syncthreads();
     }
     np_flush_counters(S, cnt);
 }
