@@ -13,9 +13,10 @@ nodes + connectivity + adjacency, surface faces) are resident in HBM before the 
   e2e     : the same through dc_classify_host with pinned HOST buffers: faces host->device, labels +
             signed distances device->host inside the timed region (the grid is registered once by
             dc_create_grid, as the paper does for grid-only structures).
-  roofline: the dominant kernel (k_narrow, FP64-ALU bound): algorithmic flops (counters x the
-            per-operation constants of DESIGN.md) / its CUDA-event duration, against the measured
-            DFMA peak of this GPU.  The HBM-bound S2 kernel is reported beside it ("roofline_s2").
+  roofline: the dominant kernel (k_np_newton, the closest-point solves of S5; FP64-ALU bound): algorithmic
+            flops (device counters x the per-operation constants of DESIGN.md) / its CUDA-event duration
+            (events recorded by the library around its two launches), against the DFMA peak measured on
+            this GPU in this run.  The HBM-bound S2 kernel is reported beside it ("roofline_s2").
   cpu_baseline: the oracle (oracle/dc_oracle.c, as it stands) on this box's host cores on a bounded
             uniform sample of the same workload's elements, each against ALL faces.
 
@@ -41,11 +42,11 @@ if ROOT not in sys.path:
 METRIC = "element_face_pair_tests_per_s"
 UNIT = "pair tests/s"
 
-# algorithmic fp64 flops per operation of the narrow phase
-FLOP_PER_BNB_NODE = 434.0       # 2 centre evals (2x27 FMA) + 2 re-centrings (3x33) + projections/norms + bounds
-FLOP_PER_NEWTON_ITER = 700.0    # 2 jets (3x2x~23 FMA) + gradient + Hessian (10 dots) + Cholesky 4x4 + f check
-FLOP_PER_NEWTON_SETUP = 400.0   # 2 re-centrings + final evaluation and normal
-BYTES_PER_ELEM_S2 = 27 * 4 + 27 * 24 / 8.0 + 48  # conn row + 3.375 unique nodes x 24 B (lattice share) + box
+# algorithmic fp64 flops per operation of the narrow phase (FMA = 2)
+FLOP_PER_BNB_NODE = 434.0       # 2 centre evals with first derivatives, 2 x 8 projected coefficients, 2 scalar ranges, leaf rule
+FLOP_PER_NEWTON_EVAL = 560.0    # 6 jets x 36 + (r, g, H) 3 x 43 + LDL^T 4x4 ~75 + trial point and its value 6 x 16 + 17 + tests ~35
+FLOP_PER_NEWTON_FINISH = 40.0   # normal, cosine, distance of a finished solve
+# S2 algorithmic bytes: every conn row (108 B) and every node (24 B) read once, one box (48 B) written per element
 
 
 def _peaks():
@@ -295,17 +296,24 @@ def main():
     # ---- rooflines
     hbm_peak, hbm_src = _peaks()
     fp64_peak = B.dc_measure_fp64_tflops(local_rank, 4000)
-    flops = (s_last.n_bnb_nodes * FLOP_PER_BNB_NODE + s_last.n_newton_iters * FLOP_PER_NEWTON_ITER
-             + s_last.n_newton * FLOP_PER_NEWTON_SETUP)
+    # dominant kernel: k_np_newton (two launches per cut: seed solves + leaf solves), timed by CUDA events
+    # recorded by the library on the caller's stream around exactly those launches (dc_stats.ms_stage[7])
+    newton_flops = s_last.n_newton_iters * FLOP_PER_NEWTON_EVAL + s_last.n_newton * FLOP_PER_NEWTON_FINISH
+    newton_ms = float(med[7])
+    ach_tf = newton_flops / (newton_ms * 1e-3) / 1e12 if newton_ms > 0 else 0.0
     narrow_ms = float(med[3])
-    ach_tf = flops / (narrow_ms * 1e-3) / 1e12 if narrow_ms > 0 else 0.0
-    s2_bytes = BYTES_PER_ELEM_S2 * w.n_elem
+    narrow_flops = newton_flops + s_last.n_bnb_nodes * FLOP_PER_BNB_NODE
+    s2_bytes = 108.0 * w.n_elem + 24.0 * len(w.xyz) + 48.0 * w.n_elem
     s2_ms = float(med[1])
     ach_gbs = s2_bytes / (s2_ms * 1e-3) / 1e9 if s2_ms > 0 else 0.0
-    roofline = {"kernel": "k_narrow (S5+S6)", "bound": "alu", "achieved": ach_tf, "peak": fp64_peak, "unit": "TFLOP/s",
+    roofline = {"kernel": "k_np_newton (S5 closest-point solves, 2 launches per cut)", "bound": "alu", "achieved": ach_tf,
+                "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": ach_tf / fp64_peak if fp64_peak > 0 else None, "traffic": None,
-                "peak_source": "dc_measure_fp64_tflops (register-resident DFMA chains) in this run",
-                "share_of_step": narrow_ms / float(med[5] + med[6]) if med[5] > 0 else None}
+                "algorithmic_flops_per_cut": newton_flops, "ms_per_cut": newton_ms,
+                "peak_source": "measured: dc_measure_fp64_tflops (register-resident DFMA chains on all SMs) in this run",
+                "share_of_step": newton_ms / float(med[5] + med[6]) if med[5] > 0 else None,
+                "narrow_phase_S5_S6": {"ms": narrow_ms, "algorithmic_flops": narrow_flops,
+                                       "achieved_tflops": narrow_flops / (narrow_ms * 1e-3) / 1e12 if narrow_ms > 0 else None}}
     roofline_s2 = {"kernel": "k_elem_boxes (S2)", "bound": "hbm", "achieved": ach_gbs, "peak": hbm_peak, "unit": "GB/s",
                    "frac": ach_gbs / hbm_peak, "traffic": None, "peak_source": hbm_src}
 

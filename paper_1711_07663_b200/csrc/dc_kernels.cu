@@ -835,7 +835,7 @@ struct dc_ctx {
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
     int *cell_count, *cell_start, *cell_fill;
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
-    cudaEvent_t ev[10];
+    cudaEvent_t ev[12];
     cudaStream_t last_stream;
     bool have_surface, have_cut;
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
@@ -977,7 +977,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
     cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
-    for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->ev[i]));
+    for (int i = 0; i < 12; ++i) CK(cudaEventCreate(&c->ev[i]));
     CK(cudaFuncSetAttribute(k_np_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, NW_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_np_newton, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
@@ -1050,8 +1050,10 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
                                            c->ecoef, c->pbox, c->best, c->dmin, c->nq);
     // seed solves: one per band element, queue = nq[0 .. n_band); failures are never re-split
     const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
+    CK(cudaEventRecord(c->ev[7], st));
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, c->pair_face, c->fcoef, c->ecoef,
                                                        c->best, c->dmin, c->pair_key);
+    CK(cudaEventRecord(c->ev[10], st));
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
                                            c->q[0], &S->qn[0], c->qcap);
     // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
@@ -1066,8 +1068,10 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
         k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                        c->nq, &S->nn[0], c->qcap);
     // all leaves in one launch; an unconverged leaf is quartered and finished by the lane that held it
+    CK(cudaEventRecord(c->ev[5], st));
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->pair_face, c->fcoef, c->ecoef,
                                                        c->best, c->dmin, c->pair_key);
+    CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
@@ -1173,6 +1177,8 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
         if (cudaEventElapsedTime(&ms, c->ev[2], c->ev[3]) == cudaSuccess) o->ms_stage[3] = ms;
         if (cudaEventElapsedTime(&ms, c->ev[3], c->ev[4]) == cudaSuccess) o->ms_stage[4] = ms;
         if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[4]) == cudaSuccess) o->ms_stage[5] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[5], c->ev[6]) == cudaSuccess) o->ms_stage[7] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[7], c->ev[10]) == cudaSuccess) o->ms_stage[7] += ms;
     }
     if (c->have_surface) {
         float ms;
@@ -1188,7 +1194,7 @@ extern "C" void dc_destroy(dc_ctx *c)
     if (!c) return;
     cudaSetDevice(c->device);
     if (c->last_stream || true) cudaStreamSynchronize(c->last_stream);
-    for (int i = 0; i < 10; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 12; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     if (c->S_host) cudaFreeHost(c->S_host);
     delete c;
 }

@@ -222,7 +222,8 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
 #pragma unroll
     for (int i = 0; i < 4; ++i) s.x[i] = 0.0;
     NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
-    bool exhausted = false;
+    NItem nxt; nxt.p = nxt.ak = nxt.w2 = nxt.w3 = 0;       // prefetched next item of this lane
+    int nst = 0, nface = 0;         // 0 none yet, 1 item asked for, 2 face id asked for too, 3 the queue is exhausted
     NItem stk[NW_STACK];            // sub-leaves of an unconverged solve, solved by the same lane (local memory, rarely touched)
     int sp = 0;
     while (true) {
@@ -234,37 +235,47 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
             s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
             s.iters = 0; s.ls = 0; s.phase = 1;
         }
-        // ---- refill idle lanes
+        // ---- refill idle lanes.  Every lane holds its NEXT item already (nxt, asked for when the lane took its
+        // current one, and the face id asked for one evaluation later), so a refill costs one memory round trip
+        // (the new item's coefficients) instead of four dependent ones (ticket -> item -> face id -> coefficients).
+        if (nst == 1) { nface = __ldg(pair_face + nxt.p); nst = 2; }
         for (int pass = 0; pass < 4; ++pass) {
-            const bool need = s.phase == 0 && !exhausted;
+            const bool need = s.phase == 0 && nst != 3;
             const unsigned mneed = __ballot_sync(0xffffffffu, need);
             const unsigned mbusy = __ballot_sync(0xffffffffu, s.phase != 0);
             if (!mneed || (__popc(mneed) < NW_REFILL && mbusy != 0)) break;
+            bool fresh = false;
+            unsigned long long pA = 0, pQ = 0;
+            if (need && nst != 0) {
+                it = nxt;
+                const int face = nst == 2 ? nface : __ldg(pair_face + it.p);
+                const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+                if (u2d(__ldcg(best + b)) > tau_exit) {          // else: the element is already CUT, drop the item
+                    fresh = true;
+                    double uc, vc, hP, sc, tc, hQ;
+                    nitem_box(it, uc, vc, hP, sc, tc, hQ);
+                    s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
+                    s.iters = 0; s.ls = 0; s.phase = 1;
+                    pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
+                    pQ = (unsigned long long)(fcoef + (size_t)face * 28);
+                }
+            }
+            // the lanes that took (or dropped, or never had) an item draw the ticket of their next one
             const int leader = __ffs(mneed) - 1;
             int base = 0;
             if (lane == leader) base = atomicAdd(head, __popc(mneed));
             base = __shfl_sync(0xffffffffu, base, leader);
-            bool fresh = false;
-            unsigned long long pA = 0, pQ = 0;
             if (need) {
                 const int i = base + __popc(mneed & lt_mask);
-                if (i >= n) exhausted = true;
+                if (i >= n) nst = 3;
                 else {
-                    it = nq[i];
-                    const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
-                    if (u2d(__ldcg(best + b)) > tau_exit) {          // else: the element is already CUT, drop the item
-                        fresh = true;
-                        double uc, vc, hP, sc, tc, hQ;
-                        nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                        s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
-                        s.iters = 0; s.ls = 0; s.phase = 1;
-                        pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
-                        pQ = (unsigned long long)(fcoef + (size_t)__ldg(pair_face + it.p) * 28);
-                    }
+                    const uint4 w = __ldg(reinterpret_cast<const uint4 *>(nq + i));
+                    nxt.p = w.x; nxt.ak = w.y; nxt.w2 = w.z; nxt.w3 = w.w;
+                    nst = 1;
                 }
             }
             unsigned mf = __ballot_sync(0xffffffffu, fresh);
-            const bool dropped = __ballot_sync(0xffffffffu, need && !fresh && !exhausted) != 0;
+            const bool again = __ballot_sync(0xffffffffu, need && !fresh && nst != 3) != 0;
             while (mf) {
                 const int L = __ffs(mf) - 1; mf &= mf - 1;
                 const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
@@ -274,10 +285,10 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 if (lane < 22) dst[(lane + 32) * NW_STRIDE] = __ldg(q + (lane + 5));
             }
             __syncwarp();
-            if (!dropped) break;
+            if (!again) break;
         }
         if (__ballot_sync(0xffffffffu, s.phase != 0) == 0) {
-            if (__ballot_sync(0xffffffffu, !exhausted) == 0) break;
+            if (__ballot_sync(0xffffffffu, nst != 3 || sp > 0) == 0) break;
             continue;
         }
         // ---- one evaluation per busy lane
