@@ -268,18 +268,23 @@ __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const d
                                                            const int *__restrict__ conn, long long n_elem,
                                                            double *__restrict__ ebox)
 {
+    // One (element, coordinate) pair per work item, 3 items per thread: consecutive lanes read CONSECUTIVE
+    // doubles of a node (x, y, z of one element, then the next element), so one warp load touches a third
+    // of the sectors a lane-per-element gather would, and the Lagrange -> Bezier conversion is per coordinate
+    // anyway.  conn rows are staged through shared memory (coalesced).
     __shared__ int s_conn[EB_THREADS * 27];
+    __shared__ double s_ext2[EB_THREADS * 3];
     const long long e0 = (long long)blockIdx.x * EB_THREADS;
     const int nloc = (int)min((long long)EB_THREADS, n_elem - e0);
     for (int i = threadIdx.x; i < nloc * 27; i += EB_THREADS) s_conn[i] = __ldg(conn + e0 * 27 + i);
     __syncthreads();
-    double diag2 = 0.0;
-    if (threadIdx.x < nloc) {
-        const long long e = e0 + threadIdx.x;
-        const int *cn = s_conn + threadIdx.x * 27;
-        double ext2 = 0.0;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
+    const int wbase = (threadIdx.x >> 5) * 32, lane = threadIdx.x & 31;
+#pragma unroll 1
+    for (int j = 0; j < 3; ++j) {
+        const int idx = j * 32 + lane;               // 0..95 within the warp's 32 elements
+        const int el = wbase + idx / 3, c = idx % 3;
+        if (el < nloc) {
+            const int *cn = s_conn + el * 27;
             double b[27];
 #pragma unroll
             for (int m = 0; m < 27; ++m) b[m] = __ldg(xyz + (size_t)cn[m] * 3 + c);
@@ -295,12 +300,15 @@ __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const d
             double lo = INFINITY, hi = -INFINITY;
 #pragma unroll
             for (int m = 0; m < 27; ++m) if (m != 13) { lo = fmin(lo, b[m]); hi = fmax(hi, b[m]); }
+            const long long e = e0 + el;
             ebox[(size_t)c * n_elem + e] = lo;
             ebox[(size_t)(3 + c) * n_elem + e] = hi;
-            ext2 = fma(hi - lo, hi - lo, ext2);
+            s_ext2[el * 3 + c] = (hi - lo) * (hi - lo);
         }
-        diag2 = ext2;
     }
+    __syncthreads();
+    double diag2 = 0.0;
+    if (threadIdx.x < nloc) diag2 = s_ext2[threadIdx.x * 3] + s_ext2[threadIdx.x * 3 + 1] + s_ext2[threadIdx.x * 3 + 2];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) diag2 = fmax(diag2, __shfl_xor_sync(0xffffffffu, diag2, o));
     if ((threadIdx.x & 31) == 0) atomicMax(&S->grid_max_diag2, (unsigned long long)__double_as_longlong(diag2));

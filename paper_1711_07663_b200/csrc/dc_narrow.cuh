@@ -152,7 +152,39 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
             bx[k * 6 + c] = lo; bx[k * 6 + 3 + c] = hi;
         }
         __syncwarp();
-        if (lane < 6) cf[lane * 28 + 27] = higher_order_const(cf + lane * 28);
+        // constants K of the 6 patches (dc_geom.cuh higher_order_const): the 6 x 6 coefficient norms it needs are
+        // spread over the warp (a lane per norm) instead of 9 square roots in a row on 6 lanes
+        {
+            // weights of |A20| |A02| |A11| |A21| |A12| |A22| (m = 2, 6, 4, 5, 7, 8) in K
+            const int mm[6] = { 2, 6, 4, 5, 7, 8 };
+            const double ww[6] = { 1.0, 1.0, 1.0, 4.0, 4.0, 11.0 };
+            double part = 0.0, part2 = 0.0;
+            {
+                const int k = lane / 6, j = lane % 6;           // lanes 0..31 -> (patch, norm) 0..31
+                const double *A = cf + k * 28;
+                const int m = mm[j];
+                part = ww[j] * sqrt(A[m] * A[m] + A[9 + m] * A[9 + m] + A[18 + m] * A[18 + m]);
+            }
+            if (lane < 4) {                                     // (patch 5, norms 2..5) = items 32..35
+                const int j = lane + 2;
+                const double *A = cf + 5 * 28;
+                const int m = mm[j];
+                part2 = ww[j] * sqrt(A[m] * A[m] + A[9 + m] * A[9 + m] + A[18 + m] * A[18 + m]);
+            }
+            // sum the 6 norms of each patch: lanes 6k .. 6k+5 (patch 5: lanes 30, 31 + part2 of lanes 0..3)
+            double sum = part;
+#pragma unroll
+            for (int o = 1; o < 6; ++o) {
+                const double v = __shfl_down_sync(0xffffffffu, part, o);
+                if (lane % 6 + o < 6 && lane + o < 32) sum += v;
+            }
+            double tail = part2;
+            tail += __shfl_down_sync(0xffffffffu, tail, 2);
+            tail += __shfl_down_sync(0xffffffffu, tail, 1);
+            tail = __shfl_sync(0xffffffffu, tail, 0);
+            if (lane % 6 == 0 && lane < 30) cf[(lane / 6) * 28 + 27] = sum;
+            if (lane == 30) cf[5 * 28 + 27] = sum + tail;
+        }
         __syncwarp();
         for (int i = lane; i < 6 * 28; i += 32) ecoef[(size_t)b * (6 * 28) + i] = cf[i];
         for (int i = lane; i < 36; i += 32) pbox[(size_t)b * 36 + i] = bx[i];
@@ -165,15 +197,15 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
             const int f = __ldg(pair_face + p0 + pl);
             const double *AQ = fcoef + (size_t)f * 28;
             const double dx = cf[k * 28] - __ldg(AQ), dy = cf[k * 28 + 9] - __ldg(AQ + 9), dz = cf[k * 28 + 18] - __ldg(AQ + 18);
-            const double d = sqrt(dx * dx + dy * dy + dz * dz);
-            const unsigned long long kk = (d2u(d) & ~0xfffffull) | (unsigned long long)min(t, 0xfffff);
+            const double d2 = dx * dx + dy * dy + dz * dz;           // (squared: one sqrt per element, below)
+            const unsigned long long kk = (d2u(d2) & ~0xfffffull) | (unsigned long long)min(t, 0xfffff);
             key = kk < key ? kk : key;
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, key, o); key = v < key ? v : key; }
         if (lane == 0) {
-            // the truncated key distance is <= the attained one: round up to stay an upper bound
-            const double dkey = u2d((key & ~0xfffffull) + 0x100000ull);
+            // the truncated key is <= the attained squared distance: round up to stay an upper bound
+            const double dkey = sqrt(u2d((key & ~0xfffffull) + 0x100000ull)) * (1.0 + 4e-16);
             best[b] = d2u(fmin(reach, dkey));
             dmin[b] = 0x7ff0000000000000ull;
             const int t = (int)(key & 0xfffffull);
