@@ -270,7 +270,13 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
         // ---- refill idle lanes.  Every lane holds its NEXT item already (nxt, asked for when the lane took its
         // current one, and the face id asked for one evaluation later), so a refill costs one memory round trip
         // (the new item's coefficients) instead of four dependent ones (ticket -> item -> face id -> coefficients).
-        if (nst == 1) { nface = __ldg(pair_face + nxt.p); nst = 2; }
+        if (nst == 1) {
+            nface = __ldg(pair_face + nxt.p); nst = 2;
+            // pull the next element patch's coefficients (224 B of the large ecoef array) into L2 ahead of the refill
+            const char *pn = reinterpret_cast<const char *>(ecoef + ((size_t)(nxt.ak & 0x1fffffffu) * 6 + (nxt.ak >> 29)) * 28);
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(pn));
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(pn + 128));
+        }
         for (int pass = 0; pass < 4; ++pass) {
             const bool need = s.phase == 0 && nst != 3;
             const unsigned mneed = __ballot_sync(0xffffffffu, need);
