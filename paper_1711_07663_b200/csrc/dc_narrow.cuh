@@ -255,7 +255,10 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
     for (int i = 0; i < 4; ++i) s.x[i] = 0.0;
     NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
     NItem nxt; nxt.p = nxt.ak = nxt.w2 = nxt.w3 = 0;       // prefetched next item of this lane
-    int nst = 0, nface = 0;         // 0 none yet, 1 item asked for, 2 face id asked for too, 3 the queue is exhausted
+    // 0 no ticket, 1 ticket asked for, 2 ticket in hand, 3 item asked for, 4 face id and best[b] asked for (ready), 9 queue exhausted
+    int nst = 0, nface = 0, tk = 0, pbase = 0, pleader = 0;
+    unsigned long long nbest = 0;
+    bool pend = false;              // (warp-uniform) a ticket atomic is in flight
     NItem stk[NW_STACK];            // sub-leaves of an unconverged solve, solved by the same lane (local memory, rarely touched)
     int sp = 0;
     while (true) {
@@ -267,66 +270,88 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
             s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
             s.iters = 0; s.ls = 0; s.phase = 1;
         }
-        // ---- refill idle lanes.  Every lane holds its NEXT item already (nxt, asked for when the lane took its
-        // current one, and the face id asked for one evaluation later), so a refill costs one memory round trip
-        // (the new item's coefficients) instead of four dependent ones (ticket -> item -> face id -> coefficients).
-        if (nst == 1) {
-            nface = __ldg(pair_face + nxt.p); nst = 2;
-            // pull the next element patch's coefficients (224 B of the large ecoef array) into L2 ahead of the refill
-            const char *pn = reinterpret_cast<const char *>(ecoef + ((size_t)(nxt.ak & 0x1fffffffu) * 6 + (nxt.ak >> 29)) * 28);
+        // ---- every lane runs a small pipeline that fetches its NEXT item while it solves the current one, one
+        // stage per trip, so that no trip waits for more than one memory round trip: ticket (warp-aggregated
+        // atomic) -> item -> face id, best[b], L2 prefetch of the element coefficients -> ready.
+        if (nst == 3) {
+            const unsigned nb = nxt.ak & 0x1fffffffu;
+            nface = __ldg(pair_face + nxt.p);
+            nbest = __ldcg(best + nb);
+            const char *pn = reinterpret_cast<const char *>(ecoef + ((size_t)nb * 6 + (nxt.ak >> 29)) * 28);
             asm volatile("prefetch.global.L2 [%0];" :: "l"(pn));
             asm volatile("prefetch.global.L2 [%0];" :: "l"(pn + 128));
+            nst = 4;
+        } else if (nst == 2) {
+            if (tk >= n) nst = 9;
+            else {
+                const uint4 w = __ldg(reinterpret_cast<const uint4 *>(nq + tk));
+                nxt.p = w.x; nxt.ak = w.y; nxt.w2 = w.z; nxt.w3 = w.w;
+                nst = 3;
+            }
         }
-        for (int pass = 0; pass < 4; ++pass) {
-            const bool need = s.phase == 0 && nst != 3;
-            const unsigned mneed = __ballot_sync(0xffffffffu, need);
+        if (pend) {                                   // (uniform) the ticket atomic of the previous trip has landed
+            const int base = __shfl_sync(0xffffffffu, pbase, pleader);
+            if (nst == 1) { tk = base + tk; nst = 2; }
+            pend = false;
+        }
+        // ---- idle lanes whose next item is ready take it
+        bool fresh = false;
+        unsigned long long pA = 0, pQ = 0;
+        {
+            const bool ready = s.phase == 0 && nst == 4;
+            const unsigned mready = __ballot_sync(0xffffffffu, ready);
             const unsigned mbusy = __ballot_sync(0xffffffffu, s.phase != 0);
-            if (!mneed || (__popc(mneed) < NW_REFILL && mbusy != 0)) break;
-            bool fresh = false;
-            unsigned long long pA = 0, pQ = 0;
-            if (need && nst != 0) {
-                it = nxt;
-                const int face = nst == 2 ? nface : __ldg(pair_face + it.p);
-                const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
-                if (u2d(__ldcg(best + b)) > tau_exit) {          // else: the element is already CUT, drop the item
-                    fresh = true;
-                    double uc, vc, hP, sc, tc, hQ;
-                    nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                    s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
-                    s.iters = 0; s.ls = 0; s.phase = 1;
-                    pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
-                    pQ = (unsigned long long)(fcoef + (size_t)face * 28);
+            if (mready && (__popc(mready) >= NW_REFILL || mbusy == 0)) {
+                if (ready) {
+                    it = nxt; nst = 0;
+                    if (u2d(nbest) > tau_exit) {      // else: the element is already CUT, drop the item
+                        const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+                        fresh = true;
+                        double uc, vc, hP, sc, tc, hQ;
+                        nitem_box(it, uc, vc, hP, sc, tc, hQ);
+                        s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
+                        s.iters = 0; s.ls = 0; s.phase = 1;
+                        pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
+                        pQ = (unsigned long long)(fcoef + (size_t)nface * 28);
+                    }
                 }
             }
-            // the lanes that took (or dropped, or never had) an item draw the ticket of their next one
-            const int leader = __ffs(mneed) - 1;
-            int base = 0;
-            if (lane == leader) base = atomicAdd(head, __popc(mneed));
-            base = __shfl_sync(0xffffffffu, base, leader);
-            if (need) {
-                const int i = base + __popc(mneed & lt_mask);
-                if (i >= n) nst = 3;
-                else {
-                    const uint4 w = __ldg(reinterpret_cast<const uint4 *>(nq + i));
-                    nxt.p = w.x; nxt.ak = w.y; nxt.w2 = w.z; nxt.w3 = w.w;
-                    nst = 1;
-                }
+        }
+        // ---- lanes without a next item draw a ticket (the result is looked at next trip)
+        {
+            const unsigned m0 = __ballot_sync(0xffffffffu, nst == 0);
+            if (m0 && !pend) {
+                pleader = __ffs(m0) - 1;
+                if (lane == pleader) pbase = atomicAdd(head, __popc(m0));
+                if (nst == 0) { tk = __popc(m0 & lt_mask); nst = 1; }
+                pend = true;
             }
+        }
+        // ---- warp-cooperative, coalesced copy of the new items' coefficients into the lanes' slots: asynchronous
+        // copies (cp.async, 8 bytes per lane), ALL issued before the one wait, so the new lanes of a trip cost one
+        // memory round trip together (a load/store loop waited for each lane's loads in turn)
+        {
             unsigned mf = __ballot_sync(0xffffffffu, fresh);
-            const bool again = __ballot_sync(0xffffffffu, need && !fresh && nst != 3) != 0;
-            while (mf) {
-                const int L = __ffs(mf) - 1; mf &= mf - 1;
-                const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
-                const double *q = (const double *)__shfl_sync(0xffffffffu, pQ, L);
-                double *dst = wslot + L;
-                dst[lane * NW_STRIDE] = lane < 27 ? __ldg(a + lane) : __ldg(q + (lane - 27));
-                if (lane < 22) dst[(lane + 32) * NW_STRIDE] = __ldg(q + (lane + 5));
+            if (mf) {
+                do {
+                    const int L = __ffs(mf) - 1; mf &= mf - 1;
+                    const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
+                    const double *q = (const double *)__shfl_sync(0xffffffffu, pQ, L);
+                    double *dst = wslot + L;
+                    const unsigned d0 = (unsigned)__cvta_generic_to_shared(dst + lane * NW_STRIDE);
+                    const double *g0 = lane < 27 ? a + lane : q + (lane - 27);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0), "l"(g0));
+                    if (lane < 22) {
+                        const unsigned d1 = (unsigned)__cvta_generic_to_shared(dst + (lane + 32) * NW_STRIDE);
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d1), "l"(q + (lane + 5)));
+                    }
+                } while (mf);
+                asm volatile("cp.async.wait_all;" ::: "memory");
             }
             __syncwarp();
-            if (!again) break;
         }
         if (__ballot_sync(0xffffffffu, s.phase != 0) == 0) {
-            if (__ballot_sync(0xffffffffu, nst != 3 || sp > 0) == 0) break;
+            if (__ballot_sync(0xffffffffu, nst != 9 || sp > 0) == 0) break;
             continue;
         }
         // ---- one evaluation per busy lane
