@@ -263,7 +263,13 @@ __global__ void k_face_scatter(const double *__restrict__ face_nodes, const doub
 // S2: conservative element boxes from the 26 boundary control points of the Bezier net.
 // One thread per element; conn rows are staged through shared memory so the global reads
 // are fully coalesced.  ebox is SoA: ebox[c*n_elem + e] (c = 0..5: min xyz, max xyz).
+#ifndef EB_THREADS
 #define EB_THREADS 128
+#endif
+#ifndef EB_UNROLL
+#define EB_UNROLL 3
+#endif
+constexpr int kEbUnroll = EB_UNROLL;
 __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const double *__restrict__ xyz,
                                                            const int *__restrict__ conn, long long n_elem,
                                                            double *__restrict__ ebox)
@@ -279,7 +285,7 @@ __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const d
     for (int i = threadIdx.x; i < nloc * 27; i += EB_THREADS) s_conn[i] = __ldg(conn + e0 * 27 + i);
     __syncthreads();
     const int wbase = (threadIdx.x >> 5) * 32, lane = threadIdx.x & 31;
-#pragma unroll 1
+#pragma unroll kEbUnroll
     for (int j = 0; j < 3; ++j) {
         const int idx = j * 32 + lane;               // 0..95 within the warp's 32 elements
         const int el = wbase + idx / 3, c = idx % 3;

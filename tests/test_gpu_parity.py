@@ -234,3 +234,18 @@ def test_error_codes(B):
     # the reported size is sufficient
     l, s, st2 = gpu_cut(B, w, max_pairs=int(st.pairs_needed))
     assert st2.status == 0 and st2.n_pairs == st.pairs_needed
+
+
+# ------------------------------------------------------------------------------ coarse grid, fine surface
+def test_many_faces_per_element(B, nproc):
+    """Large elements against a fine surface: hundreds of candidate faces per element, so k_pairs leaves its
+    shared-memory stage (PR_CAP survivors) and re-walks the ranges, and the face bins span many cell blocks
+    (the failure mode of box-only ranking in PAPER.md Fig. 10: exactness must not depend on a fixed K)."""
+    w = make_config(1, N=5, n=14)           # 125 hexes of edge 0.4 vs 1176 faces of edge ~0.06
+    ref = O.classify(w.xyz, w.conn27, w.faces, nproc=nproc)
+    labels, sdist, st, dcut = gpu_cut(B, w, keep=True)
+    e, f = dcut.pairs()
+    dcut.close()
+    assert np.bincount(e).max() > 224, "this case is meant to overflow the per-warp pair stage"
+    assert_parity(ref, labels, sdist, st)
+    assert st.n_cut > 20
