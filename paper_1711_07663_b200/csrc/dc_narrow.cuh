@@ -327,28 +327,21 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 pend = true;
             }
         }
-        // ---- warp-cooperative, coalesced copy of the new items' coefficients into the lanes' slots: asynchronous
-        // copies (cp.async, 8 bytes per lane), ALL issued before the one wait, so the new lanes of a trip cost one
-        // memory round trip together (a load/store loop waited for each lane's loads in turn)
-        {
-            unsigned mf = __ballot_sync(0xffffffffu, fresh);
-            if (mf) {
-                do {
-                    const int L = __ffs(mf) - 1; mf &= mf - 1;
-                    const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
-                    const double *q = (const double *)__shfl_sync(0xffffffffu, pQ, L);
-                    double *dst = wslot + L;
-                    const unsigned d0 = (unsigned)__cvta_generic_to_shared(dst + lane * NW_STRIDE);
-                    const double *g0 = lane < 27 ? a + lane : q + (lane - 27);
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0), "l"(g0));
-                    if (lane < 22) {
-                        const unsigned d1 = (unsigned)__cvta_generic_to_shared(dst + (lane + 32) * NW_STRIDE);
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d1), "l"(q + (lane + 5)));
-                    }
-                } while (mf);
-                asm volatile("cp.async.wait_all;" ::: "memory");
+        // ---- the new items' coefficients go into their lanes' slots by asynchronous copies (cp.async, 8 bytes each),
+        // ALL issued before the one wait, so the new lanes of a trip cost one memory round trip together.
+        // Lane-private: every new lane copies its own 54 coefficients (54 predicated instructions per trip however
+        // many lanes are new; a warp-cooperative coalesced copy cost ~30 instructions per new lane, ~6 per trip, for no gain).
+        if (__ballot_sync(0xffffffffu, fresh)) {
+            if (fresh) {
+                const double *a = (const double *)pA, *q = (const double *)pQ;
+                const unsigned d0 = (unsigned)__cvta_generic_to_shared(nw_sm + tid);
+#pragma unroll
+                for (int m = 0; m < 27; ++m) {
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0 + m * (NW_STRIDE * 8)), "l"(a + m));
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0 + (27 + m) * (NW_STRIDE * 8)), "l"(q + m));
+                }
             }
-            __syncwarp();
+            asm volatile("cp.async.wait_all;" ::: "memory");
         }
         if (__ballot_sync(0xffffffffu, s.phase != 0) == 0) {
             if (__ballot_sync(0xffffffffu, nst != 9 || sp > 0) == 0) break;
