@@ -168,6 +168,39 @@ void dc_destroy(dc_ctx *ctx);
 
 const char *dc_error_string(int code);
 
+/* ---- blanking logic that consumes direct cuts --------------------------------
+ * Stateless device routines: plain device pointers owned by the caller, enqueued on `stream`, no host sync.
+ * A blanking vector `iblank` is int8 per element: 1 = blanked ("hole cell"), 0 = field.  `cut_is_hole` != 0
+ * counts DC_CUT elements as hole cells (the paper leaves the CUT elements of a wall cut to the caller). */
+#define DC_MODE_WALL 0      /* body grid cut by solid wall surfaces (Algorithm 3.1 step 6) */
+#define DC_MODE_OVERSET 1   /* background grid cut by overset boundary surfaces (step 7) */
+
+/* Union of the hole cells of two cutting boundaries: out = HOLE if either is HOLE, else CUT if
+ * either is CUT, else NORMAL.  out_dev may alias a_dev or b_dev.  All [n_elem] int8 dev. */
+int dc_union_labels(long long n_elem, const signed char *a_dev, const signed char *b_dev,
+                    signed char *out_dev, void *stream);
+
+/* Algorithm 3.1 steps 6-7 for one grid.
+ *   iblank_prev_dev [n_elem] int8 dev  in   I_{t-}: the blanking used for the previous time step (step 1)
+ *   labels_t_dev, labels_tplus_dev      in   dc_classify labels of the cuts at t (step 5) and t + dt (step 3)
+ *   iblank_out_dev  [n_elem] int8 dev  out  the blanking of this step: wall  -> hole at t OR at t + dt  (6.1),
+ *                                           overset -> hole at t AND at t + dt (L112); may alias iblank_prev_dev
+ *   unblank_list_dev [list_cap] i32 dev out elements that were blanked and must be unblanked now (6.2, 7.1)
+ *   tohole_list_dev  [list_cap] i32 dev out elements newly blanked by this step (NULL: not wanted)
+ *   counts_dev       [2] i64 dev        out number of must-unblank / to-hole elements (may exceed list_cap: the
+ *                                           lists are then truncated; ids appear in no particular order)
+ * Returns DC_ERR_ARG on NULL / negative arguments or an unknown mode. */
+int dc_unblank(int mode, int cut_is_hole, long long n_elem, const signed char *iblank_prev_dev,
+               const signed char *labels_t_dev, const signed char *labels_tplus_dev,
+               signed char *iblank_out_dev, int *unblank_list_dev, int *tohole_list_dev, long long list_cap,
+               long long *counts_dev, void *stream);
+
+/* Artificial-boundary faces ("any face which has a hole cell on one side and a normal/field cell on
+ * the other"): ab_mask_dev[e] gets bit k set iff e is a field cell and adj6[e][k] is a hole cell (each AB face is
+ * reported on its field side); count_dev [1] i64 dev gets the number of AB faces (NULL: not wanted). */
+int dc_ab_faces(long long n_elem, const signed char *iblank_dev, const int *adj6_dev,
+                unsigned char *ab_mask_dev, long long *count_dev, void *stream);
+
 /* FP64 FMA peak microbenchmark (register-resident DFMA chains on every SM): returns measured
  * TFLOP/s (2 flop per FMA) or a negative error.  Used by bench.py for the "alu" roofline. */
 double dc_measure_fp64_tflops(int device, int iters);

@@ -17,10 +17,12 @@ DC_HOLE, DC_NORMAL, DC_CUT = 0, 1, 2
 DC_OK, DC_ERR_ARG, DC_ERR_WORKSPACE, DC_ERR_UNSUPPORTED, DC_ERR_CUDA, DC_ERR_STATE = 0, -1, -2, -3, -4, -5
 DC_STATUS_PAIR_OVERFLOW, DC_STATUS_QUEUE_OVERFLOW, DC_STATUS_FILL_CONFLICT, DC_STATUS_SEEDLESS_OVERFLOW = 1, 2, 4, 8
 DC_FLAG_RECOMPUTE_BOXES = 1
+DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
 
 EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify",
            "dc_classify_host", "dc_get_element_boxes", "dc_get_adjacency", "dc_get_pairs",
-           "dc_get_stats", "dc_destroy", "dc_error_string", "dc_measure_fp64_tflops", "dc_version"]
+           "dc_get_stats", "dc_destroy", "dc_error_string", "dc_measure_fp64_tflops", "dc_version",
+           "dc_union_labels", "dc_unblank", "dc_ab_faces"]
 
 
 class dc_params(C.Structure):
@@ -72,6 +74,9 @@ _lib.dc_error_string.restype = C.c_char_p
 _lib.dc_measure_fp64_tflops.argtypes = [C.c_int, C.c_int]
 _lib.dc_measure_fp64_tflops.restype = C.c_double
 _lib.dc_version.restype = C.c_int
+_lib.dc_union_labels.argtypes = [C.c_longlong, _vp, _vp, _vp, _vp]
+_lib.dc_unblank.argtypes = [C.c_int, C.c_int, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp, C.c_longlong, _vp, _vp]
+_lib.dc_ab_faces.argtypes = [C.c_longlong, _vp, _vp, _vp, _vp, _vp]
 
 
 class DcError(RuntimeError):
@@ -132,6 +137,51 @@ def dc_measure_fp64_tflops(device: int = 0, iters: int = 2000) -> float:
 
 def dc_version() -> int:
     return int(_lib.dc_version())
+
+
+# ---- blanking logic on torch CUDA tensors (argument marshalling only; include/dc.h documents the calls) ----------
+def _stream(t):
+    import torch
+    return C.c_void_p(torch.cuda.current_stream(t.device).cuda_stream)
+
+
+def dc_union_labels(a, b, out=None):
+    import torch
+    out = torch.empty_like(a) if out is None else out
+    rc = _lib.dc_union_labels(a.numel(), a.data_ptr(), b.data_ptr(), out.data_ptr(), _stream(a))
+    if rc:
+        raise DcError(rc, "dc_union_labels")
+    return out
+
+
+def dc_unblank(mode: int, cut_is_hole: bool, iblank_prev, labels_t, labels_tplus, list_cap: Optional[int] = None,
+               want_tohole: bool = True):
+    """Returns (iblank_new int8 tensor, must_unblank ids, to_hole ids) -- the id lists in no particular order."""
+    import torch
+    n = iblank_prev.numel()
+    cap = n if list_cap is None else int(list_cap)
+    out = torch.empty(n, dtype=torch.int8, device=iblank_prev.device)
+    unb = torch.empty(max(cap, 1), dtype=torch.int32, device=iblank_prev.device)
+    toh = torch.empty(max(cap, 1), dtype=torch.int32, device=iblank_prev.device) if want_tohole else None
+    counts = torch.zeros(2, dtype=torch.int64, device=iblank_prev.device)
+    rc = _lib.dc_unblank(int(mode), int(bool(cut_is_hole)), n, iblank_prev.data_ptr(), labels_t.data_ptr(),
+                         labels_tplus.data_ptr(), out.data_ptr(), unb.data_ptr(),
+                         toh.data_ptr() if toh is not None else None, cap, counts.data_ptr(), _stream(iblank_prev))
+    if rc:
+        raise DcError(rc, "dc_unblank")
+    c = counts.cpu().tolist()
+    return out, unb[:min(c[0], cap)], (toh[:min(c[1], cap)] if toh is not None else None), c
+
+
+def dc_ab_faces(iblank, adj6):
+    import torch
+    n = iblank.numel()
+    mask = torch.empty(n, dtype=torch.uint8, device=iblank.device)
+    count = torch.zeros(1, dtype=torch.int64, device=iblank.device)
+    rc = _lib.dc_ab_faces(n, iblank.data_ptr(), adj6.data_ptr(), mask.data_ptr(), count.data_ptr(), _stream(iblank))
+    if rc:
+        raise DcError(rc, "dc_ab_faces")
+    return mask, int(count.item())
 
 
 # ---- convenience owner of the torch buffers ----------------------------------------------------

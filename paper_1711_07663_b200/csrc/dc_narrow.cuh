@@ -243,7 +243,6 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
     const int tid = threadIdx.x, lane = tid & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     const double *slot = nw_sm + tid;
-    double *wslot = nw_sm + (tid & ~31);
     const volatile double *vslot = slot;   // volatile: re-read in the line search instead of keeping 54 values live
     auto cf = [&](int m) { return vslot[m * NW_STRIDE]; };
     const double tau_exit = S->tau_exit, tol_d2 = S->tol_d * S->tol_d;
