@@ -373,11 +373,20 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
 // S4a: one thread per element.  Initialises the per-element state of this cut and appends the
 // elements whose inflated box overlaps a non-empty 4x4x4 block of face cells to the active list
 // (warp-aggregated atomic append).  A block of 64 cells is one contiguous range of the Morton order.
-__device__ __forceinline__ int block_faces(const int *__restrict__ cell_start, int bx, int by, int bz, int &first)
+// faces of the Morton-aligned block of 2^s x 2^s x 2^s cells with block coordinates (bx, by, bz): ONE contiguous range
+__device__ __forceinline__ int block_faces(const int *__restrict__ cell_start, int bx, int by, int bz, int s, int &first)
 {
-    const unsigned c0 = morton3(bx, by, bz) << 6;
+    const unsigned c0 = morton3(bx, by, bz) << (3 * s);
     first = __ldg(cell_start + c0);
-    return __ldg(cell_start + c0 + 64) - first;
+    return __ldg(cell_start + c0 + (1u << (3 * s))) - first;
+}
+// block level of a query over the cells [i0, i1]: the finest one with at most 4 blocks per axis (64 ranges, two
+// per lane); the blocks then cover at most (4 / 3)^3 ... 2^3 times the cells of the query, whatever its size
+__device__ __forceinline__ int block_level(const int *i0, const int *i1)
+{
+    int s = 0;
+    while (s < 7 && (((i1[0] >> s) - (i0[0] >> s)) > 3 || ((i1[1] >> s) - (i0[1] >> s)) > 3 || ((i1[2] >> s) - (i0[2] >> s)) > 3)) ++s;
+    return s;
 }
 
 __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
@@ -401,14 +410,15 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
         const double reach = S->reach;
         if (d2 <= reach * reach) {
             const double pad = reach + S->fhalf;
-            int b0[3], b1[3];
+            int i0[3], i1[3];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { b0[c] = cell_coord(S, lo[c] - pad, c) >> 2; b1[c] = cell_coord(S, hi[c] + pad, c) >> 2; }
-            for (int z = b0[2]; z <= b1[2] && !active; ++z)
-                for (int y = b0[1]; y <= b1[1] && !active; ++y)
-                    for (int x = b0[0]; x <= b1[0]; ++x) {
+            for (int c = 0; c < 3; ++c) { i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c); }
+            const int sl = block_level(i0, i1);
+            for (int z = i0[2] >> sl; z <= (i1[2] >> sl) && !active; ++z)
+                for (int y = i0[1] >> sl; y <= (i1[1] >> sl) && !active; ++y)
+                    for (int x = i0[0] >> sl; x <= (i1[0] >> sl); ++x) {
                         int first;
-                        if (block_faces(cell_start, x, y, z, first) > 0) { active = true; break; }
+                        if (block_faces(cell_start, x, y, z, sl, first) > 0) { active = true; break; }
                     }
         }
     }
@@ -463,13 +473,15 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
     for (int a = warp; a < n_active; a += nwarps) {
         const long long e = act_elem[a];
         double lo[3], hi[3];
-        int b0[3], nb[3];
+        int b0[3], nb[3], i0[3], i1[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e];
-            b0[c] = cell_coord(S, lo[c] - pad, c) >> 2;
-            nb[c] = (cell_coord(S, hi[c] + pad, c) >> 2) - b0[c] + 1;
+            i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c);
         }
+        const int sl = block_level(i0, i1);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { b0[c] = i0[c] >> sl; nb[c] = (i1[c] >> sl) - b0[c] + 1; }
         const int nblk = nb[0] * nb[1] * nb[2];
         long long base = 0;
         int total = 0;
@@ -478,7 +490,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
             for (int bbase = 0; bbase < nblk; bbase += 32) {
                 const int bi = bbase + lane;
                 int cnt = 0, first = 0;
-                if (bi < nblk) cnt = block_faces(cell_start, b0[0] + bi % nb[0], b0[1] + (bi / nb[0]) % nb[1], b0[2] + bi / (nb[0] * nb[1]), first);
+                if (bi < nblk) cnt = block_faces(cell_start, b0[0] + bi % nb[0], b0[1] + (bi / nb[0]) % nb[1], b0[2] + bi / (nb[0] * nb[1]), sl, first);
                 int incl = cnt;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
