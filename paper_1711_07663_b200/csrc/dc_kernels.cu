@@ -1066,7 +1066,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     CK(cudaEventRecord(c->ev[1], st));
     k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
     k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->act_elem);
-    k_pairs<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
+    k_pairs<<<c->num_sms * 16, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
                                            c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key);
     CK(cudaEventRecord(c->ev[2], st));
     // ---- S5: wavefront narrow phase (dc_narrow.cuh)
