@@ -125,12 +125,20 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
     const int n_band = min(S->n_band, S->max_band);
     const double reach = S->reach;
     double *nd = s_nodes[wl], *cf = s_coef[wl], *bx = s_box[wl];
+    // the node gather (band_elem -> conn -> xyz: three dependent loads) of the NEXT element of this warp is issued
+    // before the current one is processed
+    double cx = 0.0, cy = 0.0, cz = 0.0;
+    if (warp < n_band && lane < 27) {
+        const int id = __ldg(conn + (size_t)band_elem[warp] * 27 + lane);
+        const double *p = xyz + (size_t)id * 3;
+        cx = __ldg(p); cy = __ldg(p + 1); cz = __ldg(p + 2);
+    }
     for (int b = warp; b < n_band; b += nwarps) {
-        const int e = band_elem[b];
-        if (lane < 27) {
-            const int id = __ldg(conn + (size_t)e * 27 + lane);
+        if (lane < 27) { nd[lane * 3 + 0] = cx; nd[lane * 3 + 1] = cy; nd[lane * 3 + 2] = cz; }
+        if (b + nwarps < n_band && lane < 27) {
+            const int id = __ldg(conn + (size_t)band_elem[b + nwarps] * 27 + lane);
             const double *p = xyz + (size_t)id * 3;
-            nd[lane * 3 + 0] = __ldg(p); nd[lane * 3 + 1] = __ldg(p + 1); nd[lane * 3 + 2] = __ldg(p + 2);
+            cx = __ldg(p); cy = __ldg(p + 1); cz = __ldg(p + 2);
         }
         __syncwarp();
         if (lane < 18) {
@@ -188,18 +196,22 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
         __syncwarp();
         for (int i = lane; i < 6 * 28; i += 32) ecoef[(size_t)b * (6 * 28) + i] = cf[i];
         for (int i = lane; i < 36; i += 32) pbox[(size_t)b * 36 + i] = bx[i];
-        // centre-centre distances of every (pair, patch): attained => upper bound; the smallest seeds Newton
+        // centre-centre distances of every (pair, patch): attained => upper bound; the smallest seeds Newton.
+        // A lane per pair (its face centre is loaded once), the 6 patch centres come from shared memory.
         const long long p0 = band_start[b];
-        const int total = band_cnt[b] * 6;
+        const int npair = band_cnt[b];
         unsigned long long key = ~0ull;
-        for (int t = lane; t < total; t += 32) {
-            const int pl = t / 6, k = t - pl * 6;
+        for (int pl = lane; pl < npair; pl += 32) {
             const int f = __ldg(pair_face + p0 + pl);
             const double *AQ = fcoef + (size_t)f * 28;
-            const double dx = cf[k * 28] - __ldg(AQ), dy = cf[k * 28 + 9] - __ldg(AQ + 9), dz = cf[k * 28 + 18] - __ldg(AQ + 18);
-            const double d2 = dx * dx + dy * dy + dz * dz;           // (squared: one sqrt per element, below)
-            const unsigned long long kk = (d2u(d2) & ~0xfffffull) | (unsigned long long)min(t, 0xfffff);
-            key = kk < key ? kk : key;
+            const double qx = __ldg(AQ), qy = __ldg(AQ + 9), qz = __ldg(AQ + 18);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+                const double dx = cf[k * 28] - qx, dy = cf[k * 28 + 9] - qy, dz = cf[k * 28 + 18] - qz;
+                const double d2 = dx * dx + dy * dy + dz * dz;           // (squared: one sqrt per element, below)
+                const unsigned long long kk = (d2u(d2) & ~0xfffffull) | (unsigned long long)min(pl * 6 + k, 0xfffff);
+                key = kk < key ? kk : key;
+            }
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, key, o); key = v < key ? v : key; }
