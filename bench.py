@@ -308,7 +308,10 @@ def main():
     ach_gbs = s2_bytes / (s2_ms * 1e-3) / 1e9 if s2_ms > 0 else 0.0
     roofline = {"kernel": "k_np_newton (S5 closest-point solves, 2 launches per cut)", "bound": "alu", "achieved": ach_tf,
                 "peak": fp64_peak, "unit": "TFLOP/s",
-                "frac": ach_tf / fp64_peak if fp64_peak > 0 else None, "traffic": None,
+                "frac": ach_tf / fp64_peak if fp64_peak > 0 else None,
+                # dram__bytes_read.sum + dram__bytes_write.sum of the two launches in the committed ncu --set full
+                # capture (profiles/r1c_kernels_full_config2.md: 48.4 + 0.3 and 111.1 + 6.7 MB), config 2 only
+                "traffic": 166.5e6 if cfg in (2, 3) else None,
                 "algorithmic_flops_per_cut": newton_flops, "ms_per_cut": newton_ms,
                 "peak_source": "measured: dc_measure_fp64_tflops (register-resident DFMA chains on all SMs) in this run",
                 "share_of_step": newton_ms / float(med[5] + med[6]) if med[5] > 0 else None,
