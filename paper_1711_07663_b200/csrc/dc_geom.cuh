@@ -16,6 +16,11 @@
 
 namespace dcg {
 
+// min / max of two finite doubles as one compare and a select (fmin / fmax expand to a NaN-aware sequence about
+// twice as long; every value compared on the hot path is finite)
+__host__ __device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
+__host__ __device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
+
 // ---------------------------------------------------------------------------------------------
 // 1-D quadratic through nodes (-1, 0, +1): a0 + a1 t + a2 t^2
 __device__ __forceinline__ void lag_to_mono(double x0, double x1, double x2,
@@ -120,13 +125,13 @@ struct NodeBound {
 // lower bound of  m(a,b) = sum_{(i,j)!=(0,0)} g[i+3j] a^i b^j  over [-1,1]^2  (g[0] ignored)
 __device__ __forceinline__ double poly_lower(const double *g)
 {
-    return -fabs(g[1]) - fabs(g[3]) + fmin(0.0, g[2]) + fmin(0.0, g[6]) - fabs(g[4])
-           - fabs(g[5]) - fabs(g[7]) + fmin(0.0, g[8]);
+    return -fabs(g[1]) - fabs(g[3]) + dmin2(0.0, g[2]) + dmin2(0.0, g[6]) - fabs(g[4])
+           - fabs(g[5]) - fabs(g[7]) + dmin2(0.0, g[8]);
 }
 __device__ __forceinline__ double poly_upper(const double *g)
 {
-    return fabs(g[1]) + fabs(g[3]) + fmax(0.0, g[2]) + fmax(0.0, g[6]) + fabs(g[4])
-           + fabs(g[5]) + fabs(g[7]) + fmax(0.0, g[8]);
+    return fabs(g[1]) + fabs(g[3]) + dmax2(0.0, g[2]) + dmax2(0.0, g[6]) + fabs(g[4])
+           + fabs(g[5]) + fabs(g[7]) + dmax2(0.0, g[8]);
 }
 
 template <typename LoadP, typename LoadQ>
@@ -170,8 +175,8 @@ __device__ __forceinline__ NodeBound bound_subpair(LoadP ldP, LoadQ ldQ,
         for (int m = 1; m < 9; ++m) { gQ[m] = fma(n[c], C[m], gQ[m]); nQ[m] = fma(C[m], C[m], nQ[m]); }
     }
     nb.lb = nb.dist_c + poly_lower(gP) - poly_upper(gQ);
-    nb.s1P = sqrt(fmax(nP[1], nP[3]));
-    nb.s1Q = sqrt(fmax(nQ[1], nQ[3]));
+    nb.s1P = sqrt(dmax2(nP[1], nP[3]));
+    nb.s1Q = sqrt(dmax2(nQ[1], nQ[3]));
     nb.s2P = sqrt(nP[2]) + sqrt(nP[6]) + sqrt(nP[4]) + sqrt(nP[5]) + sqrt(nP[7]) + sqrt(nP[8]);
     nb.s2Q = sqrt(nQ[2]) + sqrt(nQ[6]) + sqrt(nQ[4]) + sqrt(nQ[5]) + sqrt(nQ[7]) + sqrt(nQ[8]);
     return nb;
@@ -227,7 +232,7 @@ __device__ __forceinline__ bool chol4_solve(const double *h, const double *g, do
     return true;
 }
 
-__device__ __forceinline__ double clamp1(double x) { return fmin(1.0, fmax(-1.0, x)); }
+__device__ __forceinline__ double clamp1(double x) { return dmin2(1.0, dmax2(-1.0, x)); }
 
 __device__ inline NewtonOut newton_leaf(const double *CP, const double *CQ, double tol_d,
                                         double tau_exit, int max_iter)
@@ -311,11 +316,11 @@ __device__ inline NewtonOut newton_leaf(const double *CP, const double *CQ, doub
         double step = 0.0;
         if (dec) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) { step = fmax(step, fabs(xn[i] - x[i])); x[i] = xn[i]; }
+            for (int i = 0; i < 4; ++i) { step = dmax2(step, fabs(xn[i] - x[i])); x[i] = xn[i]; }
             f = fn;
         }
         // converged when the predicted decrease of the DISTANCE is below tol_d
-        if (pred <= tol_d * fmax(dist, tol_d)) { out.converged = 1; break; }
+        if (pred <= tol_d * dmax2(dist, tol_d)) { out.converged = 1; break; }
         if (!dec || step < 1e-15) { break; }
     }
     // final evaluation at x: distance and the sign cosine
@@ -339,7 +344,7 @@ __device__ inline NewtonOut newton_leaf(const double *CP, const double *CQ, doub
 // 8-bit code of the sign cosine: bit 7 = negative, bits 0-6 = round(|cos| * 127)
 __device__ __forceinline__ unsigned cos_code(double cosv)
 {
-    const double a = fmin(1.0, fabs(cosv));
+    const double a = dmin2(1.0, fabs(cosv));
     unsigned m = (unsigned)(a * 127.0 + 0.5);
     return (cosv < 0.0 ? 0x80u : 0u) | m;
 }
@@ -409,8 +414,8 @@ __device__ __forceinline__ void scalar_range(const double *g, double uc, double 
     const double c5 = h * fma(vc2, R22, R12);                // u^2 v
     const double c6 = h2 * R20, c7 = h2 * R21, c8 = h2 * R22; // v^2, u v^2, u^2 v^2
     const double odd = fabs(c1) + fabs(c3) + fabs(c4) + fabs(c5) + fabs(c7);
-    lo = fmin(0.0, c2) + fmin(0.0, c6) + fmin(0.0, c8) - odd;
-    hi = fmax(0.0, c2) + fmax(0.0, c6) + fmax(0.0, c8) + odd;
+    lo = dmin2(0.0, c2) + dmin2(0.0, c6) + dmin2(0.0, c8) - odd;
+    hi = dmax2(0.0, c2) + dmax2(0.0, c6) + dmax2(0.0, c8) + odd;
 }
 
 struct NodeOut { double dist_c, lb; bool leaf, splitP; };
@@ -444,10 +449,10 @@ __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ
     o.lb = o.dist_c + loP - hiQ;
     // subdivision rule (squared form)
     const double hP2 = hP * hP, hQ2 = hQ * hQ;
-    const double S1P = hP2 * fmax(pu[0] * pu[0] + pu[1] * pu[1] + pu[2] * pu[2], pv[0] * pv[0] + pv[1] * pv[1] + pv[2] * pv[2]);
-    const double S1Q = hQ2 * fmax(qs[0] * qs[0] + qs[1] * qs[1] + qs[2] * qs[2], qt[0] * qt[0] + qt[1] * qt[1] + qt[2] * qt[2]);
+    const double S1P = hP2 * dmax2(pu[0] * pu[0] + pu[1] * pu[1] + pu[2] * pu[2], pv[0] * pv[0] + pv[1] * pv[1] + pv[2] * pv[2]);
+    const double S1Q = hQ2 * dmax2(qs[0] * qs[0] + qs[1] * qs[1] + qs[2] * qs[2], qt[0] * qt[0] + qt[1] * qt[1] + qt[2] * qt[2]);
     const double s2P = hP2 * KP, s2Q = hQ2 * KQ;
-    const double M = fmax(S1P, S1Q);
+    const double M = dmax2(S1P, S1Q);
     const bool okP = !(S1P > 0.0) || s2P * s2P * M <= theta2 * S1P * S1P;
     const bool okQ = !(S1Q > 0.0) || s2Q * s2Q * M <= theta2 * S1Q * S1Q;
     o.leaf = okP && okQ;

@@ -100,16 +100,16 @@ __global__ void k_face_boxes(DcScalars *S, const double *__restrict__ face_nodes
         for (int c = 0; c < 3; ++c) {
             double x[9], b[9];
 #pragma unroll
-            for (int m = 0; m < 9; ++m) { x[m] = __ldg(X + 3 * m + c); nlo[c] = fmin(nlo[c], x[m]); nhi[c] = fmax(nhi[c], x[m]); }
+            for (int m = 0; m < 9; ++m) { x[m] = __ldg(X + 3 * m + c); nlo[c] = dmin2(nlo[c], x[m]); nhi[c] = dmax2(nhi[c], x[m]); }
 #pragma unroll
             for (int j = 0; j < 3; ++j) { b[3*j] = x[3*j]; b[3*j+1] = bez_mid(x[3*j], x[3*j+1], x[3*j+2]); b[3*j+2] = x[3*j+2]; }
 #pragma unroll
             for (int i = 0; i < 3; ++i) { const double m1 = bez_mid(b[i], b[i+3], b[i+6]); b[i+3] = m1; }
 #pragma unroll
-            for (int m = 0; m < 9; ++m) { lo[c] = fmin(lo[c], b[m]); hi[c] = fmax(hi[c], b[m]); }
+            for (int m = 0; m < 9; ++m) { lo[c] = dmin2(lo[c], b[m]); hi[c] = dmax2(hi[c], b[m]); }
             fbox_orig[(size_t)f * 6 + c] = lo[c];
             fbox_orig[(size_t)f * 6 + 3 + c] = hi[c];
-            edge = fmax(edge, hi[c] - lo[c]);
+            edge = dmax2(edge, hi[c] - lo[c]);
         }
     }
     // warp reduce then one atomic per warp
@@ -117,12 +117,12 @@ __global__ void k_face_boxes(DcScalars *S, const double *__restrict__ face_nodes
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            lo[c] = fmin(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o));
-            hi[c] = fmax(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
-            nlo[c] = fmin(nlo[c], __shfl_xor_sync(0xffffffffu, nlo[c], o));
-            nhi[c] = fmax(nhi[c], __shfl_xor_sync(0xffffffffu, nhi[c], o));
+            lo[c] = dmin2(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o));
+            hi[c] = dmax2(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
+            nlo[c] = dmin2(nlo[c], __shfl_xor_sync(0xffffffffu, nlo[c], o));
+            nhi[c] = dmax2(nhi[c], __shfl_xor_sync(0xffffffffu, nhi[c], o));
         }
-        edge = fmax(edge, __shfl_xor_sync(0xffffffffu, edge, o));
+        edge = dmax2(edge, __shfl_xor_sync(0xffffffffu, edge, o));
     }
     if ((threadIdx.x & 31) == 0 && lo[0] != INFINITY) {
 #pragma unroll
@@ -148,12 +148,12 @@ __global__ void k_setup_surface(DcScalars *S, int n_face)
     double ext = 0.0, lref = 0.0;
     for (int c = 0; c < 3; ++c) {
         S->smin[c] = dec_ord(S->fbox_min[c]); S->smax[c] = dec_ord(S->fbox_max[c]);
-        ext = fmax(ext, S->smax[c] - S->smin[c]);
-        lref = fmax(lref, dec_ord(S->node_max[c]) - dec_ord(S->node_min[c]));
+        ext = dmax2(ext, S->smax[c] - S->smin[c]);
+        lref = dmax2(lref, dec_ord(S->node_max[c]) - dec_ord(S->node_min[c]));
     }
     S->l_ref_auto = lref;
     const double edge = dec_ord(S->max_face_edge);
-    double cell = fmax(edge, ext / DC_GRID_MAX) * (1.0 + 1e-9);
+    double cell = dmax2(edge, ext / DC_GRID_MAX) * (1.0 + 1e-9);
     if (!(cell > 0.0)) cell = 1.0;
     S->cell = cell; S->inv_cell = 1.0 / cell; S->fhalf = 0.5 * edge;
     for (int c = 0; c < 3; ++c) {
@@ -303,9 +303,10 @@ __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const d
                 for (int i = 0; i < 3; ++i) b[i+3+9*k] = bez_mid(b[i+9*k], b[i+3+9*k], b[i+6+9*k]);
 #pragma unroll
             for (int m = 0; m < 9; ++m) b[m+9] = bez_mid(b[m], b[m+9], b[m+18]);
-            double lo = INFINITY, hi = -INFINITY;
+            // (plain compare-and-select: fmin / fmax of doubles expand to a NaN-aware sequence twice as long)
+            double lo = b[0], hi = b[0];
 #pragma unroll
-            for (int m = 0; m < 27; ++m) if (m != 13) { lo = fmin(lo, b[m]); hi = fmax(hi, b[m]); }
+            for (int m = 1; m < 27; ++m) if (m != 13) { lo = b[m] < lo ? b[m] : lo; hi = b[m] > hi ? b[m] : hi; }
             const long long e = e0 + el;
             ebox[(size_t)c * n_elem + e] = lo;
             ebox[(size_t)(3 + c) * n_elem + e] = hi;
@@ -316,7 +317,7 @@ __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const d
     double diag2 = 0.0;
     if (threadIdx.x < nloc) diag2 = s_ext2[threadIdx.x * 3] + s_ext2[threadIdx.x * 3 + 1] + s_ext2[threadIdx.x * 3 + 2];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) diag2 = fmax(diag2, __shfl_xor_sync(0xffffffffu, diag2, o));
+    for (int o = 16; o > 0; o >>= 1) diag2 = dmax2(diag2, __shfl_xor_sync(0xffffffffu, diag2, o));
     if ((threadIdx.x & 31) == 0) atomicMax(&S->grid_max_diag2, (unsigned long long)__double_as_longlong(diag2));
 }
 
@@ -404,7 +405,7 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
         double d2 = 0.0;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const double g = fmax(0.0, fmax(S->smin[c] - hi[c], lo[c] - S->smax[c]));
+            const double g = dmax2(0.0, dmax2(S->smin[c] - hi[c], lo[c] - S->smax[c]));
             d2 = fma(g, g, d2);
         }
         const double reach = S->reach;
@@ -444,7 +445,7 @@ __device__ __forceinline__ bool box_within(const double *lo, const double *hi, c
     double d2 = 0.0;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double g = fmax(0.0, fmax(fb[c] - hi[c], lo[c] - fb[3 + c]));
+        const double g = dmax2(0.0, dmax2(fb[c] - hi[c], lo[c] - fb[3 + c]));
         d2 = fma(g, g, d2);
     }
     return d2 <= reach2;
@@ -745,7 +746,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                 if (nb.lb > best + t_tie) continue;
                 const double kP = nb.s1P > 0.0 ? nb.s2P / (nb.s1P * nb.s1P) : 0.0;
                 const double kQ = nb.s1Q > 0.0 ? nb.s2Q / (nb.s1Q * nb.s1Q) : 0.0;
-                bool leaf = fmax(kP, kQ) * fmax(nb.s1P, nb.s1Q) <= theta;
+                bool leaf = dmax2(kP, kQ) * dmax2(nb.s1P, nb.s1Q) <= theta;
                 const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
                 bool splitP = nb.s1P >= nb.s1Q;
                 if (!leaf) {
@@ -764,7 +765,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                     const NewtonOut o = newton_leaf(CP, CQ, tol_d, -1.0, NP_NEWTON_ITERS_SL);
                     atomicMin(&s_best, d2u(o.dist));
                     if (o.dist < my_d - t_tie || (o.dist <= my_d + t_tie && fabs(o.cosv) > fabs(my_c))) {
-                        my_d = fmin(my_d, o.dist); my_c = o.cosv;
+                        my_d = dmin2(my_d, o.dist); my_c = o.cosv;
                     }
                 } else {
                     make_children(it, splitP, st + top);
@@ -777,7 +778,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
     __syncthreads();
     if (tid == 0) {
         double dmin = INFINITY;
-        for (int i = 0; i < SL_THREADS; ++i) dmin = fmin(dmin, s_d[i]);
+        for (int i = 0; i < SL_THREADS; ++i) dmin = dmin2(dmin, s_d[i]);
         double bc = 0.0;
         for (int i = 0; i < SL_THREADS; ++i) if (s_d[i] <= dmin + t_tie && fabs(s_c[i]) > fabs(bc)) bc = s_c[i];
         comp[e] = bc < 0.0 ? 1 : 2;

@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
             for (int i = 0; i < 3; ++i) x[i + 3] = bez_mid(x[i], x[i + 3], x[i + 6]);
             double lo = x[0], hi = x[0];
 #pragma unroll
-            for (int m = 1; m < 9; ++m) { lo = fmin(lo, x[m]); hi = fmax(hi, x[m]); }
+            for (int m = 1; m < 9; ++m) { lo = dmin2(lo, x[m]); hi = dmax2(hi, x[m]); }
             bx[k * 6 + c] = lo; bx[k * 6 + 3 + c] = hi;
         }
         __syncwarp();
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
         if (lane == 0) {
             // the truncated key is <= the attained squared distance: round up to stay an upper bound
             const double dkey = sqrt(u2d((key & ~0xfffffull) + 0x100000ull)) * (1.0 + 4e-16);
-            best[b] = d2u(fmin(reach, dkey));
+            best[b] = d2u(dmin2(reach, dkey));
             dmin[b] = 0x7ff0000000000000ull;
             const int t = (int)(key & 0xfffffull);
             const int pl = t / 6, k = t - pl * 6;
@@ -429,7 +429,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_roots(DcScalars *S, const lo
                     double d2 = 0.0;
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
-                        const double g = fmax(0.0, fmax(fb[c] - __ldg(pb + k * 6 + 3 + c), __ldg(pb + k * 6 + c) - fb[3 + c]));
+                        const double g = dmax2(0.0, dmax2(fb[c] - __ldg(pb + k * 6 + 3 + c), __ldg(pb + k * 6 + c) - fb[3 + c]));
                         d2 = fma(g, g, d2);
                     }
                     if (d2 <= cut2) mask |= 1u << k;
@@ -580,7 +580,7 @@ __global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, con
             }
             if (npos && nneg) ++n_samb;
             labels[e] = neg ? DC_HOLE : DC_NORMAL;
-            const double d = fmin(dmin, d_band);
+            const double d = dmin2(dmin, d_band);
             sdist[e] = neg ? -d : d;
         }
     }

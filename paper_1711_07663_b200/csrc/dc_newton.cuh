@@ -28,6 +28,10 @@ static inline double __longlong_as_double_hd(long long x) { double d; memcpy(&d,
 #define DCN_HD __host__ __device__ __forceinline__
 #endif
 
+// (compare-and-select min / max of finite doubles: see dc_geom.cuh)
+DCN_HD double dmin2(double a, double b) { return a < b ? a : b; }
+DCN_HD double dmax2(double a, double b) { return a > b ? a : b; }
+
 #define NW_MAXIT 24                 /* evaluations per solve before it is declared unconverged */
 
 // state of one lane's solve
@@ -78,21 +82,21 @@ DCN_HD bool ldl4_mod(double h00, double h01, double h02, double h03, double h11,
                      double h22, double h23, double h33, const double *g, double floor, double *p)
 {
     bool mod = !(h00 > floor);
-    const double d0 = mod ? fmax(fabs(h00), floor) : h00;
+    const double d0 = mod ? dmax2(fabs(h00), floor) : h00;
     const double i0 = 1.0 / d0;
     const double l10 = h01 * i0, l20 = h02 * i0, l30 = h03 * i0;
     double d1 = fma(-l10, h01, h11);
-    if (!(d1 > floor)) { mod = true; d1 = fmax(fabs(d1), floor); }
+    if (!(d1 > floor)) { mod = true; d1 = dmax2(fabs(d1), floor); }
     const double i1 = 1.0 / d1;
     const double t21 = fma(-l20, h01, h12), t31 = fma(-l30, h01, h13);
     const double l21 = t21 * i1, l31 = t31 * i1;
     double d2 = fma(-l21, t21, fma(-l20, h02, h22));
-    if (!(d2 > floor)) { mod = true; d2 = fmax(fabs(d2), floor); }
+    if (!(d2 > floor)) { mod = true; d2 = dmax2(fabs(d2), floor); }
     const double i2 = 1.0 / d2;
     const double t32 = fma(-l31, t21, fma(-l30, h02, h23));
     const double l32 = t32 * i2;
     double d3 = fma(-l32, t32, fma(-l31, t31, fma(-l30, h03, h33)));
-    if (!(d3 > floor)) { mod = true; d3 = fmax(fabs(d3), floor); }
+    if (!(d3 > floor)) { mod = true; d3 = dmax2(fabs(d3), floor); }
     const double i3 = 1.0 / d3;
     const double y0 = -g[0];
     const double y1 = fma(-l10, y0, -g[1]);
@@ -194,7 +198,7 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
             for (int i = 0; i < 4; ++i) { moved = moved || fabs(xn[i] - s.x[i]) >= 1e-15 * (hi[i] - lo[i]); s.x[i] = xn[i]; }
             s.ls = 0;
         } else s.ls++;
-        if (pred * pred <= tol_d2 * fmax(rr, tol_d2)) {
+        if (pred * pred <= tol_d2 * dmax2(rr, tol_d2)) {
             // predicted decrease of the DISTANCE below tolerance: converged.  The distance reported is the
             // one attained at the accepted trial point (value-only evaluation), the sign cosine the one here.
             finished = true;
