@@ -32,6 +32,21 @@ static inline double __longlong_as_double_hd(long long x) { double d; memcpy(&d,
 DCN_HD double dmin2(double a, double b) { return a < b ? a : b; }
 DCN_HD double dmax2(double a, double b) { return a > b ? a : b; }
 
+// reciprocal of a normal-range double: hardware seed (20 bits) + two Newton steps, ~1 ulp, no slow path (the divide
+// the compiler emits for 1.0 / x carries a range check and a call; the pivots it is used on are >= floor > 0)
+DCN_HD double rcp_fast(double x)
+{
+#ifdef __CUDA_ARCH__
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = fma(fma(-x, y, 1.0), y, y);
+    y = fma(fma(-x, y, 1.0), y, y);
+    return y;
+#else
+    return 1.0 / x;
+#endif
+}
+
 #define NW_MAXIT 24                 /* evaluations per solve before it is declared unconverged */
 
 // state of one lane's solve
@@ -83,21 +98,21 @@ DCN_HD bool ldl4_mod(double h00, double h01, double h02, double h03, double h11,
 {
     bool mod = !(h00 > floor);
     const double d0 = mod ? dmax2(fabs(h00), floor) : h00;
-    const double i0 = 1.0 / d0;
+    const double i0 = rcp_fast(d0);
     const double l10 = h01 * i0, l20 = h02 * i0, l30 = h03 * i0;
     double d1 = fma(-l10, h01, h11);
     if (!(d1 > floor)) { mod = true; d1 = dmax2(fabs(d1), floor); }
-    const double i1 = 1.0 / d1;
+    const double i1 = rcp_fast(d1);
     const double t21 = fma(-l20, h01, h12), t31 = fma(-l30, h01, h13);
     const double l21 = t21 * i1, l31 = t31 * i1;
     double d2 = fma(-l21, t21, fma(-l20, h02, h22));
     if (!(d2 > floor)) { mod = true; d2 = dmax2(fabs(d2), floor); }
-    const double i2 = 1.0 / d2;
+    const double i2 = rcp_fast(d2);
     const double t32 = fma(-l31, t21, fma(-l30, h02, h23));
     const double l32 = t32 * i2;
     double d3 = fma(-l32, t32, fma(-l31, t31, fma(-l30, h03, h33)));
     if (!(d3 > floor)) { mod = true; d3 = dmax2(fabs(d3), floor); }
-    const double i3 = 1.0 / d3;
+    const double i3 = rcp_fast(d3);
     const double y0 = -g[0];
     const double y1 = fma(-l10, y0, -g[1]);
     const double y2 = fma(-l21, y1, fma(-l20, y0, -g[2]));
@@ -214,9 +229,14 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
         const double ny = Qs[2] * Qt[0] - Qs[0] * Qt[2];
         const double nz = Qs[0] * Qt[1] - Qs[1] * Qt[0];
         const double nn = nx * nx + ny * ny + nz * nz;
-        const double den = sqrt(rr * nn);
+        const double den2 = rr * nn;
         R.dist = sqrt(rr_out);
-        R.cosv = den > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) / den : 0.0;
+        // (the cosine only decides a sign and a 7-bit magnitude: reciprocal square root instead of sqrt and divide)
+#ifdef __CUDA_ARCH__
+        R.cosv = den2 > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) * rsqrt(den2) : 0.0;
+#else
+        R.cosv = den2 > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) / sqrt(den2) : 0.0;
+#endif
         R.converged = converged;
     }
     return finished;
