@@ -2,12 +2,11 @@
 //
 // A biquadratic patch (9-node Lagrange quad, Eq. 1 L241 with K = 2) is held in the
 // MONOMIAL basis  P(u,v) = sum_{i,j<=2} A[i+3j] u^i v^j,  (u,v) in [-1,1]^2, one 9-vector per
-// coordinate.  Restricting it to a dyadic sub-rectangle (centre (uc,vc), half-widths (hu,hv))
-// and re-centring gives local coefficients C with  P = sum C[i+3j] a^i b^j, (a,b) in [-1,1]^2:
-// this one representation yields the point at the centre (an attained distance, hence an upper
-// bound), range bounds of any projection n.P (the lower bound of the branch and bound) and all
-// derivatives the projected Newton solve needs (the two-patch generalisation of Eq. 3-5,
-// L256-L270, with the paper's clamp to the reference box, L272-L278).
+// coordinate, plus one constant K bounding its higher-order part.  A sub-patch is a dyadic
+// sub-rectangle (centre (uc,vc), half-width h) of its root patch and is never re-centred: the
+// branch-and-bound node (bound_node, below) evaluates the centre (an attained distance, hence an
+// upper bound) and the range of the projections n.P, n.Q on the sub-rectangles (the lower bound)
+// straight from the root coefficients; the projected Newton solve lives in dc_newton.cuh.
 //
 // No code is shared with oracle/ (which uses Bezier nets and triangle-triangle distances).
 #pragma once
@@ -43,57 +42,6 @@ __device__ __forceinline__ void nodes_to_mono9(const double *X, double *A)
         lag_to_mono(T[i], T[i + 3], T[i + 6], A[i], A[i + 3], A[i + 6]);
 }
 
-// Re-centre one coordinate: A[9] on [-1,1]^2 -> C[9] on the sub-rectangle (uc,vc,hu,hv).
-__device__ __forceinline__ void recentre9(const double *A, double uc, double vc, double hu, double hv,
-                                          double *C)
-{
-    double R[9];
-    const double hu2 = hu * hu, hv2 = hv * hv;
-#pragma unroll
-    for (int j = 0; j < 3; ++j) {
-        const double a0 = A[3 * j], a1 = A[3 * j + 1], a2 = A[3 * j + 2];
-        R[3 * j]     = fma(uc, fma(uc, a2, a1), a0);
-        R[3 * j + 1] = hu * fma(2.0 * uc, a2, a1);
-        R[3 * j + 2] = hu2 * a2;
-    }
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const double r0 = R[i], r1 = R[i + 3], r2 = R[i + 6];
-        C[i]     = fma(vc, fma(vc, r2, r1), r0);
-        C[i + 3] = hv * fma(2.0 * vc, r2, r1);
-        C[i + 6] = hv2 * r2;
-    }
-}
-
-// value of one coordinate at (u,v)
-__device__ __forceinline__ double eval9(const double *A, double u, double v)
-{
-    const double r0 = fma(u, fma(u, A[2], A[1]), A[0]);
-    const double r1 = fma(u, fma(u, A[5], A[4]), A[3]);
-    const double r2 = fma(u, fma(u, A[8], A[7]), A[6]);
-    return fma(v, fma(v, r2, r1), r0);
-}
-
-// value and all derivatives up to second order of one coordinate at (a,b)
-struct Jet { double p, pa, pb, paa, pab, pbb; };
-__device__ __forceinline__ Jet jet9(const double *C, double a, double b)
-{
-    const double r0 = fma(a, fma(a, C[2], C[1]), C[0]);
-    const double r1 = fma(a, fma(a, C[5], C[4]), C[3]);
-    const double r2 = fma(a, fma(a, C[8], C[7]), C[6]);
-    const double d0 = fma(2.0 * a, C[2], C[1]);
-    const double d1 = fma(2.0 * a, C[5], C[4]);
-    const double d2 = fma(2.0 * a, C[8], C[7]);
-    Jet J;
-    J.p   = fma(b, fma(b, r2, r1), r0);
-    J.pb  = fma(2.0 * b, r2, r1);
-    J.pbb = 2.0 * r2;
-    J.pa  = fma(b, fma(b, d2, d1), d0);
-    J.pab = fma(2.0 * b, d2, d1);
-    J.paa = 2.0 * fma(b, fma(b, C[8], C[5]), C[2]);
-    return J;
-}
-
 // ---------------------------------------------------------------------------------------------
 // ordered-uint encoding of doubles for atomicMin/atomicMax
 __device__ __forceinline__ unsigned long long enc_ord(double x)
@@ -109,236 +57,6 @@ __device__ __host__ __forceinline__ double dec_ord(unsigned long long e)
 #else
     double d; memcpy(&d, &b, 8); return d;
 #endif
-}
-
-// ---------------------------------------------------------------------------------------------
-// Sub-pair bound.  Inputs: root monomial coefficients AP[27], AQ[27] laid out [coord][9]
-// (coord-major), and the two dyadic sub-rectangles.  Outputs everything the branch and bound
-// needs to decide prune / split / leaf.
-struct NodeBound {
-    double dist_c;   // |P_c - Q_c|: attained by real points -> valid upper bound
-    double lb;       // slab lower bound of the distance over the sub-pair
-    double s1P, s2P; // first-order size (max |C10|,|C01|) and higher-order radius of P's sub-patch
-    double s1Q, s2Q;
-};
-
-// lower bound of  m(a,b) = sum_{(i,j)!=(0,0)} g[i+3j] a^i b^j  over [-1,1]^2  (g[0] ignored)
-__device__ __forceinline__ double poly_lower(const double *g)
-{
-    return -fabs(g[1]) - fabs(g[3]) + dmin2(0.0, g[2]) + dmin2(0.0, g[6]) - fabs(g[4])
-           - fabs(g[5]) - fabs(g[7]) + dmin2(0.0, g[8]);
-}
-__device__ __forceinline__ double poly_upper(const double *g)
-{
-    return fabs(g[1]) + fabs(g[3]) + dmax2(0.0, g[2]) + dmax2(0.0, g[6]) + fabs(g[4])
-           + fabs(g[5]) + fabs(g[7]) + dmax2(0.0, g[8]);
-}
-
-template <typename LoadP, typename LoadQ>
-__device__ __forceinline__ NodeBound bound_subpair(LoadP ldP, LoadQ ldQ,
-                                                   double uc, double vc, double hP,
-                                                   double sc, double tc, double hQ)
-{
-    // pass 1: centres -> r, n
-    double r[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        double A[9];
-#pragma unroll
-        for (int m = 0; m < 9; ++m) A[m] = ldP(c * 9 + m);
-        const double p = eval9(A, uc, vc);
-#pragma unroll
-        for (int m = 0; m < 9; ++m) A[m] = ldQ(c * 9 + m);
-        r[c] = p - eval9(A, sc, tc);
-    }
-    NodeBound nb;
-    const double d2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
-    nb.dist_c = sqrt(d2);
-    const double inv = nb.dist_c > 0.0 ? 1.0 / nb.dist_c : 0.0;
-    const double n[3] = { r[0] * inv, r[1] * inv, r[2] * inv };
-    // pass 2: projections of the re-centred coefficients on n, and coefficient norms
-    double gP[9], gQ[9], nP[9], nQ[9];
-#pragma unroll
-    for (int m = 0; m < 9; ++m) { gP[m] = gQ[m] = nP[m] = nQ[m] = 0.0; }
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        double A[9], C[9];
-#pragma unroll
-        for (int m = 0; m < 9; ++m) A[m] = ldP(c * 9 + m);
-        recentre9(A, uc, vc, hP, hP, C);
-#pragma unroll
-        for (int m = 1; m < 9; ++m) { gP[m] = fma(n[c], C[m], gP[m]); nP[m] = fma(C[m], C[m], nP[m]); }
-#pragma unroll
-        for (int m = 0; m < 9; ++m) A[m] = ldQ(c * 9 + m);
-        recentre9(A, sc, tc, hQ, hQ, C);
-#pragma unroll
-        for (int m = 1; m < 9; ++m) { gQ[m] = fma(n[c], C[m], gQ[m]); nQ[m] = fma(C[m], C[m], nQ[m]); }
-    }
-    nb.lb = nb.dist_c + poly_lower(gP) - poly_upper(gQ);
-    nb.s1P = sqrt(dmax2(nP[1], nP[3]));
-    nb.s1Q = sqrt(dmax2(nQ[1], nQ[3]));
-    nb.s2P = sqrt(nP[2]) + sqrt(nP[6]) + sqrt(nP[4]) + sqrt(nP[5]) + sqrt(nP[7]) + sqrt(nP[8]);
-    nb.s2Q = sqrt(nQ[2]) + sqrt(nQ[6]) + sqrt(nQ[4]) + sqrt(nQ[5]) + sqrt(nQ[7]) + sqrt(nQ[8]);
-    return nb;
-}
-
-// ---------------------------------------------------------------------------------------------
-// Projected Newton on f(a,b,c,d) = 1/2 |P(a,b) - Q(c,d)|^2 over the LOCAL box [-1,1]^4 of a leaf
-// (the leaf's own sub-rectangles).  CP, CQ: local coefficients [coord][9] (27 each).
-struct NewtonOut {
-    double dist;      // attained distance at the final iterate
-    double cosv;      // (r . n)/(|r||n|), n = Q_c x Q_d (same orientation as Q_s x Q_t)
-    int iters;
-    int converged;    // 1: predicted decrease below tolerance; 0: cap hit / stalled
-};
-
-__device__ __forceinline__ double f_only(const double *CP, const double *CQ, const double *x)
-{
-    double f = 0.0;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const double r = eval9(CP + 9 * c, x[0], x[1]) - eval9(CQ + 9 * c, x[2], x[3]);
-        f = fma(r, r, f);
-    }
-    return 0.5 * f;
-}
-
-// Cholesky solve of the 4x4 SPD system H p = -g (H given by its upper triangle h[10] in row
-// order 00 01 02 03 11 12 13 22 23 33).  Returns false if not positive definite.
-__device__ __forceinline__ bool chol4_solve(const double *h, const double *g, double *p)
-{
-    double l00, l10, l20, l30, l11, l21, l31, l22, l32, l33;
-    if (!(h[0] > 0.0)) return false;
-    l00 = sqrt(h[0]); const double i00 = 1.0 / l00;
-    l10 = h[1] * i00; l20 = h[2] * i00; l30 = h[3] * i00;
-    double t = h[4] - l10 * l10; if (!(t > 0.0)) return false;
-    l11 = sqrt(t); const double i11 = 1.0 / l11;
-    l21 = (h[5] - l20 * l10) * i11; l31 = (h[6] - l30 * l10) * i11;
-    t = h[7] - l20 * l20 - l21 * l21; if (!(t > 0.0)) return false;
-    l22 = sqrt(t); const double i22 = 1.0 / l22;
-    l32 = (h[8] - l30 * l20 - l31 * l21) * i22;
-    t = h[9] - l30 * l30 - l31 * l31 - l32 * l32; if (!(t > 0.0)) return false;
-    l33 = sqrt(t); const double i33 = 1.0 / l33;
-    // forward: L y = -g
-    const double y0 = -g[0] * i00;
-    const double y1 = (-g[1] - l10 * y0) * i11;
-    const double y2 = (-g[2] - l20 * y0 - l21 * y1) * i22;
-    const double y3 = (-g[3] - l30 * y0 - l31 * y1 - l32 * y2) * i33;
-    // backward: L^T p = y
-    p[3] = y3 * i33;
-    p[2] = (y2 - l32 * p[3]) * i22;
-    p[1] = (y1 - l21 * p[2] - l31 * p[3]) * i11;
-    p[0] = (y0 - l10 * p[1] - l20 * p[2] - l30 * p[3]) * i00;
-    return true;
-}
-
-__device__ __forceinline__ double clamp1(double x) { return dmin2(1.0, dmax2(-1.0, x)); }
-
-__device__ inline NewtonOut newton_leaf(const double *CP, const double *CQ, double tol_d,
-                                        double tau_exit, int max_iter)
-{
-    double x[4] = { 0.0, 0.0, 0.0, 0.0 };
-    NewtonOut out; out.iters = 0; out.converged = 0;
-    double f = 0.0, r[3], Qc[3], Qd[3];
-    for (int it = 0; it < max_iter; ++it) {
-        out.iters = it + 1;
-        // jets
-        double Pa[3], Pb[3], Paa[3], Pab[3], Pbb[3], Qcc[3], Qcd[3], Qdd[3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const Jet JP = jet9(CP + 9 * c, x[0], x[1]);
-            const Jet JQ = jet9(CQ + 9 * c, x[2], x[3]);
-            r[c] = JP.p - JQ.p;
-            Pa[c] = JP.pa; Pb[c] = JP.pb; Paa[c] = JP.paa; Pab[c] = JP.pab; Pbb[c] = JP.pbb;
-            Qc[c] = JQ.pa; Qd[c] = JQ.pb; Qcc[c] = JQ.paa; Qcd[c] = JQ.pab; Qdd[c] = JQ.pbb;
-        }
-#define DOT(A, B) (A[0] * B[0] + A[1] * B[1] + A[2] * B[2])
-        f = 0.5 * DOT(r, r);
-        const double dist = sqrt(2.0 * f);
-        if (dist <= tau_exit) { out.converged = 1; break; }
-        double g[4] = { DOT(r, Pa), DOT(r, Pb), -DOT(r, Qc), -DOT(r, Qd) };
-        double h[10];
-        h[0] = DOT(Pa, Pa) + DOT(r, Paa);
-        h[1] = DOT(Pa, Pb) + DOT(r, Pab);
-        h[2] = -DOT(Pa, Qc);
-        h[3] = -DOT(Pa, Qd);
-        h[4] = DOT(Pb, Pb) + DOT(r, Pbb);
-        h[5] = -DOT(Pb, Qc);
-        h[6] = -DOT(Pb, Qd);
-        h[7] = DOT(Qc, Qc) - DOT(r, Qcc);
-        h[8] = DOT(Qc, Qd) - DOT(r, Qcd);
-        h[9] = DOT(Qd, Qd) - DOT(r, Qdd);
-        // active set: variables at a bound whose gradient pushes outward are held (L272-L278)
-        bool fixed[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-            fixed[i] = (x[i] <= -1.0 && g[i] > 0.0) || (x[i] >= 1.0 && g[i] < 0.0);
-        const int di[4] = { 0, 4, 7, 9 };
-        // decouple held variables
-        if (fixed[0]) { h[1] = h[2] = h[3] = 0.0; h[0] = 1.0; g[0] = 0.0; }
-        if (fixed[1]) { h[1] = h[5] = h[6] = 0.0; h[4] = 1.0; g[1] = 0.0; }
-        if (fixed[2]) { h[2] = h[5] = h[8] = 0.0; h[7] = 1.0; g[2] = 0.0; }
-        if (fixed[3]) { h[3] = h[6] = h[8] = 0.0; h[9] = 1.0; g[3] = 0.0; }
-        const double gg = g[0] * g[0] + g[1] * g[1] + g[2] * g[2] + g[3] * g[3];
-        if (gg == 0.0) { out.converged = 1; break; }
-        // Levenberg damping only if the (reduced) Hessian is not positive definite
-        double tr = 0.0;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) if (!fixed[i]) tr += fabs(h[di[i]]);
-        double p[4];
-        double lam = 0.0;
-        bool ok = false;
-        for (int tries = 0; tries < 6 && !ok; ++tries) {
-            double hd[10];
-#pragma unroll
-            for (int i = 0; i < 10; ++i) hd[i] = h[i];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) if (!fixed[i]) hd[di[i]] += lam;
-            ok = chol4_solve(hd, g, p);
-            lam = (lam == 0.0) ? 1e-6 * tr + 1e-300 : lam * 100.0;
-        }
-        if (!ok) { // steepest descent fallback, scaled by the trace
-            const double s = tr > 0.0 ? 1.0 / tr : 1.0;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) p[i] = -g[i] * s;
-        }
-        const double pred = -0.5 * (g[0] * p[0] + g[1] * p[1] + g[2] * p[2] + g[3] * p[3]);
-        // projected step with backtracking on f
-        double xn[4], fn = f, alpha = 1.0;
-        bool dec = false;
-        for (int ls = 0; ls < 6; ++ls) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) xn[i] = clamp1(fma(alpha, p[i], x[i]));
-            fn = f_only(CP, CQ, xn);
-            if (fn <= f) { dec = true; break; }
-            alpha *= 0.25;
-        }
-        double step = 0.0;
-        if (dec) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) { step = dmax2(step, fabs(xn[i] - x[i])); x[i] = xn[i]; }
-            f = fn;
-        }
-        // converged when the predicted decrease of the DISTANCE is below tol_d
-        if (pred <= tol_d * dmax2(dist, tol_d)) { out.converged = 1; break; }
-        if (!dec || step < 1e-15) { break; }
-    }
-    // final evaluation at x: distance and the sign cosine
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const Jet JP = jet9(CP + 9 * c, x[0], x[1]);
-        const Jet JQ = jet9(CQ + 9 * c, x[2], x[3]);
-        r[c] = JP.p - JQ.p; Qc[c] = JQ.pa; Qd[c] = JQ.pb;
-    }
-    const double nx = Qc[1] * Qd[2] - Qc[2] * Qd[1];
-    const double ny = Qc[2] * Qd[0] - Qc[0] * Qd[2];
-    const double nz = Qc[0] * Qd[1] - Qc[1] * Qd[0];
-    const double rr = DOT(r, r), nn = nx * nx + ny * ny + nz * nz;
-    out.dist = sqrt(rr);
-    const double den = sqrt(rr * nn);
-    out.cosv = den > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) / den : 0.0;
-#undef DOT
-    return out;
 }
 
 // 8-bit code of the sign cosine: bit 7 = negative, bits 0-6 = round(|cos| * 127)

@@ -554,12 +554,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
 }
 
 // ------------------------------------------------------------------------------------------
-// S5 + S6: narrow phase -> dc_narrow.cuh (wavefront kernels).  Item / item_box / make_children below
-// serve k_seedless only.
-#define NP_NEWTON_ITERS_SL 40
-struct __align__(16) Item { unsigned f, w1, w2, w3; };
-// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20      w3: is(12) | it(12)<<12
-
+// S5 + S6: narrow phase -> dc_narrow.cuh.
 __constant__ int c_face_node[6][9] = {
     { 0, 3, 6, 9, 12, 15, 18, 21, 24 },      // xi = -1 : (a,b) = (j,k)
     { 2, 5, 8, 11, 14, 17, 20, 23, 26 },     // xi = +1
@@ -568,36 +563,6 @@ __constant__ int c_face_node[6][9] = {
     { 0, 1, 2, 3, 4, 5, 6, 7, 8 },           // zeta = -1 : (a,b) = (i,j)
     { 18, 19, 20, 21, 22, 23, 24, 25, 26 },  // zeta = +1
 };
-
-__device__ __forceinline__ void item_box(const Item &it, double &uc, double &vc, double &hP,
-                                         double &sc, double &tc, double &hQ)
-{
-    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
-    const int iu = (it.w2 >> 8) & 0xfff, iv = (it.w2 >> 20) & 0xfff;
-    const int is = it.w3 & 0xfff, itt = (it.w3 >> 12) & 0xfff;
-    hP = __longlong_as_double((long long)(1023 - lP) << 52);
-    hQ = __longlong_as_double((long long)(1023 - lQ) << 52);
-    uc = fma((double)(2 * iu + 1), hP, -1.0); vc = fma((double)(2 * iv + 1), hP, -1.0);
-    sc = fma((double)(2 * is + 1), hQ, -1.0); tc = fma((double)(2 * itt + 1), hQ, -1.0);
-}
-
-__device__ __forceinline__ void make_children(const Item &it, bool splitP, Item *ch)
-{
-    const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
-    const int iu = (it.w2 >> 8) & 0xfff, iv = (it.w2 >> 20) & 0xfff;
-    const int is = it.w3 & 0xfff, itt = (it.w3 >> 12) & 0xfff;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        ch[c].f = it.f; ch[c].w1 = it.w1;
-        if (splitP) {
-            ch[c].w2 = (unsigned)(lP + 1) | ((unsigned)lQ << 4) | ((unsigned)(2 * iu + (c & 1)) << 8) | ((unsigned)(2 * iv + (c >> 1)) << 20);
-            ch[c].w3 = it.w3 & 0x00ffffffu;
-        } else {
-            ch[c].w2 = (unsigned)lP | ((unsigned)(lQ + 1) << 4) | ((unsigned)iu << 8) | ((unsigned)iv << 20);
-            ch[c].w3 = (unsigned)(2 * is + (c & 1)) | ((unsigned)(2 * itt + (c >> 1)) << 12);
-        }
-    }
-}
 
 #include "dc_narrow.cuh"
 
@@ -703,7 +668,7 @@ __global__ void k_uf_collect(DcScalars *S, const signed char *__restrict__ label
 __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
                                                          const double *__restrict__ fcoef, int n_face, unsigned char *comp)
 {
-    __shared__ double s_ecoef[6][27];
+    __shared__ double s_ecoef[6][28];
     __shared__ double s_nodes[81];
     __shared__ unsigned long long s_best;
     __shared__ double s_d[SL_THREADS], s_c[SL_THREADS];
@@ -725,51 +690,43 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
         for (int m = 0; m < 9; ++m) s_ecoef[k][c * 9 + m] = a[m];
     }
     __syncthreads();
-    const double t_tie = S->t_tie, theta = S->theta, tol_d = S->tol_d;
+    if (tid < 6) s_ecoef[tid][27] = higher_order_const(s_ecoef[tid]);
+    __syncthreads();
+    const double t_tie = S->t_tie, theta2 = S->theta * S->theta, tol_d2 = S->tol_d * S->tol_d;
     const int max_level = S->max_level;
     double my_d = INFINITY, my_c = 0.0;
     for (int f = tid; f < n_face; f += SL_THREADS) {
-        const double *AQ = fcoef + (size_t)f * 28;
+        double AQ[28];
+        for (int m = 0; m < 28; ++m) AQ[m] = __ldg(fcoef + (size_t)f * 28 + m);
         for (int k = 0; k < 6; ++k) {
             const double *AP = s_ecoef[k];
-            Item st[80];
+            NItem st[80];
             int top = 0;
-            st[top].f = f; st[top].w1 = 0; st[top].w2 = 0; st[top].w3 = 0; ++top;
+            st[top].p = (unsigned)f; st[top].ak = 0; st[top].w2 = 0; st[top].w3 = 0; ++top;
             while (top > 0) {
-                const Item it = st[--top];
+                const NItem it = st[--top];
                 double uc, vc, hP, sc, tc, hQ;
-                item_box(it, uc, vc, hP, sc, tc, hQ);
-                const NodeBound nb = bound_subpair([&](int m) { return AP[m]; }, [&](int m) { return __ldg(AQ + m); },
-                                                   uc, vc, hP, sc, tc, hQ);
+                nitem_box(it, uc, vc, hP, sc, tc, hQ);
+                const NodeOut nb = bound_node(AP, AQ, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
                 double best = u2d(s_best);
                 if (nb.dist_c < best) { atomicMin(&s_best, d2u(nb.dist_c)); best = nb.dist_c; }
                 if (nb.lb > best + t_tie) continue;
-                const double kP = nb.s1P > 0.0 ? nb.s2P / (nb.s1P * nb.s1P) : 0.0;
-                const double kQ = nb.s1Q > 0.0 ? nb.s2Q / (nb.s1Q * nb.s1Q) : 0.0;
-                bool leaf = dmax2(kP, kQ) * dmax2(nb.s1P, nb.s1Q) <= theta;
-                const int lP = it.w2 & 15, lQ = (it.w2 >> 4) & 15;
-                bool splitP = nb.s1P >= nb.s1Q;
-                if (!leaf) {
-                    if (splitP && lP >= max_level) splitP = false;
-                    if (!splitP && lQ >= max_level) { if (lP < max_level) splitP = true; else leaf = true; }
-                }
+                bool leaf = nb.leaf, splitP = false;
+                if (!leaf) leaf = !choose_split(it, nb.splitP, max_level, splitP);
                 if (leaf || top + 4 > 80) {
-                    double CP[27], CQ[27];
-                    for (int c = 0; c < 3; ++c) {
-                        double A[9];
-                        for (int m = 0; m < 9; ++m) A[m] = AP[c * 9 + m];
-                        recentre9(A, uc, vc, hP, hP, CP + 9 * c);
-                        for (int m = 0; m < 9; ++m) A[m] = __ldg(AQ + c * 9 + m);
-                        recentre9(A, sc, tc, hQ, hQ, CQ + 9 * c);
-                    }
-                    const NewtonOut o = newton_leaf(CP, CQ, tol_d, -1.0, NP_NEWTON_ITERS_SL);
-                    atomicMin(&s_best, d2u(o.dist));
-                    if (o.dist < my_d - t_tie || (o.dist <= my_d + t_tie && fabs(o.cosv) > fabs(my_c))) {
-                        my_d = dmin2(my_d, o.dist); my_c = o.cosv;
+                    // the same lockstep iteration as k_np_newton, run to the end by this thread (an unconverged
+                    // solve still yields an attained distance; a seedless component only needs the sign)
+                    dcn::NwState s; s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc; s.iters = 0; s.ls = 0; s.phase = 1;
+                    const double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };
+                    dcn::NwResult R; R.dist = INFINITY; R.cosv = 0.0; R.converged = 0;
+                    auto cf = [&](int m) { return m < 27 ? AP[m] : AQ[m - 27]; };
+                    while (!dcn::iterate(cf, s, lo, hi, tol_d2, -1.0, R)) { }
+                    atomicMin(&s_best, d2u(R.dist));
+                    if (R.dist < my_d - t_tie || (R.dist <= my_d + t_tie && fabs(R.cosv) > fabs(my_c))) {
+                        my_d = dmin2(my_d, R.dist); my_c = R.cosv;
                     }
                 } else {
-                    make_children(it, splitP, st + top);
-                    top += 4;
+                    for (int c = 0; c < 4; ++c) st[top++] = nitem_child(it, splitP, c);
                 }
             }
         }
