@@ -249,3 +249,33 @@ def test_many_faces_per_element(B, nproc):
     assert np.bincount(e).max() > 224, "this case is meant to overflow the per-warp pair stage"
     assert_parity(ref, labels, sdist, st)
     assert st.n_cut > 20
+
+
+def test_rigid_motion_of_grid_and_surface(B):
+    """Metamorphic (the paper's edge-case sweep under rotation, L282): moving grid and surface
+    together by one rigid motion leaves every label unchanged and every distance within rounding."""
+    w = make_config(2, N=18, n=8)
+    l0, s0, st0 = gpu_cut(B, w)
+    rng = np.random.default_rng(11)
+    q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    t = np.array([0.3, -0.2, 0.5])
+    w2 = type(w)(**{**w.__dict__, "xyz": w.xyz @ q.T + t, "faces": w.faces @ q.T + t})
+    l1, s1, st1 = gpu_cut(B, w2)
+    # a rotated box is not the box of the rotated element, so d_band (the clamp of far distances) changes: compare inside the band
+    band = min(st0.d_band, st1.d_band) * (1 - 1e-9)
+    assert np.array_equal(l0, l1)
+    near = (np.abs(s0) < band) & (np.abs(s1) < band)
+    assert near.sum() > 100 and np.abs(s0 - s1)[near].max() <= 1e-11 * st0.l_ref
+
+
+def test_parameters_theta_and_max_level_do_not_change_the_result(B):
+    """The leaf rule (theta_leaf) and the subdivision bound (max_level) steer the work, not the answer."""
+    w = make_config(2, N=16, n=8)
+    l0, s0, st0 = gpu_cut(B, w)
+    for theta, ml in ((0.03, 12), (0.5, 12), (0.125, 3)):
+        p = B.dc_params(); p.theta_leaf = theta; p.max_level = ml
+        l1, s1, st1 = gpu_cut(B, w, params=p)
+        assert np.array_equal(l0, l1) and np.abs(s0 - s1).max() <= 1e-11 * st0.l_ref, (theta, ml)
+    assert st0.n_newton > 0
