@@ -621,16 +621,36 @@ __global__ void __launch_bounds__(UF_TILE) k_uf_local(const signed char *__restr
 __global__ void k_uf_union(const signed char *__restrict__ labels, const int *__restrict__ adj, long long n_elem, int *parent)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n_elem || labels[e] == DC_CUT) return;
+    const bool live = e < n_elem && labels[e] != DC_CUT;
     const long long base = e & ~(long long)(UF_TILE - 1);
-    int nbs[6];
-    const int2 *ap = reinterpret_cast<const int2 *>(adj + e * 6);
+    const int lane = threadIdx.x & 31;
+    int nbs[6] = { -1, -1, -1, -1, -1, -1 };
+    int mine = 0;
+    if (live) {
+        const int2 *ap = reinterpret_cast<const int2 *>(adj + e * 6);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) { const int2 v = __ldg(ap + k); nbs[2 * k] = v.x; nbs[2 * k + 1] = v.y; }
+        for (int k = 0; k < 3; ++k) { const int2 v = __ldg(ap + k); nbs[2 * k] = v.x; nbs[2 * k + 1] = v.y; }
+        mine = ((volatile int *)parent)[e];              // its tile-local root (or an ancestor of it by now)
+    }
+    // all the gathers of the six neighbours first (independent loads in flight together), the unions after
+    int other[6];
+    bool edge[6];
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
         const int nb = nbs[k];
-        if (nb >= 0 && nb < base && labels[nb] != DC_CUT) uf_union(parent, (int)e, nb);
+        const bool cross = live && nb >= 0 && nb < base;
+        const int lab = cross ? labels[nb] : DC_CUT;
+        const int par = cross ? ((volatile int *)parent)[nb] : 0;
+        edge[k] = cross && lab != DC_CUT;
+        other[k] = edge[k] ? par : -1 - lane;
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        // neighbouring elements mostly sit in the same tile-local components on both sides of a tile border: a lane
+        // whose (root, root) pair equals that of the lane before it leaves the union to that lane (its own would be a
+        // no-op after three dependent loads)
+        const int pm = __shfl_up_sync(0xffffffffu, mine, 1), po = __shfl_up_sync(0xffffffffu, other[k], 1);
+        if (edge[k] && !(lane > 0 && pm == mine && po == other[k])) uf_union(parent, mine, other[k]);
     }
 }
 
