@@ -654,15 +654,16 @@ __global__ void k_uf_union(const signed char *__restrict__ labels, const int *__
     }
 }
 
-__global__ void k_uf_seed(const signed char *__restrict__ labels, long long n_elem, int *parent, unsigned char *comp)
+// seeds: only the band elements carry a sign from S6 (one thread per band element, not per element)
+__global__ void k_uf_seed(const DcScalars *S, const int *__restrict__ band_elem, const signed char *__restrict__ labels,
+                          int *parent, unsigned char *comp)
 {
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n_elem) return;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= min(S->n_band, S->max_band)) return;
+    const int e = band_elem[b];
     const int lab = labels[e];
-    if (lab == DC_CUT) return;
-    const int r = uf_find(parent, (int)e);
-    parent[e] = r;
     if (lab == DC_HOLE || lab == DC_NORMAL) {
+        const int r = uf_find(parent, e);
         // byte-wide OR through a 32-bit atomic
         unsigned *w = reinterpret_cast<unsigned *>(comp + (r & ~3));
         atomicOr(w, (unsigned)(lab == DC_HOLE ? 1 : 2) << (8 * (r & 3)));
@@ -763,7 +764,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
     }
 }
 
-__global__ void k_uf_assign(DcScalars *S, long long n_elem, const int *__restrict__ parent,
+__global__ void k_uf_assign(DcScalars *S, long long n_elem, int *parent,
                             const unsigned char *__restrict__ comp, signed char *__restrict__ labels,
                             double *__restrict__ sdist)
 {
@@ -773,7 +774,7 @@ __global__ void k_uf_assign(DcScalars *S, long long n_elem, const int *__restric
     if (e < n_elem) {
         lab = labels[e];
         if (lab != DC_CUT) {
-            const int bits = comp[parent[e]];
+            const int bits = comp[uf_find(parent, (int)e)];
             if (lab < 0) {
                 conflict = bits == 3;
                 lab = (bits == 1) ? DC_HOLE : DC_NORMAL;
@@ -1081,7 +1082,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     CK(cudaEventRecord(c->ev[3], st));
     k_uf_local<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(labels_dev, c->adj, ne, c->parent);
     k_uf_union<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, c->adj, ne, c->parent);
-    k_uf_seed<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, ne, c->parent, c->comp);
+    k_uf_seed<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
     k_uf_collect<<<nblk(ne, 256), 256, 0, st>>>(c->S, labels_dev, ne, c->parent, c->comp);
     k_seedless<<<DC_MAX_SEEDLESS, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
