@@ -136,7 +136,10 @@ __device__ __forceinline__ void scalar_range(const double *g, double uc, double 
     hi = dmax2(0.0, c2) + dmax2(0.0, c6) + dmax2(0.0, c8) + odd;
 }
 
-struct NodeOut { double dist_c, lb; bool leaf, splitP; };
+struct NodeOut {
+    double dist_c, lb; bool leaf, splitP;
+    double r[3], pu[3], pv[3], qs[3], qt[3];     // centre difference and first derivatives there (for the leaf's first step)
+};
 
 __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ, double KP, double KQ,
                                               double uc, double vc, double hP, double sc, double tc, double hQ,
@@ -151,6 +154,8 @@ __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ
         r[c] = p - q;
     }
     NodeOut o;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { o.r[c] = r[c]; o.pu[c] = pu[c]; o.pv[c] = pv[c]; o.qs[c] = qs[c]; o.qt[c] = qt[c]; }
     const double d2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
     const double inv = d2 > 0.0 ? rsqrt(d2) : 0.0;
     o.dist_c = d2 * inv;

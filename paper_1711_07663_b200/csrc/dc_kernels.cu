@@ -835,7 +835,7 @@ struct dc_ctx {
     int *act_elem;
     int *band_elem; long long *band_start; int *band_cnt;
     double *ecoef, *pbox; unsigned long long *best, *dmin;
-    NItem *q[2], *nq;
+    NItem *q[2], *nq; float4 *nqx;
     int *pair_face; unsigned long long *pair_key;
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
     int *cell_count, *cell_start, *cell_fill;
@@ -851,7 +851,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
     size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
-        off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq,
+        off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq, off_nqx,
         off_pair_face, off_pair_key, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
         off_cell_count, off_cell_start, off_cell_fill, off_hfaces, off_hlabels, off_hsdist, total;
     long long max_band, qcap;
@@ -887,6 +887,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_q0 = take((size_t)L.qcap * sizeof(NItem));
     L.off_q1 = take((size_t)L.qcap * sizeof(NItem));
     L.off_nq = take((size_t)(L.qcap > L.max_band ? L.qcap : L.max_band) * sizeof(NItem));
+    L.off_nqx = take((size_t)(L.qcap > L.max_band ? L.qcap : L.max_band) * sizeof(float4));
     // pair arrays double as the scratch of the adjacency derivation (2 x n_nodes ints)
     size_t pf = (size_t)max_pairs * 4, pk = (size_t)max_pairs * 8;
     size_t need_adj = (size_t)n_nodes * 8;
@@ -967,6 +968,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->q[0] = (NItem *)(c->ws + L.off_q0);
     c->q[1] = (NItem *)(c->ws + L.off_q1);
     c->nq = (NItem *)(c->ws + L.off_nq);
+    c->nqx = (float4 *)(c->ws + L.off_nqx);
     c->pair_face = (int *)(c->ws + L.off_pair_face);
     c->pair_key = (unsigned long long *)(c->ws + L.off_pair_key);
     c->fbox_orig = (double *)(c->ws + L.off_fbox_orig);
@@ -1056,7 +1058,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     // seed solves: one per band element, queue = nq[0 .. n_band); failures are never re-split
     const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
     CK(cudaEventRecord(c->ev[7], st));
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, c->pair_face, c->fcoef, c->ecoef,
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, nullptr, c->pair_face, c->fcoef, c->ecoef,
                                                        c->best, c->dmin, c->pair_key);
     CK(cudaEventRecord(c->ev[10], st));
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
@@ -1068,13 +1070,13 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
     for (int r = 0; r < grid_rounds; ++r)
         k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, &S->nn[0], c->qcap);
+                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap);
     if (rounds > grid_rounds)
         k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                       c->nq, &S->nn[0], c->qcap);
+                                                       c->nq, c->nqx, &S->nn[0], c->qcap);
     // all leaves in one launch; an unconverged leaf is quartered and finished by the lane that held it
     CK(cudaEventRecord(c->ev[5], st));
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->pair_face, c->fcoef, c->ecoef,
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
                                                        c->best, c->dmin, c->pair_key);
     CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,

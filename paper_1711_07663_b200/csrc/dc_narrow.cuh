@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
 
 __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
-                                                            const NItem *__restrict__ nq,
+                                                            const NItem *__restrict__ nq, const float4 *__restrict__ nqx,
                                                             const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                             const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                             unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key)
@@ -269,6 +269,7 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
     // 0 no ticket, 1 ticket asked for, 2 ticket in hand, 3 item asked for, 4 face id and best[b] asked for (ready), 9 queue exhausted
     int nst = 0, nface = 0, tk = 0, pbase = 0, pleader = 0;
     unsigned long long nbest = 0;
+    float4 nx0 = make_float4(0.f, 0.f, 0.f, 0.f);   // its starting point (local coordinates; zero = the centre, for seeds)
     bool pend = false;              // (warp-uniform) a ticket atomic is in flight
     NItem stk[NW_STACK];            // sub-leaves of an unconverged solve, solved by the same lane (local memory, rarely touched)
     int sp = 0;
@@ -297,6 +298,7 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
             else {
                 const uint4 w = __ldg(reinterpret_cast<const uint4 *>(nq + tk));
                 nxt.p = w.x; nxt.ak = w.y; nxt.w2 = w.z; nxt.w3 = w.w;
+                if (nqx) nx0 = __ldg(nqx + tk);
                 nst = 3;
             }
         }
@@ -320,7 +322,12 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                         fresh = true;
                         double uc, vc, hP, sc, tc, hQ;
                         nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                        s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
+                        // start at the first step k_np_bound took from the centre (local coordinates; on a bound when within float rounding of it)
+                        const double a0 = nx0.x, a1 = nx0.y, a2 = nx0.z, a3 = nx0.w, e1 = 1.0 - 1e-6;
+                        s.x[0] = a0 >= e1 ? uc + hP : (a0 <= -e1 ? uc - hP : fma(hP, a0, uc));
+                        s.x[1] = a1 >= e1 ? vc + hP : (a1 <= -e1 ? vc - hP : fma(hP, a1, vc));
+                        s.x[2] = a2 >= e1 ? sc + hQ : (a2 <= -e1 ? sc - hQ : fma(hQ, a2, sc));
+                        s.x[3] = a3 >= e1 ? tc + hQ : (a3 <= -e1 ? tc - hQ : fma(hQ, a3, tc));
                         s.iters = 0; s.ls = 0; s.phase = 1;
                         pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
                         pQ = (unsigned long long)(fcoef + (size_t)nface * 28);
@@ -455,6 +462,27 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_roots(DcScalars *S, const lo
     }
 }
 
+// First step of a leaf's closest-point solve, taken here where the centre evaluation already exists: the
+// Gauss-Newton step of |r + P_u du + P_v dv - Q_s ds - Q_t dt|^2 from the centre, clamped to the leaf's box, in the
+// leaf's local coordinates [-1,1]^4 (floats: it is a starting point).  Saves k_np_newton its evaluation at the centre.
+__device__ __forceinline__ float4 leaf_first_step(const NodeOut &o, double hP, double hQ)
+{
+#define DOT3(A, B) (A[0] * B[0] + A[1] * B[1] + A[2] * B[2])
+    // local variables a = du / hP ... : columns scaled by the half-widths
+    const double h00 = hP * hP * DOT3(o.pu, o.pu), h01 = hP * hP * DOT3(o.pu, o.pv), h02 = -hP * hQ * DOT3(o.pu, o.qs), h03 = -hP * hQ * DOT3(o.pu, o.qt);
+    const double h11 = hP * hP * DOT3(o.pv, o.pv), h12 = -hP * hQ * DOT3(o.pv, o.qs), h13 = -hP * hQ * DOT3(o.pv, o.qt);
+    const double h22 = hQ * hQ * DOT3(o.qs, o.qs), h23 = hQ * hQ * DOT3(o.qs, o.qt), h33 = hQ * hQ * DOT3(o.qt, o.qt);
+    const double g[4] = { hP * DOT3(o.r, o.pu), hP * DOT3(o.r, o.pv), -hQ * DOT3(o.r, o.qs), -hQ * DOT3(o.r, o.qt) };
+#undef DOT3
+    const double tr = h00 + h11 + h22 + h33;
+    double p[4] = { 0.0, 0.0, 0.0, 0.0 };
+    if (tr > 0.0) dcn::ldl4_mod(h00, h01, h02, h03, h11, h12, h13, h22, h23, h33, g, 1e-6 * tr, p);
+    float4 x;
+    x.x = (float)dmax2(-1.0, dmin2(1.0, p[0])); x.y = (float)dmax2(-1.0, dmin2(1.0, p[1]));
+    x.z = (float)dmax2(-1.0, dmin2(1.0, p[2])); x.w = (float)dmax2(-1.0, dmin2(1.0, p[3]));
+    return x;
+}
+
 // ------------------------------------------------------------------------------------------
 // Bound: one thread per item of qin[0 .. n): prune, or 4 children -> qout, or leaf -> the ONE leaf queue nq
 // (all rounds append to it; the Newton kernel runs once, after the last round).  Items i0, i0 + stride, ...
@@ -462,7 +490,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                                                const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                NItem *__restrict__ qout, int *__restrict__ qout_n,
-                                               NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap,
+                                               NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap,
                                                int i0, int stride, NpCounters &cnt)
 {
     const double t_tie = S->t_tie, tau_exit = S->tau_exit, theta2 = S->theta * S->theta;
@@ -471,6 +499,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
     for (int i = i0; i < n_round; i += stride) {
         bool split = false, leaf = false, splitP = false;
         NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
+        float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (i < n) {
             // (L2 load: the tail kernel reads items the same launch wrote)
             const uint4 w = __ldcg(reinterpret_cast<const uint4 *>(qin + i));
@@ -498,11 +527,12 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                         split = choose_split(it, o.splitP, max_level, splitP);
                         if (!split) { leaf = true; cnt.depth++; }
                     }
+                    if (leaf) x0 = leaf_first_step(o, hP, hQ);
                 }
             }
         }
         const long long sl = warp_reserve(nq_n, leaf, 1, qcap, &S->status);
-        if (sl >= 0) nq[sl] = it;
+        if (sl >= 0) { nq[sl] = it; nqx[sl] = x0; }
         const long long slot = warp_reserve(qout_n, split, 4, qcap, &S->status);
         if (slot >= 0) {
 #pragma unroll
@@ -515,13 +545,13 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
-                                                          NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap)
+                                                          NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
 {
     const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
     if (n == 0) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
     NpCounters cnt = { 0, 0, 0, 0, 0 };
-    np_bound_items(S, n, qin, pair_face, fcoef, ecoef, best, qout, qout_n, nq, nq_n, qcap,
+    np_bound_items(S, n, qin, pair_face, fcoef, ecoef, best, qout, qout_n, nq, nqx, nq_n, qcap,
                    blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, cnt);
     np_flush_counters(S, cnt);
 }
@@ -532,14 +562,14 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
 __global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S, int r_begin, int r_end, NItem *q0, NItem *q1,
                                                                    const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                                    const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                                   NItem *__restrict__ nq, int *__restrict__ nq_n, long long qcap)
+                                                                   NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
 {
     NpCounters cnt = { 0, 0, 0, 0, 0 };
     for (int r = r_begin; r < r_end; ++r) {
         const int n = min(*(volatile int *)&S->qn[r], (int)min(qcap, (long long)0x7fffffff));
         if (n == 0) break;
         if (threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
-        np_bound_items(S, n, (r & 1) ? q1 : q0, pair_face, fcoef, ecoef, best, (r & 1) ? q0 : q1, &S->qn[r + 1], nq, nq_n, qcap,
+        np_bound_items(S, n, (r & 1) ? q1 : q0, pair_face, fcoef, ecoef, best, (r & 1) ? q0 : q1, &S->qn[r + 1], nq, nqx, nq_n, qcap,
                        threadIdx.x, NP_TAIL_THREADS, cnt);
         __threadfence();
         __syncthreads();
