@@ -1059,7 +1059,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
     CK(cudaEventRecord(c->ev[7], st));
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key);
+                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0);
     CK(cudaEventRecord(c->ev[10], st));
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
                                            c->q[0], &S->qn[0], c->qcap);
@@ -1070,14 +1070,25 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
     for (int r = 0; r < grid_rounds; ++r)
         k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap);
+                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
     if (rounds > grid_rounds)
         k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                        c->nq, c->nqx, &S->nn[0], c->qcap);
     // all leaves in one launch; an unconverged leaf is quartered and finished by the lane that held it
     CK(cudaEventRecord(c->ev[5], st));
+    // The sub-leaves of unconverged solves go to an overflow queue (the bound queues are free by now) and come back
+    // through one bound pass (best[b] is final or nearly so: most of them are pruned) and one Newton launch, twice;
+    // the last launch finishes whatever still fails on the lane that held it.
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key);
+                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[1], c->qcap);
+    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           c->nq, &S->qn[DC_NQN - 1], c->q[1], c->nqx, &S->nn[2], c->qcap, 1);
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[2], c->qcap, &S->nh[2], c->q[1], c->nqx, c->pair_face, c->fcoef, c->ecoef,
+                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[3], c->qcap);
+    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           c->q[1], &S->qn[DC_NQN - 1], c->nq, c->nqx, &S->nn[4], c->qcap, 1);
+    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[4], c->qcap, &S->nh[3], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
+                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0);
     CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
@@ -1090,7 +1101,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
-    c->launches_classify = 14 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
+    c->launches_classify = 18 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }

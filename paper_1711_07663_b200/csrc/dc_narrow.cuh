@@ -241,13 +241,15 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_STRIDE 129
 #define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
 #define NW_STACK 12                 /* sub-leaves a lane may hold (3 levels of quartering) */
+#define NW_TICKETS 64                /* queue tickets a warp draws per atomic on the queue head */
 #define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
 
 __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
                                                             const NItem *__restrict__ nq, const float4 *__restrict__ nqx,
                                                             const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                             const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                            unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key)
+                                                            unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
+                                                            NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap)
 {
     extern __shared__ double nw_sm[];
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
@@ -266,8 +268,11 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
     for (int i = 0; i < 4; ++i) s.x[i] = 0.0;
     NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
     NItem nxt; nxt.p = nxt.ak = nxt.w2 = nxt.w3 = 0;       // prefetched next item of this lane
-    // 0 no ticket, 1 ticket asked for, 2 ticket in hand, 3 item asked for, 4 face id and best[b] asked for (ready), 9 queue exhausted
-    int nst = 0, nface = 0, tk = 0, pbase = 0, pleader = 0;
+    // 0 no ticket, 2 ticket in hand, 3 item asked for, 4 face id and best[b] asked for (ready), 9 queue exhausted
+    int nst = 0, nface = 0, tk = 0, pbase = 0;
+    int pool_next = 0, pool_end = 0;    // (warp-uniform) tickets this warp holds
+    // tickets per draw: half a warp's share of the queue, between 8 and NW_TICKETS (short queues stay spread out)
+    const int chunk = max(8, min(NW_TICKETS, n / (int)(gridDim.x * (NW_THREADS / 32) * 2)));
     unsigned long long nbest = 0;
     float4 nx0 = make_float4(0.f, 0.f, 0.f, 0.f);   // its starting point (local coordinates; zero = the centre, for seeds)
     bool pend = false;              // (warp-uniform) a ticket atomic is in flight
@@ -302,9 +307,9 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 nst = 3;
             }
         }
-        if (pend) {                                   // (uniform) the ticket atomic of the previous trip has landed
-            const int base = __shfl_sync(0xffffffffu, pbase, pleader);
-            if (nst == 1) { tk = base + tk; nst = 2; }
+        if (pend) {                                   // (uniform) the ticket atomic of an earlier trip has landed
+            pool_next = __shfl_sync(0xffffffffu, pbase, 0);
+            pool_end = pool_next + chunk;
             pend = false;
         }
         // ---- idle lanes whose next item is ready take it
@@ -335,13 +340,18 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 }
             }
         }
-        // ---- lanes without a next item draw a ticket (the result is looked at next trip)
+        // ---- lanes without a next item draw a ticket from the warp's pool; the pool is refilled NW_TICKETS at a time by
+        // one atomic on the queue head whose result is looked at on a later trip (a ticket per lane per trip from the
+        // head itself made 2 368 warps queue up on ONE address: the kernel ran at the pace of that atomic)
         {
             const unsigned m0 = __ballot_sync(0xffffffffu, nst == 0);
-            if (m0 && !pend) {
-                pleader = __ffs(m0) - 1;
-                if (lane == pleader) pbase = atomicAdd(head, __popc(m0));
-                if (nst == 0) { tk = __popc(m0 & lt_mask); nst = 1; }
+            if (m0) {
+                const int avail = pool_end - pool_next, rank = __popc(m0 & lt_mask);
+                if (nst == 0 && rank < avail) { tk = pool_next + rank; nst = 2; }
+                pool_next += min(__popc(m0), avail);
+            }
+            if (pool_next == pool_end && !pend) {
+                if (lane == 0) pbase = atomicAdd(head, chunk);
                 pend = true;
             }
         }
@@ -376,6 +386,7 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
             fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R);
         }
         // ---- results of the solves that finished (an attained distance is an upper bound whether converged or not)
+        bool resplit = false, splitP = false;
         if (fin) {
             const unsigned b = it.ak & 0x1fffffffu;
             cnt.newton++; cnt.iters += s.iters;
@@ -386,15 +397,26 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 const unsigned long long key = (d2u(R.dist) & ~0xffull) | (unsigned long long)cos_code(R.cosv);
                 atomicMin(pair_key + it.p, key);
                 if (!R.converged && !((it.w3 >> 24) & 1)) {
-                    // unconverged: the distance above stands as an upper bound; the leaf is quartered and the four
-                    // sub-leaves are solved by this lane (a seed solve is never split: the roots cover its pair)
+                    // unconverged: the distance above stands as an upper bound and the leaf is quartered (a seed solve is
+                    // never split: the roots cover its pair).  With an overflow queue the four sub-leaves go there, for
+                    // the next launch to spread over the machine: solved one after the other by this lane they were a
+                    // serial chain of up to 5 x NW_MAXIT evaluations that the whole launch waited for (175 us of 690).
                     cnt.fail++;
-                    bool splitP = false;
-                    if (sp + 4 <= NW_STACK && choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP)) {
+                    if (choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP)) {
+                        if (ovf) resplit = true;
+                        else if (sp + 4 <= NW_STACK) {
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) stk[sp++] = nitem_child(it, splitP, c);
+                            for (int c = 0; c < 4; ++c) stk[sp++] = nitem_child(it, splitP, c);
+                        } else cnt.depth++;
                     } else cnt.depth++;
                 }
+            }
+        }
+        if (ovf) {
+            const long long sl = warp_reserve(ovf_n, resplit, 4, ovf_cap, &S->status);
+            if (sl >= 0) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) ovf[sl + c] = nitem_child(it, splitP, c);
             }
         }
     }
@@ -491,7 +513,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                                                const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                NItem *__restrict__ qout, int *__restrict__ qout_n,
                                                NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap,
-                                               int i0, int stride, NpCounters &cnt)
+                                               int i0, int stride, NpCounters &cnt, bool force_leaf = false)
 {
     const double t_tie = S->t_tie, tau_exit = S->tau_exit, theta2 = S->theta * S->theta;
     const int max_level = S->max_level;
@@ -522,7 +544,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                 cnt.nodes++;
                 if (o.dist_c < bst) { atomicMin(best + b, d2u(o.dist_c)); bst = o.dist_c; }
                 if (o.dist_c > tau_exit && o.lb <= bst + t_tie) {
-                    leaf = o.leaf;
+                    leaf = o.leaf || force_leaf;     // (sub-leaves of an unconverged leaf stay leaves)
                     if (!leaf) {
                         split = choose_split(it, o.splitP, max_level, splitP);
                         if (!split) { leaf = true; cnt.depth++; }
@@ -545,14 +567,14 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
-                                                          NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
+                                                          NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap, int force_leaf)
 {
     const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
     if (n == 0) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
     NpCounters cnt = { 0, 0, 0, 0, 0 };
     np_bound_items(S, n, qin, pair_face, fcoef, ecoef, best, qout, qout_n, nq, nqx, nq_n, qcap,
-                   blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, cnt);
+                   blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, cnt, force_leaf != 0);
     np_flush_counters(S, cnt);
 }
 
