@@ -355,21 +355,28 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                 pend = true;
             }
         }
-        // ---- the new items' coefficients go into their lanes' slots by asynchronous copies (cp.async, 8 bytes each),
-        // ALL issued before the one wait, so the new lanes of a trip cost one memory round trip together.
-        // Lane-private: every new lane copies its own 54 coefficients (54 predicated instructions per trip however
-        // many lanes are new; a warp-cooperative coalesced copy cost ~30 instructions per new lane, ~6 per trip, for no gain).
-        if (__ballot_sync(0xffffffffu, fresh)) {
-            if (fresh) {
-                const double *a = (const double *)pA, *q = (const double *)pQ;
-                const unsigned d0 = (unsigned)__cvta_generic_to_shared(nw_sm + tid);
-#pragma unroll
-                for (int m = 0; m < 27; ++m) {
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0 + m * (NW_STRIDE * 8)), "l"(a + m));
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0 + (27 + m) * (NW_STRIDE * 8)), "l"(q + m));
-                }
+        // ---- the new items' coefficients go into their lanes' slots by asynchronous copies (cp.async, 8 bytes per
+        // lane), ALL issued before the one wait, so the new lanes of a trip cost one memory round trip together.
+        // Warp-cooperative: the warp copies one new lane's 2 x 216 contiguous bytes at a time (~5 L1 wavefronts per new
+        // lane; every new lane copying its own 54 coefficients cost 54, and the L1 data pipe -- shared-memory reads
+        // of the coefficients plus these copies -- is the resource this kernel saturates).
+        {
+            unsigned mf = __ballot_sync(0xffffffffu, fresh);
+            if (mf) {
+                double *wslot = nw_sm + (tid & ~31);
+                do {
+                    const int L = __ffs(mf) - 1; mf &= mf - 1;
+                    const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
+                    const double *q = (const double *)__shfl_sync(0xffffffffu, pQ, L);
+                    const unsigned d0 = (unsigned)__cvta_generic_to_shared(wslot + L + lane * NW_STRIDE);
+                    const double *g0 = lane < 27 ? a + lane : q + (lane - 27);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0), "l"(g0));
+                    if (lane < 22)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0 + 32 * NW_STRIDE * 8), "l"(q + (lane + 5)));
+                } while (mf);
+                asm volatile("cp.async.wait_all;" ::: "memory");
             }
-            asm volatile("cp.async.wait_all;" ::: "memory");
+            __syncwarp();
         }
         if (__ballot_sync(0xffffffffu, s.phase != 0) == 0) {
             if (__ballot_sync(0xffffffffu, nst != 9 || sp > 0) == 0) break;
