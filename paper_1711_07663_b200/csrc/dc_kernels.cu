@@ -1055,11 +1055,12 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     DcScalars *S = c->S;
     k_np_stage<<<gw, NPW_THREADS, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fcoef,
                                            c->ecoef, c->pbox, c->best, c->dmin, c->nq);
-    // seed solves: one per band element, queue = nq[0 .. n_band); failures are never re-split
+    // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
+    // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
     const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
     CK(cudaEventRecord(c->ev[7], st));
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0);
+                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_SEED_MAXIT);
     CK(cudaEventRecord(c->ev[10], st));
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
                                            c->q[0], &S->qn[0], c->qcap);
@@ -1080,15 +1081,15 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     // through one bound pass (best[b] is final or nearly so: most of them are pruned) and one Newton launch, twice;
     // the last launch finishes whatever still fails on the lane that held it.
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[1], c->qcap);
+                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[1], c->qcap, NW_MAXIT);
     k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
                                            c->nq, &S->qn[DC_NQN - 1], c->q[1], c->nqx, &S->nn[2], c->qcap, 1);
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[2], c->qcap, &S->nh[2], c->q[1], c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[3], c->qcap);
+                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[3], c->qcap, NW_MAXIT);
     k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
                                            c->q[1], &S->qn[DC_NQN - 1], c->nq, c->nqx, &S->nn[4], c->qcap, 1);
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[4], c->qcap, &S->nh[3], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0);
+                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_MAXIT);
     CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);

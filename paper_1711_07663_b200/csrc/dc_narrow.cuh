@@ -242,6 +242,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
 #define NW_STACK 12                 /* sub-leaves a lane may hold (3 levels of quartering) */
 #define NW_TICKETS 64                /* queue tickets a warp draws per atomic on the queue head */
+#define NW_SEED_MAXIT 8              /* evaluations a seed solve may take */
 #define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
 
 __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
@@ -249,7 +250,7 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                                                             const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                             const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                             unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
-                                                            NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap)
+                                                            NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap, int maxit)
 {
     extern __shared__ double nw_sm[];
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
@@ -390,7 +391,7 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
             double uc, vc, hP, sc, tc, hQ;
             nitem_box(it, uc, vc, hP, sc, tc, hQ);
             const double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };
-            fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R);
+            fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R, maxit);
         }
         // ---- results of the solves that finished (an attained distance is an upper bound whether converged or not)
         bool resplit = false, splitP = false;

@@ -127,7 +127,8 @@ DCN_HD bool ldl4_mod(double h00, double h01, double h02, double h03, double h11,
 // One lockstep iteration (tol_d2 = tol_d^2, tau_exit2 = tau_exit^2 or negative to disable).  Returns true when the solve is finished (R filled: the distance is attained
 // at the point just evaluated, hence an upper bound of the minimum whether or not it converged).
 template <class CF>
-DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, double tol_d2, double tau_exit2, NwResult &R)
+DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, double tol_d2, double tau_exit2, NwResult &R,
+                    int maxit = NW_MAXIT)
 {
     const double u = s.x[0], v = s.x[1], sq = s.x[2], tq = s.x[3];
     double rr = 0.0, g[4] = { 0.0, 0.0, 0.0, 0.0 };
@@ -220,7 +221,7 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
             if (dec) rr_out = fn;
         } else if ((dec && !moved) || s.ls > 7) {
             finished = true; converged = 0;              // stalled at the point just evaluated
-        } else if (s.iters >= NW_MAXIT - 1) {
+        } else if (s.iters >= maxit - 1) {
             s.phase = 3;                                  // one last evaluation
         }
     }
