@@ -296,8 +296,9 @@ def main():
     # ---- rooflines
     hbm_peak, hbm_src = _peaks()
     fp64_peak = B.dc_measure_fp64_tflops(local_rank, 4000)
-    # dominant kernel: k_np_newton (two launches per cut: seed solves + leaf solves), timed by CUDA events
-    # recorded by the library on the caller's stream around exactly those launches (dc_stats.ms_stage[7])
+    # dominant kernel: k_np_newton (seed solves, leaf solves, two short launches over the sub-leaves of unconverged
+    # solves), timed by CUDA events recorded by the library on the caller's stream around the seed launch and around
+    # the other three (two ~7 us k_np_bound passes sit between those and are inside the interval): dc_stats.ms_stage[7]
     newton_flops = s_last.n_newton_iters * FLOP_PER_NEWTON_EVAL + s_last.n_newton * FLOP_PER_NEWTON_FINISH
     newton_ms = float(med[7])
     ach_tf = newton_flops / (newton_ms * 1e-3) / 1e12 if newton_ms > 0 else 0.0
@@ -306,12 +307,12 @@ def main():
     s2_bytes = 108.0 * w.n_elem + 24.0 * len(w.xyz) + 48.0 * w.n_elem
     s2_ms = float(med[1])
     ach_gbs = s2_bytes / (s2_ms * 1e-3) / 1e9 if s2_ms > 0 else 0.0
-    roofline = {"kernel": "k_np_newton (S5 closest-point solves, 2 launches per cut)", "bound": "alu", "achieved": ach_tf,
+    roofline = {"kernel": "k_np_newton (S5 closest-point solves: seed, leaf and two overflow launches per cut)", "bound": "alu", "achieved": ach_tf,
                 "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": ach_tf / fp64_peak if fp64_peak > 0 else None,
                 # dram__bytes_read.sum + dram__bytes_write.sum of the two launches in the committed ncu --set full
-                # capture (profiles/r1c_kernels_full_config2.md: 48.4 + 0.3 and 111.1 + 6.7 MB), config 2 only
-                "traffic": 166.5e6 if cfg in (2, 3) else None,
+                # capture (profiles/r1c_kernels_full_config2.md: 48.5 + 0.5 and 133.0 + 7.4 MB, the overflow launches < 0.1 MB), config 2 only
+                "traffic": 189.4e6 if cfg in (2, 3) else None,
                 "algorithmic_flops_per_cut": newton_flops, "ms_per_cut": newton_ms,
                 "peak_source": "measured: dc_measure_fp64_tflops (register-resident DFMA chains on all SMs) in this run",
                 "share_of_step": newton_ms / float(med[5] + med[6]) if med[5] > 0 else None,
