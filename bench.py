@@ -15,7 +15,7 @@ nodes + connectivity + adjacency, surface faces) are resident in HBM before the 
             dc_create_grid, as the paper does for grid-only structures).
   roofline: the dominant kernel (k_np_newton, the closest-point solves of S5; FP64-ALU bound): algorithmic
             flops (device counters x the per-operation constants of DESIGN.md) / its CUDA-event duration
-            (events recorded by the library around its two launches), against the DFMA peak measured on
+            (events recorded by the library around its launches), against the DFMA peak measured on
             this GPU in this run.  The HBM-bound S2 kernel is reported beside it ("roofline_s2").
   cpu_baseline: the oracle (oracle/dc_oracle.c, as it stands) on this box's host cores on a bounded
             uniform sample of the same workload's elements, each against ALL faces.
@@ -310,7 +310,7 @@ def main():
     roofline = {"kernel": "k_np_newton (S5 closest-point solves: seed, leaf and two overflow launches per cut)", "bound": "alu", "achieved": ach_tf,
                 "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": ach_tf / fp64_peak if fp64_peak > 0 else None,
-                # dram__bytes_read.sum + dram__bytes_write.sum of the two launches in the committed ncu --set full
+                # dram__bytes_read.sum + dram__bytes_write.sum of its launches in the committed ncu --set full
                 # capture (profiles/r1c_kernels_full_config2.md: 48.5 + 0.5 and 133.0 + 7.4 MB, the overflow launches < 0.1 MB), config 2 only
                 "traffic": 189.4e6 if cfg in (2, 3) else None,
                 "algorithmic_flops_per_cut": newton_flops, "ms_per_cut": newton_ms,

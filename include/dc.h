@@ -98,7 +98,7 @@ typedef struct {
     double l_ref, tau_cut, d_band;
     float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
                                     4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface,
-                                    7 the two k_np_newton launches of S5 (seed + leaf solves: the dominant kernel) */
+                                    7 the k_np_newton launches of S5 (seed, leaf and overflow solves: the dominant kernel) */
     int status;                  /* DC_STATUS_* bits */
     int n_launches;              /* kernels launched by the last dc_set_cut_surface + dc_classify */
 } dc_stats;
