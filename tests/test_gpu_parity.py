@@ -279,3 +279,34 @@ def test_parameters_theta_and_max_level_do_not_change_the_result(B):
         l1, s1, st1 = gpu_cut(B, w, params=p)
         assert np.array_equal(l0, l1) and np.abs(s0 - s1).max() <= 1e-11 * st0.l_ref, (theta, ml)
     assert st0.n_newton > 0
+
+
+def test_element_permutation(B):
+    """Elements renumbered at random (adjacency remapped): neighbours no longer have nearby ids, so the tile-local
+    union-find pass settles almost nothing and every edge goes through the global forest; the labels and distances
+    must simply be permuted."""
+    w = make_config(1, N=13, n=4)
+    l0, s0, st0 = gpu_cut(B, w)
+    rng = np.random.default_rng(8)
+    perm = rng.permutation(w.n_elem)                 # new element i is old element perm[i]
+    inv = np.empty_like(perm); inv[perm] = np.arange(w.n_elem)
+    adj = w.adj6[perm]
+    adj = np.where(adj >= 0, inv[np.maximum(adj, 0)], -1).astype(np.int32)
+    w2 = type(w)(**{**w.__dict__, "conn27": np.ascontiguousarray(w.conn27[perm]), "adj6": np.ascontiguousarray(adj)})
+    l1, s1, st1 = gpu_cut(B, w2)
+    assert np.array_equal(l1, l0[perm]) and np.abs(s1 - s0[perm]).max() <= 1e-12 * st0.l_ref
+    # and with the adjacency derived by the library from the shared face-centre nodes
+    l2, s2, _ = gpu_cut(B, w2, adj="derive")
+    assert np.array_equal(l2, l1) and np.array_equal(s2, s1)
+
+
+def test_whole_grid_inside_the_band(B, nproc):
+    """d_band larger than the grid: every element gets its exact distance (no flood fill at all; the 'exact everywhere'
+    option of reading A5), against the oracle with the same band."""
+    w = make_config(1, N=9, n=3)
+    p = B.dc_params(); p.d_band = 10.0
+    ref = O.classify(w.xyz, w.conn27, w.faces, nproc=nproc, d_band=10.0)
+    labels, sdist, st = gpu_cut(B, w, params=p, max_pairs=w.n_elem * w.n_face)
+    assert st.n_pairs == w.n_elem * w.n_face
+    assert_parity(ref, labels, sdist, st, expect_zero_ambiguous=True)
+    assert np.abs(sdist).max() < 10.0 and np.abs(sdist).max() > 0.5
