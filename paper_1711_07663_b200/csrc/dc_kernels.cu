@@ -5,7 +5,7 @@
 //   S3 face bins      k_face_hist, k_scan_sums, k_scan_cells, k_face_scatter        (Morton-ordered uniform bins)
 //   S2 element boxes  k_elem_boxes                                    (HBM-bound stream)
 //   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
-//   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound (wavefront of uniform kernels, FP64)
+//   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound, k_np_bound_tail (FP64)
 //   S6 decide         k_np_decide
 //   S7 flood fill     k_uf_local, k_uf_union, k_uf_seed, k_uf_collect, k_seedless, k_uf_assign
 //
@@ -261,8 +261,8 @@ __global__ void k_face_scatter(const double *__restrict__ face_nodes, const doub
 
 // ------------------------------------------------------------------------------------------
 // S2: conservative element boxes from the 26 boundary control points of the Bezier net.
-// One thread per element; conn rows are staged through shared memory so the global reads
-// are fully coalesced.  ebox is SoA: ebox[c*n_elem + e] (c = 0..5: min xyz, max xyz).
+// conn rows are staged through shared memory so the global reads are fully coalesced.
+// ebox is SoA: ebox[c*n_elem + e] (c = 0..5: min xyz, max xyz).
 #ifndef EB_THREADS
 #define EB_THREADS 128
 #endif

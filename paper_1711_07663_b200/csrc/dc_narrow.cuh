@@ -1,22 +1,24 @@
-// dc_narrow.cuh -- S5 (narrow phase) and S6 (decide) as a WAVEFRONT of small uniform kernels.
+// dc_narrow.cuh -- S5 (narrow phase) and S6 (decide) as a short sequence of uniform kernels over global queues.
 //
-// Every kernel does one operation on one item per thread and compacts its output into a global
-// queue (warp-aggregated atomics), so warps stay full and no kernel carries another's registers:
+// Every kernel does one kind of operation and compacts its output into a global queue (warp-aggregated
+// atomics), so warps stay full and no kernel carries another's registers:
 //
-//   k_np_stage   warp / band element : gather the 27 nodes (coalesced conn row), monomial coefficients
-//                                      and Bezier boxes of the 6 boundary patches -> ecoef, pbox;
-//                                      centre-centre distances of all (pair, patch) -> first upper
-//                                      bound best[b] and ONE seed item per element
-//   k_np_newton  persistent warps    : projected Newton (Eq. 3-5 L256-L270 generalised to two patches,
-//                                      clamp L272-L278) on a leaf; min into best/dmin/pair_key;
-//                                      an unconverged non-seed leaf is re-split
-//   k_np_roots   warp / band element : (pair, patch) whose boxes are within best + t_tie (A.2,
-//                                      L689-L709) become root items
-//   k_np_bound   thread / item       : bound_node -> prune / 4 children / leaf
-//   k_np_decide  thread / band elem  : S6 (L215 nearest face and its normal; tie rule L294)
+//   k_np_stage      warp / band element : gather the 27 nodes, monomial coefficients and Bezier boxes of the 6
+//                                         boundary patches -> ecoef, pbox; centre-centre distances of all
+//                                         (pair, patch) -> first upper bound best[b] and ONE seed item per element
+//   k_np_newton     persistent warps    : projected Newton (Eq. 3-5 L256-L270 generalised to two patches, clamp
+//                                         L272-L278), one solve per lane in lockstep, lanes refilled from the
+//                                         queue; min into best / dmin / pair_key; the sub-leaves of an unconverged
+//                                         leaf go to an overflow queue
+//   k_np_roots      warp / band element : (pair, patch) whose boxes are within best + t_tie (A.2, L689-L709)
+//                                         become the items of round 0
+//   k_np_bound      thread / item       : bound_node -> prune / 4 children / leaf (+ the leaf's first step)
+//   k_np_bound_tail one CTA             : the sparse late rounds, until one comes up empty
+//   k_np_decide     thread / band elem  : S6 (L215 nearest face and its normal; tie rule L294)
 //
-// Round r = k_np_bound(r) + k_np_newton(r): every item of round r has lP + lQ = r, so 2 max_level + 1
-// rounds always terminate the branch and bound; empty rounds exit at once.
+// Launch order (dc_classify): stage, newton(seeds), roots, bound x 8, bound_tail, newton(leaves),
+// [bound(overflow), newton] x 2, decide.  Every item of bound round r has lP + lQ = r, so 2 max_level + 1
+// rounds always terminate the branch and bound.
 #pragma once
 
 #define NPW_THREADS 128
