@@ -1085,11 +1085,11 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
                                            c->nq, &S->qn[DC_NQN - 1], c->q[1], c->nqx, &S->nn[2], c->qcap, 1);
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[2], c->qcap, &S->nh[2], c->q[1], c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[3], c->qcap, NW_MAXIT);
+                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[3], c->qcap, NW_OVF_MAXIT);
     k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
                                            c->q[1], &S->qn[DC_NQN - 1], c->nq, c->nqx, &S->nn[4], c->qcap, 1);
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[4], c->qcap, &S->nh[3], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_MAXIT);
+                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_OVF_MAXIT);
     CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);

@@ -244,6 +244,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
 #define NW_STACK 12                 /* sub-leaves a lane may hold (3 levels of quartering) */
 #define NW_TICKETS 64                /* queue tickets a warp draws per atomic on the queue head */
+#define NW_OVF_MAXIT 12              /* evaluations a sub-leaf of an unconverged leaf may take (a quarter of the box) */
 #define NW_SEED_MAXIT 8              /* evaluations a seed solve may take */
 #define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
 
@@ -388,6 +389,11 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
         // ---- one evaluation per busy lane
         bool fin = false;
         dcn::NwResult R; R.dist = 0.0; R.cosv = 0.0; R.converged = 0;
+        // a solve that drags on looks, every 4th evaluation, whether its element has been found CUT meanwhile (by
+        // another of its pairs): nothing it could still find would matter then.  The solves that do not converge are
+        // almost all of this kind -- other patch pairs of an element the surface passes through, where the minimum
+        // is a curve of zeros and the Hessian is singular -- and each used to cost two extra launches of sub-leaves.
+        if (s.phase == 1 && s.iters >= 4 && (s.iters & 3) == 0 && u2d(__ldcg(best + (it.ak & 0x1fffffffu))) <= tau_exit) s.phase = 0;
         if (s.phase != 0) {
             // the leaf's box (dyadic, exact) is re-derived from the item every time instead of living in registers
             double uc, vc, hP, sc, tc, hQ;
@@ -412,7 +418,8 @@ __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const
                     // the next launch to spread over the machine: solved one after the other by this lane they were a
                     // serial chain of up to 5 x NW_MAXIT evaluations that the whole launch waited for (175 us of 690).
                     cnt.fail++;
-                    if (choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP)) {
+                    if (u2d(__ldcg(best + b)) <= tau_exit) { /* the element is CUT by now: no sub-leaves */ }
+                    else if (choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP)) {
                         if (ovf) resplit = true;
                         else if (sp + 4 <= NW_STACK) {
 #pragma unroll
