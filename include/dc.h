@@ -73,7 +73,7 @@ typedef struct {
     double tau_cut_rel; /* CUT threshold / L_ref; <= 0: default 1e-7 (A.3 L719; reading A3) */
     double d_band;      /* exact-distance band; <= 0: auto = max element Bezier-box diagonal (A5) */
     double l_ref;       /* reference length; <= 0: auto = longest edge of the surface-node AABB */
-    double theta_leaf;  /* subdivision stops when (patch size) x (curvature) <= theta; <= 0: 0.125 */
+    double theta_leaf;  /* subdivision stops when (patch size) x (curvature) <= theta; <= 0: 0.25 */
     int max_level;      /* subdivision bound per patch, 1..12; <= 0: default 12 */
     int flags;          /* DC_FLAG_* */
 } dc_params;

@@ -360,7 +360,7 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
     S->tol_d = 1e-13 * lref;
     S->d_band = P.d_band > 0.0 ? P.d_band : sqrt(__longlong_as_double((long long)S->grid_max_diag2));
     S->reach = S->d_band + 2.0 * S->tau + S->t_tie;
-    S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.125;
+    S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.25;
     S->max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->status = 0; S->n_pairs = 0ull;
     for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; S->nh[i] = 0; }

@@ -274,7 +274,7 @@ def test_parameters_theta_and_max_level_do_not_change_the_result(B):
     """The leaf rule (theta_leaf) and the subdivision bound (max_level) steer the work, not the answer."""
     w = make_config(2, N=16, n=8)
     l0, s0, st0 = gpu_cut(B, w)
-    for theta, ml in ((0.03, 12), (0.5, 12), (0.125, 3)):
+    for theta, ml in ((0.03, 12), (0.125, 12), (0.5, 12), (0.25, 3)):
         p = B.dc_params(); p.theta_leaf = theta; p.max_level = ml
         l1, s1, st1 = gpu_cut(B, w, params=p)
         assert np.array_equal(l0, l1) and np.abs(s0 - s1).max() <= 1e-11 * st0.l_ref, (theta, ml)
