@@ -28,7 +28,7 @@ using namespace dcg;
 #define DC_GRID_MAX 64              /* face-bin cells per axis (Morton code: 6 bits per axis) */
 #define DC_NCELL (DC_GRID_MAX * DC_GRID_MAX * DC_GRID_MAX)
 #define DC_NQN 28                   /* >= DC_MAX_ROUNDS + 2 */
-#define DC_GRID_ROUNDS 8             /* branch-and-bound rounds launched as grids; the rest run inside one CTA */
+#define DC_GRID_ROUNDS 4             /* branch-and-bound rounds launched as grids; the rest run inside one CTA */
 
 // ------------------------------------------------------------------------------------------
 // device-resident scalars and counters

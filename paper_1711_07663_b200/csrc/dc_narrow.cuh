@@ -16,7 +16,7 @@
 //   k_np_bound_tail one CTA             : the sparse late rounds, until one comes up empty
 //   k_np_decide     thread / band elem  : S6 (L215 nearest face and its normal; tie rule L294)
 //
-// Launch order (dc_classify): stage, newton(seeds), roots, bound x 8, bound_tail, newton(leaves),
+// Launch order (dc_classify): stage, newton(seeds), roots, bound x 4, bound_tail, newton(leaves),
 // [bound(overflow), newton] x 2, decide.  Every item of bound round r has lP + lQ = r, so 2 max_level + 1
 // rounds always terminate the branch and bound.
 #pragma once
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_TICKETS 64                /* queue tickets a warp draws per atomic on the queue head */
 #define NW_OVF_MAXIT 12              /* evaluations a sub-leaf of an unconverged leaf may take (a quarter of the box) */
 #define NW_SEED_MAXIT 8              /* evaluations a seed solve may take */
-#define NW_REFILL 4                 /* idle lanes that trigger a refill while others are still iterating */
+#define NW_REFILL 1                 /* idle lanes that trigger a refill while others are still iterating */
 
 __global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
                                                             const NItem *__restrict__ nq, const float4 *__restrict__ nqx,
