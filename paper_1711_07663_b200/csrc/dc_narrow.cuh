@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 #define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
 #define NW_STACK 12                 /* sub-leaves a lane may hold (3 levels of quartering) */
 #define NW_TICKETS 64                /* queue tickets a warp draws per atomic on the queue head */
-#define NW_OVF_MAXIT 12              /* evaluations a sub-leaf of an unconverged leaf may take (a quarter of the box) */
+#define NW_OVF_MAXIT 20              /* evaluations a sub-leaf of an unconverged leaf may take (a quarter of the box) */
 #define NW_SEED_MAXIT 8              /* evaluations a seed solve may take */
 #define NW_REFILL 1                 /* idle lanes that trigger a refill while others are still iterating */
 
