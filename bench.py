@@ -335,15 +335,17 @@ def main():
                 "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": ach_tf / fp64_peak if fp64_peak > 0 else None,
                 # dram__bytes_read.sum + dram__bytes_write.sum of its launches in the committed ncu --set full
-                # capture (profiles/r1c_kernels_full_config2.md: 48.5 + 0.5 and 133.0 + 7.4 MB, the overflow launches < 0.1 MB), config 2 only
-                "traffic": 189.4e6 if cfg in (2, 3) else None,
+                # capture (profiles/r1c_kernels_full_config2.md: 48.4 + 0.1 and 121.3 + 5.8 MB, the overflow launches < 0.1 MB), config 2 only
+                "traffic": 175.7e6 if cfg in (2, 3) else None,
                 "algorithmic_flops_per_cut": newton_flops, "ms_per_cut": newton_ms,
                 "peak_source": "measured: dc_measure_fp64_tflops (register-resident DFMA chains on all SMs) in this run",
                 "share_of_step": newton_ms / float(med[5] + med[6]) if med[5] > 0 else None,
                 "narrow_phase_S5_S6": {"ms": narrow_ms, "algorithmic_flops": narrow_flops,
                                        "achieved_tflops": narrow_flops / (narrow_ms * 1e-3) / 1e12 if narrow_ms > 0 else None}}
     roofline_s2 = {"kernel": "k_elem_boxes (S2)", "bound": "hbm", "achieved": ach_gbs, "peak": hbm_peak, "unit": "GB/s",
-                   "frac": ach_gbs / hbm_peak, "traffic": None, "peak_source": hbm_src}
+                   "frac": ach_gbs / hbm_peak,
+                   # same capture: 634.5 MB read + 92.2 MB written (algorithmic: 734 MB), config 2 only
+                   "traffic": 726.7e6 if cfg in (2, 3) else None, "algorithmic_bytes": s2_bytes, "peak_source": hbm_src}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
