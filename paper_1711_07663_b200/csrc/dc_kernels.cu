@@ -414,13 +414,27 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
             int i0[3], i1[3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) { i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c); }
+            // coarse to fine: most elements near the surface AABB sit in empty space, and at most 8 blocks two levels up
+            // say so; only the others look at the (<= 64) blocks k_pairs will walk
             const int sl = block_level(i0, i1);
-            for (int z = i0[2] >> sl; z <= (i1[2] >> sl) && !active; ++z)
-                for (int y = i0[1] >> sl; y <= (i1[1] >> sl) && !active; ++y)
-                    for (int x = i0[0] >> sl; x <= (i1[0] >> sl); ++x) {
-                        int first;
-                        if (block_faces(cell_start, x, y, z, sl, first) > 0) { active = true; break; }
-                    }
+            bool maybe = false;
+            {
+                int sc = sl;
+                while (sc < 7 && (((i1[0] >> sc) - (i0[0] >> sc)) > 1 || ((i1[1] >> sc) - (i0[1] >> sc)) > 1 || ((i1[2] >> sc) - (i0[2] >> sc)) > 1)) ++sc;
+                for (int z = i0[2] >> sc; z <= (i1[2] >> sc) && !maybe; ++z)
+                    for (int y = i0[1] >> sc; y <= (i1[1] >> sc) && !maybe; ++y)
+                        for (int x = i0[0] >> sc; x <= (i1[0] >> sc); ++x) {
+                            int first;
+                            if (block_faces(cell_start, x, y, z, sc, first) > 0) { maybe = true; break; }
+                        }
+            }
+            if (maybe)
+                for (int z = i0[2] >> sl; z <= (i1[2] >> sl) && !active; ++z)
+                    for (int y = i0[1] >> sl; y <= (i1[1] >> sl) && !active; ++y)
+                        for (int x = i0[0] >> sl; x <= (i1[0] >> sl); ++x) {
+                            int first;
+                            if (block_faces(cell_start, x, y, z, sl, first) > 0) { active = true; break; }
+                        }
         }
     }
     const unsigned m = __ballot_sync(0xffffffffu, active);
