@@ -672,15 +672,16 @@ __global__ void k_uf_union(const signed char *__restrict__ labels, const int *__
 __global__ void k_uf_seed(const DcScalars *S, const int *__restrict__ band_elem, const signed char *__restrict__ labels,
                           int *parent, unsigned char *comp)
 {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= min(S->n_band, S->max_band)) return;
-    const int e = band_elem[b];
-    const int lab = labels[e];
-    if (lab == DC_HOLE || lab == DC_NORMAL) {
-        const int r = uf_find(parent, e);
-        // byte-wide OR through a 32-bit atomic
-        unsigned *w = reinterpret_cast<unsigned *>(comp + (r & ~3));
-        atomicOr(w, (unsigned)(lab == DC_HOLE ? 1 : 2) << (8 * (r & 3)));
+    const int n_band = min(S->n_band, S->max_band);
+    for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < n_band; b += gridDim.x * blockDim.x) {
+        const int e = band_elem[b];
+        const int lab = labels[e];
+        if (lab == DC_HOLE || lab == DC_NORMAL) {
+            const int r = uf_find(parent, e);
+            // byte-wide OR through a 32-bit atomic
+            unsigned *w = reinterpret_cast<unsigned *>(comp + (r & ~3));
+            atomicOr(w, (unsigned)(lab == DC_HOLE ? 1 : 2) << (8 * (r & 3)));
+        }
     }
 }
 
@@ -1105,12 +1106,12 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[4], c->qcap, &S->nh[3], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
                                                        c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_OVF_MAXIT);
     CK(cudaEventRecord(c->ev[6], st));
-    k_np_decide<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
+    k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
     k_uf_local<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(labels_dev, c->adj, ne, c->parent);
     k_uf_union<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, c->adj, ne, c->parent);
-    k_uf_seed<<<nblk(c->max_band < ne ? c->max_band : ne, 256), 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
+    k_uf_seed<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
     k_uf_collect<<<nblk(ne, 256), 256, 0, st>>>(c->S, labels_dev, ne, c->parent, c->comp);
     k_seedless<<<DC_MAX_SEEDLESS, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);

@@ -625,10 +625,9 @@ __global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, con
                             signed char *__restrict__ labels, double *__restrict__ sdist)
 {
     const int n_band = min(S->n_band, S->max_band);
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
     const double tau = S->tau, tau_exit = S->tau_exit, amb = S->amb, t_tie = S->t_tie, d_band = S->d_band;
     unsigned n_amb = 0, n_samb = 0;
-    if (b < n_band) {
+    for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < n_band; b += gridDim.x * blockDim.x) {   // (n_band is only known on the device)
         const int e = band_elem[b];
         const double dmin = u2d(dmin_arr[b]);
         if (u2d(best[b]) <= tau_exit) { labels[e] = DC_CUT; sdist[e] = 0.0; }
