@@ -285,7 +285,7 @@ def test_element_permutation(B):
     """Elements renumbered at random (adjacency remapped): neighbours no longer have nearby ids, so the tile-local
     union-find pass settles almost nothing and every edge goes through the global forest; the labels and distances
     must simply be permuted."""
-    w = make_config(1, N=13, n=4)
+    w = make_config(1, N=22, n=5)                    # 10 648 elements: 11 tiles of the fill, all of them mixed up
     l0, s0, st0 = gpu_cut(B, w)
     rng = np.random.default_rng(8)
     perm = rng.permutation(w.n_elem)                 # new element i is old element perm[i]
