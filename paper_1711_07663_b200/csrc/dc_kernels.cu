@@ -467,6 +467,8 @@ __device__ __forceinline__ bool box_within(const double *lo, const double *hi, c
 
 #define PR_WARPS 8
 #define PR_CAP 224
+#define PR_W 16                     /* lanes per element: two elements in flight per warp (the walk is latency bound) */
+#define PR_GROUPS (PR_WARPS * 32 / PR_W)
 __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
                                                const int *__restrict__ act_elem, const int *__restrict__ cell_start,
                                                const double *__restrict__ fbox, long long max_pairs,
@@ -474,13 +476,16 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                                                int *__restrict__ band_cnt,
                                                int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key)
 {
-    __shared__ int s_list[PR_WARPS][PR_CAP];
-    __shared__ int s_off[PR_WARPS][33];
-    __shared__ int s_first[PR_WARPS][32];
-    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    __shared__ int s_list[PR_GROUPS][PR_CAP];
+    __shared__ int s_off[PR_GROUPS][PR_W + 1];
+    __shared__ int s_first[PR_GROUPS][PR_W];
+    // a GROUP of PR_W lanes per element; every warp primitive below is confined to the group's lanes
+    const int lane = threadIdx.x & (PR_W - 1), wl = threadIdx.x / PR_W;
+    const int gshift = (threadIdx.x & 31) & ~(PR_W - 1);
+    const unsigned gmask = (PR_W == 32 ? 0xffffffffu : ((1u << PR_W) - 1u)) << gshift;
     const unsigned lt_mask = (1u << lane) - 1u;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) / PR_W;
+    const int nwarps = (gridDim.x * blockDim.x) / PR_W;
     const int n_active = S->n_active;
     const double reach = S->reach, reach2 = reach * reach, pad = reach + S->fhalf;
     int *list = s_list[wl], *off = s_off[wl], *firsts = s_first[wl];
@@ -502,25 +507,25 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
         int total = 0;
         for (int phase = 0; phase < 2; ++phase) {
             int running = 0;
-            for (int bbase = 0; bbase < nblk; bbase += 32) {
+            for (int bbase = 0; bbase < nblk; bbase += PR_W) {
                 const int bi = bbase + lane;
                 int cnt = 0, first = 0;
                 if (bi < nblk) cnt = block_faces(cell_start, b0[0] + bi % nb[0], b0[1] + (bi / nb[0]) % nb[1], b0[2] + bi / (nb[0] * nb[1]), sl, first);
                 int incl = cnt;
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-                const int T = __shfl_sync(0xffffffffu, incl, 31);
+                for (int o = 1; o < PR_W; o <<= 1) { const int v = __shfl_up_sync(gmask, incl, o, PR_W); if (lane >= o) incl += v; }
+                const int T = __shfl_sync(gmask, incl, PR_W - 1, PR_W);
                 if (lane == 0) off[0] = 0;
                 off[lane + 1] = incl; firsts[lane] = first;
-                __syncwarp();
-                for (int j0 = 0; j0 < T; j0 += 32) {
+                __syncwarp(gmask);
+                for (int j0 = 0; j0 < T; j0 += PR_W) {
                     const int j = j0 + lane;
                     bool hit = false;
                     int p = -1;
                     if (j < T) {
                         int L = 0;                       // largest L with off[L] <= j
 #pragma unroll
-                        for (int st = 16; st > 0; st >>= 1) if (off[L + st] <= j) L += st;
+                        for (int st = PR_W / 2; st > 0; st >>= 1) if (off[L + st] <= j) L += st;
                         p = firsts[L] + (j - off[L]);
                         double fb[6];
 #pragma unroll
@@ -531,7 +536,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                         hit = box_within(lo, hi, fb, reach2);
                         if (phase == 0) ++tests;
                     }
-                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    const unsigned m = (__ballot_sync(gmask, hit) >> gshift) & (PR_W == 32 ? 0xffffffffu : ((1u << PR_W) - 1u));
                     const int pos = running + __popc(m & lt_mask);
                     if (hit) {
                         if (phase == 0) { if (pos < PR_CAP) list[pos] = p; }
@@ -539,7 +544,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                     }
                     running += __popc(m);
                 }
-                __syncwarp();
+                __syncwarp(gmask);
             }
             if (phase == 1) break;
             total = running;
@@ -553,18 +558,19 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                 }
                 base = b;
             }
-            base = __shfl_sync(0xffffffffu, base, 0);
+            base = __shfl_sync(gmask, base, 0, PR_W);
             if (base < 0 || total == 0) break;
             if (total <= PR_CAP) {
-                for (int i = lane; i < total; i += 32) { pair_face[base + i] = list[i]; pair_key[base + i] = 0x7ff0000000000000ull; }
+                for (int i = lane; i < total; i += PR_W) { pair_face[base + i] = list[i]; pair_key[base + i] = 0x7ff0000000000000ull; }
                 break;
             }
         }
-        __syncwarp();
+        __syncwarp(gmask);
     }
+    __syncwarp();
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(0xffffffffu, tests, o);
-    if (lane == 0 && tests) atomicAdd(&S->c_box_tests, tests);
+    if ((threadIdx.x & 31) == 0 && tests) atomicAdd(&S->c_box_tests, tests);
 }
 
 // ------------------------------------------------------------------------------------------
