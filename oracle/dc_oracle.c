@@ -644,13 +644,15 @@ int orc_classify(long long n_nodes, const double *xyz, long long n_elem, const i
         }
         int far = lb_min > d_band + t_tie;
         double eps = far ? eps_far : eps_near;
+        const double ub_nodes = ub;
         /* step 3b: every face whose box bound does not exceed the cutoff, nearest box first */
         long long nc = 0;
         for (long long f = 0; f < n_face; ++f)
             if (lbs[f] <= ub + t_tie) { cands[nc].lb = lbs[f]; cands[nc].f = (int)f; nc++; }
         qsort(cands, (size_t)nc, sizeof(cand), cand_cmp);
-        n_tie = 0;
         int is_cut = 0, depth_hit = 0;
+    redo:
+        n_tie = 0;
         for (long long ci = 0; ci < nc && !is_cut; ++ci) {
             double c = ub + t_tie;
             if (cands[ci].lb > c) break;
@@ -677,6 +679,12 @@ int orc_classify(long long n_nodes, const double *xyz, long long n_elem, const i
                 ties[n_tie].hi = R.hi; ties[n_tie].cosv = cosv; ties[n_tie].f = f; n_tie++;
             }
         }
+        /* The relaxed enclosure of a far element (SURVEY 8(c) "Far elements") only certifies a pair's minimum to
+         * eps_far, so PATCHPAIR may report "beyond the cutoff" for a pair whose minimum lies within eps_far below
+         * it; when the node-pair bound `ub` happens to be that sharp for EVERY pair, no tie member is left and
+         * step 5 would have no r.n to take a sign from.  The strict enclosure is the definition: redo the element
+         * with it (then hi <= d* + eps_near < ub + t_tie for the nearest pair, so the list cannot be empty). */
+        if (!is_cut && n_tie == 0 && eps != eps_near) { eps = eps_near; ub = ub_nodes; goto redo; }
         /* step 5: label */
         unsigned char fl = 0;
         if (far) { fl |= ORC_FLAG_FAR; S.n_far++; }
