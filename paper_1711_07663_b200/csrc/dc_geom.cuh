@@ -75,11 +75,19 @@ __device__ __forceinline__ unsigned cos_code(double cosv)
 // A node is a pair of dyadic sub-rectangles (centre, half-width) of a root patch pair given by
 // root monomial coefficients AP, AQ ([coord][9]) and the root constants KP, KQ (see
 // higher_order_const).  It returns
-//   dist_c : |P(centre) - Q(centre)|, attained by real points => an upper bound of the minimum;
-//   lb     : a lower bound of the distance over the node: with n = r/|r| (r = centre difference)
-//            min |P - Q| >= n.(P - Q) >= dist_c + min n.(P - Pc) - max n.(Q - Qc), the ranges of
-//            the two SCALAR biquadratics n.P, n.Q re-centred on the node (project first, re-centre
-//            the 8 non-constant scalar coefficients after: 3x cheaper than re-centring vectors);
+//   ub     : an ATTAINED distance (hence an upper bound of the minimum): the smaller of the centre distance and the
+//            distance of the TRUE patches at x0, the closest pair of the node's first-order model
+//            min |r_c + J a|, a in [-1,1]^4, J = [h P_u, h P_v, -h Q_s, -h Q_t] at the centre (a few sweeps of exact
+//            coordinate minimisation with the clamp of L272-L278: the model is a box-constrained 4-variable least
+//            squares problem whose J^T J is singular -- two patches can slide along each other -- so a plain
+//            Gauss-Newton step lands anywhere; the sweeps only ever decrease |r|);
+//   lb     : a lower bound of the distance over the node: for ANY unit n,
+//            min |P - Q| >= n.(P_c - Q_c) + min n.(P - P_c) - max n.(Q - Q_c); with n = r(x0)/|r(x0)|, the direction
+//            of the closest pair, the first-order part of the bound is tight (the centre direction loses 13 % of the
+//            distance in the median on config 2, this one 1 %), and the ranges of the two SCALAR biquadratics n.P,
+//            n.Q over the sub-rectangles come from their Bernstein coefficients (convex-hull property; exact for a
+//            bilinear function, where bounding term by term is not: the twist u v is coupled to u and v);
+//   x0     : that point in the node's local coordinates [-1,1]^4 (a leaf's solve starts there);
 //   leaf / splitP : the subdivision rule.  s1^2 = h^2 max(|P_u|^2,|P_v|^2) at the centre is the
 //            squared first-order size, s2 = h^2 K bounds the sum of the norms of the node's six
 //            higher-order coefficients.  leaf <=> max(kP,kQ) max(s1P,s1Q) <= theta, k = s2/s1^2,
@@ -116,29 +124,68 @@ __device__ __forceinline__ void eval_d1(const double *A, double u, double v, dou
     pu = fma(v, fma(v, d2, d1), d0);
 }
 
-// range [lo, hi] of the non-constant part of the scalar biquadratic g (g[0] ignored) over the
-// sub-rectangle (uc, vc, h): re-centre, then bound term by term.
+// value of one coordinate at (u,v)
+__device__ __forceinline__ double eval_d0(const double *A, double u, double v)
+{
+    const double r0 = fma(u, fma(u, A[2], A[1]), A[0]);
+    const double r1 = fma(u, fma(u, A[5], A[4]), A[3]);
+    const double r2 = fma(u, fma(u, A[8], A[7]), A[6]);
+    return fma(v, fma(v, r2, r1), r0);
+}
+
+// Bernstein coefficients on [-1,1] of a0 + a1 t + a2 t^2
+__device__ __forceinline__ void mono_to_bern(double a0, double a1, double a2, double &b0, double &b1, double &b2)
+{
+    const double s = a0 + a2;
+    b0 = s - a1; b1 = a0 - a2; b2 = s + a1;
+}
+
+// range [lo, hi] of the non-constant part of the scalar biquadratic g (g[0] ignored) over the sub-rectangle
+// (uc, vc, h): re-centre and scale to [-1,1]^2, convert to the Bernstein basis, take the smallest and the largest
+// of the 9 coefficients (the function lies in their convex hull).
 __device__ __forceinline__ void scalar_range(const double *g, double uc, double vc, double h, double &lo, double &hi)
 {
     const double h2 = h * h, uc2 = uc + uc, vc2 = vc + vc;
-    // rows j = 0,1,2 (powers of v): R_j0 (only j = 1,2 feed non-constant terms), R_j1, R_j2
+    // rows j = 0,1,2 (powers of v) re-centred in u: R_j0, R_j1, R_j2
     const double R01 = h * fma(uc2, g[2], g[1]), R02 = h2 * g[2];
     const double R10 = fma(uc, fma(uc, g[5], g[4]), g[3]), R11 = h * fma(uc2, g[5], g[4]), R12 = h2 * g[5];
     const double R20 = fma(uc, fma(uc, g[8], g[7]), g[6]), R21 = h * fma(uc2, g[8], g[7]), R22 = h2 * g[8];
-    const double c1 = fma(vc, fma(vc, R21, R11), R01);       // u
-    const double c2 = fma(vc, fma(vc, R22, R12), R02);       // u^2
-    const double c3 = h * fma(vc2, R20, R10);                // v
-    const double c4 = h * fma(vc2, R21, R11);                // u v
-    const double c5 = h * fma(vc2, R22, R12);                // u^2 v
-    const double c6 = h2 * R20, c7 = h2 * R21, c8 = h2 * R22; // v^2, u v^2, u^2 v^2
-    const double odd = fabs(c1) + fabs(c3) + fabs(c4) + fabs(c5) + fabs(c7);
-    lo = dmin2(0.0, c2) + dmin2(0.0, c6) + dmin2(0.0, c8) - odd;
-    hi = dmax2(0.0, c2) + dmax2(0.0, c6) + dmax2(0.0, c8) + odd;
+    // columns re-centred in v: c[j][i], constant term dropped
+    const double c01 = fma(vc, fma(vc, R21, R11), R01), c02 = fma(vc, fma(vc, R22, R12), R02);
+    const double c10 = h * fma(vc2, R20, R10), c11 = h * fma(vc2, R21, R11), c12 = h * fma(vc2, R22, R12);
+    const double c20 = h2 * R20, c21 = h2 * R21, c22 = h2 * R22;
+    // Bernstein in u (rows), then in v (columns)
+    double r0[3], r1[3], r2[3];
+    mono_to_bern(0.0, c01, c02, r0[0], r0[1], r0[2]);
+    mono_to_bern(c10, c11, c12, r1[0], r1[1], r1[2]);
+    mono_to_bern(c20, c21, c22, r2[0], r2[1], r2[2]);
+    lo = 0.0; hi = 0.0;                 // (the centre value, 0, is attained)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        double b0, b1, b2;
+        mono_to_bern(r0[i], r1[i], r2[i], b0, b1, b2);
+        lo = dmin2(lo, dmin2(b0, dmin2(b1, b2)));
+        hi = dmax2(hi, dmax2(b0, dmax2(b1, b2)));
+    }
 }
 
+// reciprocal of a positive normal-range double: hardware seed + two Newton steps (no slow path)
+__device__ __forceinline__ double rcp_pos(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = fma(fma(-x, y, 1.0), y, y);
+    y = fma(fma(-x, y, 1.0), y, y);
+    return y;
+}
+
+#ifndef DC_CD_SWEEPS
+#define DC_CD_SWEEPS 3
+#endif
+
 struct NodeOut {
-    double dist_c, lb; bool leaf, splitP;
-    double r[3], pu[3], pv[3], qs[3], qt[3];     // centre difference and first derivatives there (for the leaf's first step)
+    double ub, lb; bool leaf, splitP;
+    double x0[4];                                  // closest pair of the first-order model, local coordinates
 };
 
 __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ, double KP, double KQ,
@@ -154,32 +201,69 @@ __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ
         r[c] = p - q;
     }
     NodeOut o;
+    const double d2c = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+    // subdivision rule (squared form)
+    const double hP2 = hP * hP, hQ2 = hQ * hQ;
+    const double npu = pu[0] * pu[0] + pu[1] * pu[1] + pu[2] * pu[2], npv = pv[0] * pv[0] + pv[1] * pv[1] + pv[2] * pv[2];
+    const double nqs = qs[0] * qs[0] + qs[1] * qs[1] + qs[2] * qs[2], nqt = qt[0] * qt[0] + qt[1] * qt[1] + qt[2] * qt[2];
+    {
+        const double S1P = hP2 * dmax2(npu, npv), S1Q = hQ2 * dmax2(nqs, nqt);
+        const double s2P = hP2 * KP, s2Q = hQ2 * KQ;
+        const double M = dmax2(S1P, S1Q);
+        const bool okP = !(S1P > 0.0) || s2P * s2P * M <= theta2 * S1P * S1P;
+        const bool okQ = !(S1Q > 0.0) || s2Q * s2Q * M <= theta2 * S1Q * S1Q;
+        o.leaf = okP && okQ;
+        o.splitP = S1P >= S1Q;
+    }
+    // closest pair of the first-order model: exact coordinate minimisation with clamping, rho = r_c + J a
+    double a[4] = { 0.0, 0.0, 0.0, 0.0 };
+    {
+        const double sc4[4] = { hP, hP, -hQ, -hQ };
+        const double *col[4] = { pu, pv, qs, qt };
+        const double nrm[4] = { hP2 * npu, hP2 * npv, hQ2 * nqs, hQ2 * nqt };
+        double inv[4];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { o.r[c] = r[c]; o.pu[c] = pu[c]; o.pv[c] = pv[c]; o.qs[c] = qs[c]; o.qt[c] = qt[c]; }
-    const double d2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
-    const double inv = d2 > 0.0 ? rsqrt(d2) : 0.0;
-    o.dist_c = d2 * inv;
-    const double n0 = r[0] * inv, n1 = r[1] * inv, n2 = r[2] * inv;
+        for (int i = 0; i < 4; ++i) inv[i] = nrm[i] > 1e-300 ? rcp_pos(nrm[i]) * sc4[i] : 0.0;
+        double rho[3] = { r[0], r[1], r[2] };
+#pragma unroll
+        for (int sw = 0; sw < DC_CD_SWEEPS; ++sw)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const double *J = col[i];
+                const double dot = J[0] * rho[0] + J[1] * rho[1] + J[2] * rho[2];      // (J_i . rho) / h_i
+                double t = fma(-dot, inv[i], a[i]);
+                t = dmax2(-1.0, dmin2(1.0, t));
+                const double da = (t - a[i]) * sc4[i];
+                rho[0] = fma(J[0], da, rho[0]); rho[1] = fma(J[1], da, rho[1]); rho[2] = fma(J[2], da, rho[2]);
+                a[i] = t;
+            }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) o.x0[i] = a[i];
+    // the true patches at x0
+    const double u0 = fma(hP, a[0], uc), v0 = fma(hP, a[1], vc), s0 = fma(hQ, a[2], sc), t0 = fma(hQ, a[3], tc);
+    double r0[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) r0[c] = eval_d0(AP + 9 * c, u0, v0) - eval_d0(AQ + 9 * c, s0, t0);
+    const double d20 = r0[0] * r0[0] + r0[1] * r0[1] + r0[2] * r0[2];
+    // direction of the bound: the closest pair's (the centre's if the patches touch there)
+    const bool use0 = d20 > 0.0;
+    const double dd = use0 ? d20 : d2c;
+    const double inv = dd > 0.0 ? rsqrt(dd) : 0.0;
+    const double n[3] = { (use0 ? r0[0] : r[0]) * inv, (use0 ? r0[1] : r[1]) * inv, (use0 ? r0[2] : r[2]) * inv };
+    // attained distances, rounded up (sqrt of the smaller square)
+    const double dmin = dmin2(d20, d2c);
+    o.ub = sqrt(dmin) * (1.0 + 4e-16);
     double gP[9], gQ[9];
 #pragma unroll
     for (int m = 1; m < 9; ++m) {
-        gP[m] = fma(n2, AP[18 + m], fma(n1, AP[9 + m], n0 * AP[m]));
-        gQ[m] = fma(n2, AQ[18 + m], fma(n1, AQ[9 + m], n0 * AQ[m]));
+        gP[m] = fma(n[2], AP[18 + m], fma(n[1], AP[9 + m], n[0] * AP[m]));
+        gQ[m] = fma(n[2], AQ[18 + m], fma(n[1], AQ[9 + m], n[0] * AQ[m]));
     }
     double loP, hiP, loQ, hiQ;
     scalar_range(gP, uc, vc, hP, loP, hiP);
     scalar_range(gQ, sc, tc, hQ, loQ, hiQ);
-    o.lb = o.dist_c + loP - hiQ;
-    // subdivision rule (squared form)
-    const double hP2 = hP * hP, hQ2 = hQ * hQ;
-    const double S1P = hP2 * dmax2(pu[0] * pu[0] + pu[1] * pu[1] + pu[2] * pu[2], pv[0] * pv[0] + pv[1] * pv[1] + pv[2] * pv[2]);
-    const double S1Q = hQ2 * dmax2(qs[0] * qs[0] + qs[1] * qs[1] + qs[2] * qs[2], qt[0] * qt[0] + qt[1] * qt[1] + qt[2] * qt[2]);
-    const double s2P = hP2 * KP, s2Q = hQ2 * KQ;
-    const double M = dmax2(S1P, S1Q);
-    const bool okP = !(S1P > 0.0) || s2P * s2P * M <= theta2 * S1P * S1P;
-    const bool okQ = !(S1Q > 0.0) || s2Q * s2Q * M <= theta2 * S1Q * S1Q;
-    o.leaf = okP && okQ;
-    o.splitP = S1P >= S1Q;
+    o.lb = fma(n[2], r[2], fma(n[1], r[1], n[0] * r[0])) + loP - hiQ;
     return o;
 }
 

@@ -751,7 +751,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                 nitem_box(it, uc, vc, hP, sc, tc, hQ);
                 const NodeOut nb = bound_node(AP, AQ, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
                 double best = u2d(s_best);
-                if (nb.dist_c < best) { atomicMin(&s_best, d2u(nb.dist_c)); best = nb.dist_c; }
+                if (nb.ub < best) { atomicMin(&s_best, d2u(nb.ub)); best = nb.ub; }
                 if (nb.lb > best + t_tie) continue;
                 bool leaf = nb.leaf, splitP = false;
                 if (!leaf) leaf = !choose_split(it, nb.splitP, max_level, splitP);
@@ -856,7 +856,7 @@ struct dc_ctx {
     int *act_elem;
     int *band_elem; long long *band_start; int *band_cnt;
     double *ecoef, *pbox; unsigned long long *best, *dmin;
-    NItem *q[2], *nq; float4 *nqx;
+    NItem *q[2], *nq; NLeafX *nqx;
     int *pair_face; unsigned long long *pair_key;
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
     int *cell_count, *cell_start, *cell_fill;
@@ -908,7 +908,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_q0 = take((size_t)L.qcap * sizeof(NItem));
     L.off_q1 = take((size_t)L.qcap * sizeof(NItem));
     L.off_nq = take((size_t)(L.qcap > L.max_band ? L.qcap : L.max_band) * sizeof(NItem));
-    L.off_nqx = take((size_t)(L.qcap > L.max_band ? L.qcap : L.max_band) * sizeof(float4));
+    L.off_nqx = take((size_t)(L.qcap > L.max_band ? L.qcap : L.max_band) * sizeof(NLeafX));
     // pair arrays double as the scratch of the adjacency derivation (2 x n_nodes ints)
     size_t pf = (size_t)max_pairs * 4, pk = (size_t)max_pairs * 8;
     size_t need_adj = (size_t)n_nodes * 8;
@@ -989,7 +989,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->q[0] = (NItem *)(c->ws + L.off_q0);
     c->q[1] = (NItem *)(c->ws + L.off_q1);
     c->nq = (NItem *)(c->ws + L.off_nq);
-    c->nqx = (float4 *)(c->ws + L.off_nqx);
+    c->nqx = (NLeafX *)(c->ws + L.off_nqx);
     c->pair_face = (int *)(c->ws + L.off_pair_face);
     c->pair_key = (unsigned long long *)(c->ws + L.off_pair_key);
     c->fbox_orig = (double *)(c->ws + L.off_fbox_orig);
@@ -1006,8 +1006,6 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     for (int i = 0; i < 12; ++i) CK(cudaEventCreate(&c->ev[i]));
-    CK(cudaFuncSetAttribute(k_np_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, NW_SMEM_BYTES));
-    CK(cudaFuncSetAttribute(k_np_newton, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
     int rc = run_elem_boxes(c, st);
@@ -1078,10 +1076,10 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
                                            c->ecoef, c->pbox, c->best, c->dmin, c->nq);
     // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
     // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
-    const int gn = c->num_sms * 4;     // persistent Newton warps: 4 CTAs of 128 threads per SM (shared-memory bound)
+    const int gs = c->num_sms * 2 * 4;     // solve grids: grid-stride, 2 resident CTAs of 128 threads per SM
     CK(cudaEventRecord(c->ev[7], st));
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->n_band, c->max_band, &S->nh[0], c->nq, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_SEED_MAXIT);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT);
     CK(cudaEventRecord(c->ev[10], st));
     k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
                                            c->q[0], &S->qn[0], c->qcap);
@@ -1096,21 +1094,32 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     if (rounds > grid_rounds)
         k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                        c->nq, c->nqx, &S->nn[0], c->qcap);
-    // all leaves in one launch; an unconverged leaf is quartered and finished by the lane that held it
+    // all leaves: first dropped if their element's best distance has fallen below their lower bound meanwhile (the two
+    // bound queues are free by now and take the compacted leaf queue), then three solve passes (the old leaf queue's
+    // memory holds the continuations and the overflow queue of sub-leaves)
     CK(cudaEventRecord(c->ev[5], st));
-    // The sub-leaves of unconverged solves go to an overflow queue (the bound queues are free by now) and come back
-    // through one bound pass (best[b] is final or nearly so: most of them are pruned) and one Newton launch, twice;
-    // the last launch finishes whatever still fails on the lane that held it.
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[0], c->qcap, &S->nh[1], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[1], c->qcap, NW_MAXIT);
-    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                           c->nq, &S->qn[DC_NQN - 1], c->q[1], c->nqx, &S->nn[2], c->qcap, 1);
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[2], c->qcap, &S->nh[2], c->q[1], c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, c->q[0], &S->nn[3], c->qcap, NW_OVF_MAXIT);
-    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                           c->q[1], &S->qn[DC_NQN - 1], c->nq, c->nqx, &S->nn[4], c->qcap, 1);
-    k_np_newton<<<gn, NW_THREADS, NW_SMEM_BYTES, st>>>(S, &S->nn[4], c->qcap, &S->nh[3], c->nq, c->nqx, c->pair_face, c->fcoef, c->ecoef,
-                                                       c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, NW_OVF_MAXIT);
+    NItem *lq = c->q[0]; NLeafX *lqx = (NLeafX *)c->q[1];
+    NCont *contA = (NCont *)c->nq, *contB = (NCont *)c->nqx;
+    const long long capA = c->qcap / 4, capB = c->qcap / 8;
+    NItem *ovf1 = (NItem *)c->nqx + c->qcap / 2;
+    const long long cap_ovf1 = c->qcap / 2;
+    k_np_compact<<<c->num_sms * 8, 256, 0, st>>>(S, &S->nn[0], c->qcap, c->nq, c->nqx, c->best, lq, lqx, &S->nn[5]);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[5], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, contA, &S->nh[0], capA, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET1, NW_MAXIT);
+    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[0], capA, nullptr, nullptr, contA, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, contB, &S->nh[1], capB, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET2, NW_MAXIT);
+    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[1], capB, nullptr, nullptr, contB, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, ovf1, &S->nn[1], cap_ovf1, 0, NW_MAXIT);
+    // The sub-leaves of unconverged solves come back through one bound pass (best[b] is final or nearly so: most of them
+    // are pruned) and one solve launch, twice; the last launch finishes whatever still fails on the lane that held it.
+    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[2], c->qcap, 1);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[2], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, c->nq, &S->nn[3], c->qcap, 0, NW_OVF_MAXIT);
+    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[4], c->qcap, 1);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[4], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_OVF_MAXIT);
     CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
@@ -1123,7 +1132,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
-    c->launches_classify = 18 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
+    c->launches_classify = 21 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }

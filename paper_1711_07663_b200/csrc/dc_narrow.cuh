@@ -30,6 +30,11 @@ struct __align__(16) NItem { unsigned p, ak, w2, w3; };
 // w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20
 // w3: is(12) | it(12)<<12 | flags(8)<<24      flags bit0: seed solve (no re-split on failure)
 
+// what a leaf carries beside its item (16 bytes): the starting point of its solve (the first step k_np_bound took from
+// the centre, local coordinates in [-1,1] as 16-bit fixed point: +-32767 = on the bound) and its lower bound (the solve
+// is skipped when the element's best distance has dropped below it by the time a lane picks it up)
+struct __align__(16) NLeafX { short x[4]; double lb; };
+
 struct NpCounters { unsigned nodes, newton, iters, fail, depth; };
 
 __device__ __forceinline__ double u2d(unsigned long long b) { return __longlong_as_double((long long)b); }
@@ -232,209 +237,217 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const do
 }
 
 // ------------------------------------------------------------------------------------------
-// Newton: PERSISTENT warps over the leaf queue nq[0 .. *n_items), one solve per lane, all lanes of a warp
-// in lockstep (dcn::iterate = exactly one value+gradient+Hessian evaluation), lanes whose solve has
-// finished are refilled from the queue (one warp-aggregated atomic on *head), so the iteration count of
-// one solve never holds up the other 31.  The two patches' 54 root monomial coefficients of every lane
-// live in shared memory, transposed (coefficient-major, lane-minor: conflict-free reads), which keeps the
-// kernel at <= 128 registers and 16 warps per SM; a refill is a warp-cooperative coalesced copy of the
-// 2 x 216 B of the new item (the odd stride makes the transposed store 2-way conflicted instead of 32).
+// Solve: projected Newton (dc_newton.cuh), ONE THREAD PER LEAF, both patches' 54 root monomial coefficients in
+// REGISTERS (two CTAs of 128 threads per SM at <= 255 registers: the FP64 pipe issues one warp instruction every other
+// cycle, so two warps per scheduler with the instruction-level parallelism of six independent jets keep it busy; no
+// shared memory, no refill machinery).  Iteration counts differ between the lanes of a warp (2 to 5 evaluations from the
+// starting point k_np_bound hands over, rarely many more), so a pass gives every solve a BUDGET of evaluations; a solve
+// that needs more is handed, with its state, to the next pass through a continuation queue (64 bytes), where it
+// meets other long solves: three passes (budgets NW_BUDGET1, NW_BUDGET2, the rest) keep the lanes of every pass busy.
+// Unconverged leaves (NW_MAXIT evaluations, or a stalled step) keep their attained distance as an upper bound and
+// are quartered: the four sub-leaves go to an overflow queue, back through one k_np_bound pass (best[b] is final by
+// then: most are pruned) and one more solve launch, twice; the last launch finishes what still fails from a small
+// local stack.
 #define NW_THREADS 128
-#define NW_STRIDE 129
-#define NW_SMEM_BYTES (54 * NW_STRIDE * 8)
-#define NW_STACK 12                 /* sub-leaves a lane may hold (3 levels of quartering) */
-#define NW_TICKETS 64                /* queue tickets a warp draws per atomic on the queue head */
+#define NW_STACK 12                 /* sub-leaves a lane of the last launch may hold (3 levels of quartering) */
+#ifndef NW_OVF_MAXIT
 #define NW_OVF_MAXIT 20              /* evaluations a sub-leaf of an unconverged leaf may take (a quarter of the box) */
+#endif
 #define NW_SEED_MAXIT 8              /* evaluations a seed solve may take */
-#define NW_REFILL 1                 /* idle lanes that trigger a refill while others are still iterating */
+#ifndef NW_BUDGET1
+#define NW_BUDGET1 20                 /* busy lanes below which a warp of pass 1 hands its stragglers on */
+#endif
+#ifndef NW_BUDGET2
+#define NW_BUDGET2 12
+#endif
 
-__global__ void __launch_bounds__(NW_THREADS, 4) k_np_newton(DcScalars *S, const int *__restrict__ n_items, long long in_cap, int *head,
-                                                            const NItem *__restrict__ nq, const float4 *__restrict__ nqx,
-                                                            const int *__restrict__ pair_face, const double *__restrict__ fcoef,
-                                                            const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                            unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
-                                                            NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap, int maxit)
+struct __align__(16) NCont { NItem it; double x[4]; double lb; short iters, ls, phase, pad; };
+
+// warp-aggregated append of one entry per lane that asks; -1 if the queue is full (no status bit: the caller copes)
+__device__ __forceinline__ long long warp_reserve_try(int *counter, int per, long long cap)
 {
-    extern __shared__ double nw_sm[];
+    const unsigned m = __activemask();           // (every lane that calls wants `per` entries)
+    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(counter, __popc(m) * per);
+    base = __shfl_sync(m, base, leader);
+    const long long slot = (long long)base + (long long)__popc(m & ((1u << lane) - 1)) * per;
+    return slot + per <= cap ? slot : -1;
+}
+
+// Leaves are queued with the lower bound they had when k_np_bound met them; by the end of the branch and bound the
+// element's best distance has usually dropped below most of them (two thirds at config 2).  One streaming pass drops
+// those (and the leaves of elements found CUT) so that the solve launches get dense warps.
+__global__ void __launch_bounds__(256) k_np_compact(const DcScalars *S, const int *__restrict__ n_in, long long in_cap,
+                                                    const NItem *__restrict__ nq, const NLeafX *__restrict__ nqx,
+                                                    const unsigned long long *__restrict__ best,
+                                                    NItem *__restrict__ nq_out, NLeafX *__restrict__ nqx_out, int *__restrict__ n_out)
+{
+    const int n = min(*n_in, (int)min(in_cap, (long long)0x7fffffff));
+    const double tau_exit = S->tau_exit, t_tie = S->t_tie;
+    const int n_round = (n + 31) & ~31;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += gridDim.x * blockDim.x) {
+        bool keep = false;
+        uint4 w = make_uint4(0, 0, 0, 0), xw = make_uint4(0, 0, 0, 0);
+        if (i < n) {
+            w = __ldg(reinterpret_cast<const uint4 *>(nq + i));
+            xw = __ldg(reinterpret_cast<const uint4 *>(nqx + i));
+            const double bst = u2d(__ldcg(best + (w.y & 0x1fffffffu)));
+            keep = bst > tau_exit && __hiloint2double((int)xw.w, (int)xw.z) <= bst + t_tie;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, keep);
+        if (!m) continue;
+        const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(n_out, __popc(m));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (keep) {
+            const int sl = base + __popc(m & ((1u << lane) - 1));
+            reinterpret_cast<uint4 *>(nq_out)[sl] = w;
+            reinterpret_cast<uint4 *>(nqx_out)[sl] = xw;
+        }
+    }
+}
+
+// MODE 0: items are leaves (nq + nqx: starting point and lower bound; nqx == nullptr: seeds, started at the centre)
+// MODE 1: items are continuations (cin)
+template <int MODE>
+__global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const int *__restrict__ n_items, long long in_cap,
+                                                           const NItem *__restrict__ nq, const NLeafX *__restrict__ nqx,
+                                                           const NCont *__restrict__ cin,
+                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
+                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
+                                                           unsigned long long *__restrict__ dmin, unsigned long long *__restrict__ pair_key,
+                                                           NCont *__restrict__ cout, int *__restrict__ cout_n, long long cout_cap,
+                                                           NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap,
+                                                           int budget, int maxit)
+{
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
-    if (n == 0) return;
-    const int tid = threadIdx.x, lane = tid & 31;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    const double *slot = nw_sm + tid;
-    const volatile double *vslot = slot;   // volatile: re-read in the line search instead of keeping 54 values live
-    auto cf = [&](int m) { return vslot[m * NW_STRIDE]; };
-    const double tau_exit = S->tau_exit, tol_d2 = S->tol_d * S->tol_d;
+    const double tau_exit = S->tau_exit, tol_d2 = S->tol_d * S->tol_d, t_tie = S->t_tie;
     const double tau_exit2 = tau_exit > 0.0 ? tau_exit * tau_exit : -1.0;
     const int max_level = S->max_level;
     NpCounters cnt = { 0, 0, 0, 0, 0 };
-    dcn::NwState s; s.phase = 0; s.iters = 0; s.ls = 0;
+    const int stride = gridDim.x * blockDim.x;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        NItem it;
+        dcn::NwState s; s.iters = 0; s.ls = 0; s.phase = 1;
+        double lb = 0.0;
+        int a4[4] = { 0, 0, 0, 0 };
+        if (MODE == 0) {
+            const uint4 w = __ldg(reinterpret_cast<const uint4 *>(nq + i));
+            it.p = w.x; it.ak = w.y; it.w2 = w.z; it.w3 = w.w;
+            if (nqx) {
+                const uint4 xw = __ldg(reinterpret_cast<const uint4 *>(nqx + i));
+                a4[0] = (short)(xw.x & 0xffff); a4[1] = (short)(xw.x >> 16); a4[2] = (short)(xw.y & 0xffff); a4[3] = (short)(xw.y >> 16);
+                lb = __hiloint2double((int)xw.w, (int)xw.z);
+            }
+        } else {
+            const uint4 *cp = reinterpret_cast<const uint4 *>(cin + i);
+            const uint4 w = __ldg(cp), x01 = __ldg(cp + 1), x23 = __ldg(cp + 2), st = __ldg(cp + 3);
+            it.p = w.x; it.ak = w.y; it.w2 = w.z; it.w3 = w.w;
+            s.x[0] = __hiloint2double((int)x01.y, (int)x01.x); s.x[1] = __hiloint2double((int)x01.w, (int)x01.z);
+            s.x[2] = __hiloint2double((int)x23.y, (int)x23.x); s.x[3] = __hiloint2double((int)x23.w, (int)x23.z);
+            lb = __hiloint2double((int)st.y, (int)st.x);
+            s.iters = (int)(st.z & 0xffff); s.ls = (int)(st.z >> 16); s.phase = (int)(st.w & 0xffff);
+        }
+        const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+        const double bst0 = u2d(__ldcg(best + b));
+        // dropped: the element is already CUT, or its best distance is below this leaf's lower bound by now
+        if (!(bst0 > tau_exit) || lb > bst0 + t_tie) continue;
+        double AP[28], AQ[28];
+        {
+            const double2 *APg = reinterpret_cast<const double2 *>(ecoef + ((size_t)b * 6 + k) * 28);
+            const double2 *AQg = reinterpret_cast<const double2 *>(fcoef + (size_t)__ldg(pair_face + it.p) * 28);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) s.x[i] = 0.0;
-    NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
-    NItem nxt; nxt.p = nxt.ak = nxt.w2 = nxt.w3 = 0;       // prefetched next item of this lane
-    // 0 no ticket, 2 ticket in hand, 3 item asked for, 4 face id and best[b] asked for (ready), 9 queue exhausted
-    int nst = 0, nface = 0, tk = 0, pbase = 0;
-    int pool_next = 0, pool_end = 0;    // (warp-uniform) tickets this warp holds
-    // tickets per draw: half a warp's share of the queue, between 8 and NW_TICKETS (short queues stay spread out)
-    const int chunk = max(8, min(NW_TICKETS, n / (int)(gridDim.x * (NW_THREADS / 32) * 2)));
-    unsigned long long nbest = 0;
-    float4 nx0 = make_float4(0.f, 0.f, 0.f, 0.f);   // its starting point (local coordinates; zero = the centre, for seeds)
-    bool pend = false;              // (warp-uniform) a ticket atomic is in flight
-    NItem stk[NW_STACK];            // sub-leaves of an unconverged solve, solved by the same lane (local memory, rarely touched)
-    int sp = 0;
-    while (true) {
-        // ---- a lane with sub-leaves of its own goes on with those (same pair: its coefficients are already in place)
-        if (s.phase == 0 && sp > 0) {
-            it = stk[--sp];
-            double uc, vc, hP, sc, tc, hQ;
-            nitem_box(it, uc, vc, hP, sc, tc, hQ);
-            s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
-            s.iters = 0; s.ls = 0; s.phase = 1;
-        }
-        // ---- every lane runs a small pipeline that fetches its NEXT item while it solves the current one, one
-        // stage per trip, so that no trip waits for more than one memory round trip: ticket (warp-aggregated
-        // atomic) -> item -> face id, best[b], L2 prefetch of the element coefficients -> ready.
-        if (nst == 3) {
-            const unsigned nb = nxt.ak & 0x1fffffffu;
-            nface = __ldg(pair_face + nxt.p);
-            nbest = __ldcg(best + nb);
-            const char *pn = reinterpret_cast<const char *>(ecoef + ((size_t)nb * 6 + (nxt.ak >> 29)) * 28);
-            asm volatile("prefetch.global.L2 [%0];" :: "l"(pn));
-            asm volatile("prefetch.global.L2 [%0];" :: "l"(pn + 128));
-            nst = 4;
-        } else if (nst == 2) {
-            if (tk >= n) nst = 9;
-            else {
-                const uint4 w = __ldg(reinterpret_cast<const uint4 *>(nq + tk));
-                nxt.p = w.x; nxt.ak = w.y; nxt.w2 = w.z; nxt.w3 = w.w;
-                if (nqx) nx0 = __ldg(nqx + tk);
-                nst = 3;
+            for (int m = 0; m < 14; ++m) {
+                const double2 vp = __ldg(APg + m), vq = __ldg(AQg + m);
+                AP[2 * m] = vp.x; AP[2 * m + 1] = vp.y; AQ[2 * m] = vq.x; AQ[2 * m + 1] = vq.y;
             }
         }
-        if (pend) {                                   // (uniform) the ticket atomic of an earlier trip has landed
-            pool_next = __shfl_sync(0xffffffffu, pbase, 0);
-            pool_end = pool_next + chunk;
-            pend = false;
+        auto cf = [&](int m) { return m < 27 ? AP[m] : AQ[m - 27]; };
+        double uc, vc, hP, sc, tc, hQ;
+        nitem_box(it, uc, vc, hP, sc, tc, hQ);
+        double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };
+        if (MODE == 0) {
+            // start at the closest pair of the leaf's first-order model (on a bound when the fixed point says so)
+            const double q15 = 1.0 / 32767.0;
+            const double cen[4] = { uc, vc, sc, tc }, hw[4] = { hP, hP, hQ, hQ };
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                s.x[j] = a4[j] >= 32767 ? hi[j] : (a4[j] <= -32767 ? lo[j] : fma(hw[j] * q15, (double)a4[j], cen[j]));
         }
-        // ---- idle lanes whose next item is ready take it
-        bool fresh = false;
-        unsigned long long pA = 0, pQ = 0;
-        {
-            const bool ready = s.phase == 0 && nst == 4;
-            const unsigned mready = __ballot_sync(0xffffffffu, ready);
-            const unsigned mbusy = __ballot_sync(0xffffffffu, s.phase != 0);
-            if (mready && (__popc(mready) >= NW_REFILL || mbusy == 0)) {
-                if (ready) {
-                    it = nxt; nst = 0;
-                    if (u2d(nbest) > tau_exit) {      // else: the element is already CUT, drop the item
-                        const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
-                        fresh = true;
-                        double uc, vc, hP, sc, tc, hQ;
-                        nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                        // start at the first step k_np_bound took from the centre (local coordinates; on a bound when within float rounding of it)
-                        const double a0 = nx0.x, a1 = nx0.y, a2 = nx0.z, a3 = nx0.w, e1 = 1.0 - 1e-6;
-                        s.x[0] = a0 >= e1 ? uc + hP : (a0 <= -e1 ? uc - hP : fma(hP, a0, uc));
-                        s.x[1] = a1 >= e1 ? vc + hP : (a1 <= -e1 ? vc - hP : fma(hP, a1, vc));
-                        s.x[2] = a2 >= e1 ? sc + hQ : (a2 <= -e1 ? sc - hQ : fma(hQ, a2, sc));
-                        s.x[3] = a3 >= e1 ? tc + hQ : (a3 <= -e1 ? tc - hQ : fma(hQ, a3, tc));
-                        s.iters = 0; s.ls = 0; s.phase = 1;
-                        pA = (unsigned long long)(ecoef + ((size_t)b * 6 + k) * 28);
-                        pQ = (unsigned long long)(fcoef + (size_t)nface * 28);
-                    }
+        const bool seed = (it.w3 >> 24) & 1;
+        NItem stk[NW_STACK];            // (last launch only: sub-leaves of an unconverged solve; local memory, rarely touched)
+        int sp = 0;
+        int left = maxit;
+        while (true) {
+            dcn::NwResult R; R.dist = 0.0; R.cosv = 0.0; R.converged = 0;
+            bool fin = false, dropped = false;
+            while (left > 0 && !fin) {
+                // a solve that drags on looks, every 4th evaluation, whether its element has been found CUT meanwhile (by
+                // another of its pairs), or its best distance has dropped below this leaf's lower bound: nothing it could
+                // still find would matter then
+                if (s.iters >= 4 && (s.iters & 3) == 0) {
+                    const double bnow = u2d(__ldcg(best + b));
+                    if (bnow <= tau_exit || lb > bnow + t_tie) { dropped = true; break; }
                 }
+                fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R, maxit);
+                --left;
+                // the budget of a pass is not a number of evaluations but a number of busy lanes: a warp goes on while at
+                // least `budget` of its lanes are still iterating, then hands the stragglers to the next pass
+                if (!fin && cout && __popc(__activemask()) < budget) left = 0;
             }
-        }
-        // ---- lanes without a next item draw a ticket from the warp's pool; the pool is refilled NW_TICKETS at a time by
-        // one atomic on the queue head whose result is looked at on a later trip (a ticket per lane per trip from the
-        // head itself made 2 368 warps queue up on ONE address: the kernel ran at the pace of that atomic)
-        {
-            const unsigned m0 = __ballot_sync(0xffffffffu, nst == 0);
-            if (m0) {
-                const int avail = pool_end - pool_next, rank = __popc(m0 & lt_mask);
-                if (nst == 0 && rank < avail) { tk = pool_next + rank; nst = 2; }
-                pool_next += min(__popc(m0), avail);
+            if (dropped) break;
+            if (!fin) {
+                // out of budget: hand the solve to the next pass (or go on here if its queue is full)
+                const long long sl = cout ? warp_reserve_try(cout_n, 1, cout_cap) : -1;
+                if (sl >= 0) {
+                    uint4 *cp = reinterpret_cast<uint4 *>(cout + sl);
+                    cp[0] = make_uint4(it.p, it.ak, it.w2, it.w3);
+                    cp[1] = make_uint4((unsigned)__double2loint(s.x[0]), (unsigned)__double2hiint(s.x[0]), (unsigned)__double2loint(s.x[1]), (unsigned)__double2hiint(s.x[1]));
+                    cp[2] = make_uint4((unsigned)__double2loint(s.x[2]), (unsigned)__double2hiint(s.x[2]), (unsigned)__double2loint(s.x[3]), (unsigned)__double2hiint(s.x[3]));
+                    cp[3] = make_uint4((unsigned)__double2loint(lb), (unsigned)__double2hiint(lb), (unsigned)s.iters | ((unsigned)s.ls << 16), (unsigned)s.phase);
+                    break;
+                }
+                left = maxit;
+                continue;
             }
-            if (pool_next == pool_end && !pend) {
-                if (lane == 0) pbase = atomicAdd(head, chunk);
-                pend = true;
-            }
-        }
-        // ---- the new items' coefficients go into their lanes' slots by asynchronous copies (cp.async, 8 bytes per
-        // lane), ALL issued before the one wait, so the new lanes of a trip cost one memory round trip together.
-        // Warp-cooperative: the warp copies one new lane's 2 x 216 contiguous bytes at a time (~5 L1 wavefronts per new
-        // lane; every new lane copying its own 54 coefficients cost 54, and the L1 data pipe -- shared-memory reads
-        // of the coefficients plus these copies -- is the resource this kernel saturates).
-        {
-            unsigned mf = __ballot_sync(0xffffffffu, fresh);
-            if (mf) {
-                double *wslot = nw_sm + (tid & ~31);
-                do {
-                    const int L = __ffs(mf) - 1; mf &= mf - 1;
-                    const double *a = (const double *)__shfl_sync(0xffffffffu, pA, L);
-                    const double *q = (const double *)__shfl_sync(0xffffffffu, pQ, L);
-                    const unsigned d0 = (unsigned)__cvta_generic_to_shared(wslot + L + lane * NW_STRIDE);
-                    const double *g0 = lane < 27 ? a + lane : q + (lane - 27);
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0), "l"(g0));
-                    if (lane < 22)
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(d0 + 32 * NW_STRIDE * 8), "l"(q + (lane + 5)));
-                } while (mf);
-                asm volatile("cp.async.wait_all;" ::: "memory");
-            }
-            __syncwarp();
-        }
-        if (__ballot_sync(0xffffffffu, s.phase != 0) == 0) {
-            if (__ballot_sync(0xffffffffu, nst != 9 || sp > 0) == 0) break;
-            continue;
-        }
-        // ---- one evaluation per busy lane
-        bool fin = false;
-        dcn::NwResult R; R.dist = 0.0; R.cosv = 0.0; R.converged = 0;
-        // a solve that drags on looks, every 4th evaluation, whether its element has been found CUT meanwhile (by
-        // another of its pairs): nothing it could still find would matter then.  The solves that do not converge are
-        // almost all of this kind -- other patch pairs of an element the surface passes through, where the minimum
-        // is a curve of zeros and the Hessian is singular -- and each used to cost two extra launches of sub-leaves.
-        if (s.phase == 1 && s.iters >= 4 && (s.iters & 3) == 0 && u2d(__ldcg(best + (it.ak & 0x1fffffffu))) <= tau_exit) s.phase = 0;
-        if (s.phase != 0) {
-            // the leaf's box (dyadic, exact) is re-derived from the item every time instead of living in registers
-            double uc, vc, hP, sc, tc, hQ;
-            nitem_box(it, uc, vc, hP, sc, tc, hQ);
-            const double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };
-            fin = dcn::iterate(cf, s, lo, hi, tol_d2, tau_exit2, R, maxit);
-        }
-        // ---- results of the solves that finished (an attained distance is an upper bound whether converged or not)
-        bool resplit = false, splitP = false;
-        if (fin) {
-            const unsigned b = it.ak & 0x1fffffffu;
+            // ---- result of the finished solve (an attained distance is an upper bound whether converged or not)
             cnt.newton++; cnt.iters += s.iters;
-            s.phase = 0;
             atomicMin(best + b, d2u(R.dist));
             if (R.dist > tau_exit) {
                 atomicMin(dmin + b, d2u(R.dist));
                 const unsigned long long key = (d2u(R.dist) & ~0xffull) | (unsigned long long)cos_code(R.cosv);
                 atomicMin(pair_key + it.p, key);
-                if (!R.converged && !((it.w3 >> 24) & 1)) {
+                if (!R.converged && !seed) {
                     // unconverged: the distance above stands as an upper bound and the leaf is quartered (a seed solve is
-                    // never split: the roots cover its pair).  With an overflow queue the four sub-leaves go there, for
-                    // the next launch to spread over the machine: solved one after the other by this lane they were a
-                    // serial chain of up to 5 x NW_MAXIT evaluations that the whole launch waited for (175 us of 690).
+                    // never split: the roots cover its pair)
                     cnt.fail++;
+                    bool splitP = false;
                     if (u2d(__ldcg(best + b)) <= tau_exit) { /* the element is CUT by now: no sub-leaves */ }
                     else if (choose_split(it, (it.w2 & 15) <= ((it.w2 >> 4) & 15), max_level, splitP)) {
-                        if (ovf) resplit = true;
-                        else if (sp + 4 <= NW_STACK) {
+                        if (ovf) {
+                            const long long sl = warp_reserve_try(ovf_n, 4, ovf_cap);
+                            if (sl >= 0) {
+#pragma unroll
+                                for (int c = 0; c < 4; ++c) ovf[sl + c] = nitem_child(it, splitP, c);
+                            } else { atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW); }
+                        } else if (sp + 4 <= NW_STACK) {
 #pragma unroll
                             for (int c = 0; c < 4; ++c) stk[sp++] = nitem_child(it, splitP, c);
                         } else cnt.depth++;
                     } else cnt.depth++;
                 }
             }
-        }
-        if (ovf) {
-            const long long sl = warp_reserve(ovf_n, resplit, 4, ovf_cap, &S->status);
-            if (sl >= 0) {
-#pragma unroll
-                for (int c = 0; c < 4; ++c) ovf[sl + c] = nitem_child(it, splitP, c);
-            }
+            if (sp == 0) break;
+            // (last launch) next sub-leaf of this lane's own: same pair, the coefficients are in place
+            it = stk[--sp];
+            nitem_box(it, uc, vc, hP, sc, tc, hQ);
+            lo[0] = uc - hP; lo[1] = vc - hP; lo[2] = sc - hQ; lo[3] = tc - hQ;
+            hi[0] = uc + hP; hi[1] = vc + hP; hi[2] = sc + hQ; hi[3] = tc + hQ;
+            s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc;
+            s.iters = 0; s.ls = 0; s.phase = 1;
+            left = maxit;
         }
     }
     np_flush_counters(S, cnt);
@@ -501,27 +514,6 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_roots(DcScalars *S, const lo
     }
 }
 
-// First step of a leaf's closest-point solve, taken here where the centre evaluation already exists: the
-// Gauss-Newton step of |r + P_u du + P_v dv - Q_s ds - Q_t dt|^2 from the centre, clamped to the leaf's box, in the
-// leaf's local coordinates [-1,1]^4 (floats: it is a starting point).  Saves k_np_newton its evaluation at the centre.
-__device__ __forceinline__ float4 leaf_first_step(const NodeOut &o, double hP, double hQ)
-{
-#define DOT3(A, B) (A[0] * B[0] + A[1] * B[1] + A[2] * B[2])
-    // local variables a = du / hP ... : columns scaled by the half-widths
-    const double h00 = hP * hP * DOT3(o.pu, o.pu), h01 = hP * hP * DOT3(o.pu, o.pv), h02 = -hP * hQ * DOT3(o.pu, o.qs), h03 = -hP * hQ * DOT3(o.pu, o.qt);
-    const double h11 = hP * hP * DOT3(o.pv, o.pv), h12 = -hP * hQ * DOT3(o.pv, o.qs), h13 = -hP * hQ * DOT3(o.pv, o.qt);
-    const double h22 = hQ * hQ * DOT3(o.qs, o.qs), h23 = hQ * hQ * DOT3(o.qs, o.qt), h33 = hQ * hQ * DOT3(o.qt, o.qt);
-    const double g[4] = { hP * DOT3(o.r, o.pu), hP * DOT3(o.r, o.pv), -hQ * DOT3(o.r, o.qs), -hQ * DOT3(o.r, o.qt) };
-#undef DOT3
-    const double tr = h00 + h11 + h22 + h33;
-    double p[4] = { 0.0, 0.0, 0.0, 0.0 };
-    if (tr > 0.0) dcn::ldl4_mod(h00, h01, h02, h03, h11, h12, h13, h22, h23, h33, g, 1e-6 * tr, p);
-    float4 x;
-    x.x = (float)dmax2(-1.0, dmin2(1.0, p[0])); x.y = (float)dmax2(-1.0, dmin2(1.0, p[1]));
-    x.z = (float)dmax2(-1.0, dmin2(1.0, p[2])); x.w = (float)dmax2(-1.0, dmin2(1.0, p[3]));
-    return x;
-}
-
 // ------------------------------------------------------------------------------------------
 // Bound: one thread per item of qin[0 .. n): prune, or 4 children -> qout, or leaf -> the ONE leaf queue nq
 // (all rounds append to it; the Newton kernel runs once, after the last round).  Items i0, i0 + stride, ...
@@ -529,7 +521,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                                                const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                NItem *__restrict__ qout, int *__restrict__ qout_n,
-                                               NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap,
+                                               NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap,
                                                int i0, int stride, NpCounters &cnt, bool force_leaf = false)
 {
     const double t_tie = S->t_tie, tau_exit = S->tau_exit, theta2 = S->theta * S->theta;
@@ -539,6 +531,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
         bool split = false, leaf = false, splitP = false;
         NItem it; it.p = it.ak = it.w2 = it.w3 = 0;
         float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f);
+        double lbq = 0.0;                      // the leaf's lower bound
         if (i < n) {
             // (L2 load: the tail kernel reads items the same launch wrote)
             const uint4 w = __ldcg(reinterpret_cast<const uint4 *>(qin + i));
@@ -559,19 +552,27 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                 }
                 const NodeOut o = bound_node(AP, AQ, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
                 cnt.nodes++;
-                if (o.dist_c < bst) { atomicMin(best + b, d2u(o.dist_c)); bst = o.dist_c; }
-                if (o.dist_c > tau_exit && o.lb <= bst + t_tie) {
+                if (o.ub < bst) { atomicMin(best + b, d2u(o.ub)); bst = o.ub; }
+                const bool alive = o.ub > tau_exit && o.lb <= bst + t_tie;
+                lbq = o.lb;
+                x0 = make_float4((float)o.x0[0], (float)o.x0[1], (float)o.x0[2], (float)o.x0[3]);
+                if (alive) {
                     leaf = o.leaf || force_leaf;     // (sub-leaves of an unconverged leaf stay leaves)
                     if (!leaf) {
                         split = choose_split(it, o.splitP, max_level, splitP);
                         if (!split) { leaf = true; cnt.depth++; }
                     }
-                    if (leaf) x0 = leaf_first_step(o, hP, hQ);
                 }
             }
         }
         const long long sl = warp_reserve(nq_n, leaf, 1, qcap, &S->status);
-        if (sl >= 0) { nq[sl] = it; nqx[sl] = x0; }
+        if (sl >= 0) {
+            NLeafX lx;
+            lx.x[0] = (short)__float2int_rn(x0.x * 32767.f); lx.x[1] = (short)__float2int_rn(x0.y * 32767.f);
+            lx.x[2] = (short)__float2int_rn(x0.z * 32767.f); lx.x[3] = (short)__float2int_rn(x0.w * 32767.f);
+            lx.lb = lbq;
+            nq[sl] = it; nqx[sl] = lx;
+        }
         const long long slot = warp_reserve(qout_n, split, 4, qcap, &S->status);
         if (slot >= 0) {
 #pragma unroll
@@ -584,7 +585,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
-                                                          NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap, int force_leaf)
+                                                          NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap, int force_leaf)
 {
     const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
     if (n == 0) return;
@@ -601,7 +602,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
 __global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S, int r_begin, int r_end, NItem *q0, NItem *q1,
                                                                    const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                                    const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
-                                                                   NItem *__restrict__ nq, float4 *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
+                                                                   NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
 {
     NpCounters cnt = { 0, 0, 0, 0, 0 };
     for (int r = r_begin; r < r_end; ++r) {

@@ -47,7 +47,9 @@ DCN_HD double rcp_fast(double x)
 #endif
 }
 
+#ifndef NW_MAXIT
 #define NW_MAXIT 24                 /* evaluations per solve before it is declared unconverged */
+#endif
 
 // state of one lane's solve
 struct NwState {
