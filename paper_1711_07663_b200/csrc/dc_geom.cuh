@@ -13,6 +13,13 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// a work item of the narrow phase: a candidate pair, a boundary patch of its element, and a dyadic sub-rectangle of each
+struct __align__(16) NItem { unsigned p, ak, w2, w3; };
+// p : global pair index (face = pair_face[p], key slot = pair_key[p])
+// ak: band index b (29 bits) | boundary patch k << 29
+// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20
+// w3: is(12) | it(12)<<12 | flags(8)<<24      flags bit0: seed solve (no re-split on failure)
+
 namespace dcg {
 
 // min / max of two finite doubles as one compare and a select (fmin / fmax expand to a NaN-aware sequence about

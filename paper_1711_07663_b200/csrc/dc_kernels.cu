@@ -454,7 +454,7 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
 // (PAPER.md L689-L709).  Survivors are staged in shared memory and written as ONE contiguous segment of
 // the pair list (one atomic per element); an element with more survivors than the stage holds re-walks its
 // ranges and writes directly.  pair_key is initialised to +inf for S5.
-__device__ __forceinline__ bool box_within(const double *lo, const double *hi, const double *fb, double reach2)
+__device__ __forceinline__ double box_dist2(const double *lo, const double *hi, const double *fb)
 {
     double d2 = 0.0;
 #pragma unroll
@@ -462,7 +462,7 @@ __device__ __forceinline__ bool box_within(const double *lo, const double *hi, c
         const double g = dmax2(0.0, dmax2(fb[c] - hi[c], lo[c] - fb[3 + c]));
         d2 = fma(g, g, d2);
     }
-    return d2 <= reach2;
+    return d2;
 }
 
 #define PR_WARPS 8
@@ -474,7 +474,9 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                                                const double *__restrict__ fbox, long long max_pairs,
                                                int *__restrict__ band_elem, long long *__restrict__ band_start,
                                                int *__restrict__ band_cnt,
-                                               int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key)
+                                               int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key,
+                                               int *__restrict__ pair_band, NItem *__restrict__ seed_q,
+                                               unsigned long long *__restrict__ best, unsigned long long *__restrict__ dmin)
 {
     __shared__ int s_list[PR_GROUPS][PR_CAP];
     __shared__ int s_off[PR_GROUPS][PR_W + 1];
@@ -504,7 +506,8 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
         for (int c = 0; c < 3; ++c) { b0[c] = i0[c] >> sl; nb[c] = (i1[c] >> sl) - b0[c] + 1; }
         const int nblk = nb[0] * nb[1] * nb[2];
         long long base = 0;
-        int total = 0;
+        int total = 0, bslot = 0;
+        unsigned long long skey = ~0ull;
         for (int phase = 0; phase < 2; ++phase) {
             int running = 0;
             for (int bbase = 0; bbase < nblk; bbase += PR_W) {
@@ -522,6 +525,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                     const int j = j0 + lane;
                     bool hit = false;
                     int p = -1;
+                    double d2 = 0.0;
                     if (j < T) {
                         int L = 0;                       // largest L with off[L] <= j
 #pragma unroll
@@ -533,14 +537,20 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                             const double2 v = __ldg(reinterpret_cast<const double2 *>(fbox + (size_t)p * 6 + m));
                             fb[m] = v.x; fb[m + 1] = v.y;
                         }
-                        hit = box_within(lo, hi, fb, reach2);
+                        d2 = box_dist2(lo, hi, fb);
+                        hit = d2 <= reach2;
                         if (phase == 0) ++tests;
                     }
                     const unsigned m = (__ballot_sync(gmask, hit) >> gshift) & (PR_W == 32 ? 0xffffffffu : ((1u << PR_W) - 1u));
                     const int pos = running + __popc(m & lt_mask);
                     if (hit) {
-                        if (phase == 0) { if (pos < PR_CAP) list[pos] = p; }
-                        else { pair_face[base + pos] = p; pair_key[base + pos] = 0x7ff0000000000000ull; }
+                        if (phase == 0) {
+                            if (pos < PR_CAP) list[pos] = p;
+                            // (the seed of the narrow phase: the pair with the nearest face box)
+                            const unsigned long long kk = ((unsigned long long)__double_as_longlong(d2) & ~0xfffffull) | (unsigned long long)min(pos, 0xfffff);
+                            skey = kk < skey ? kk : skey;
+                        }
+                        else { pair_face[base + pos] = p; pair_key[base + pos] = 0x7ff0000000000000ull; pair_band[base + pos] = (int)bslot; }
                     }
                     running += __popc(m);
                 }
@@ -548,20 +558,29 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
             }
             if (phase == 1) break;
             total = running;
+#pragma unroll
+            for (int o = PR_W / 2; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(gmask, skey, o, PR_W); skey = v < skey ? v : skey; }
             if (lane == 0) {
                 long long b = (long long)atomicAdd(&S->n_pairs, (unsigned long long)total);
                 if (b + total > max_pairs) { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
                 if (b >= 0 && total > 0) {
                     const int slot = atomicAdd(&S->n_band, 1);
-                    if (slot < S->max_band) { band_elem[slot] = (int)e; band_start[slot] = b; band_cnt[slot] = total; }
-                    else atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW);
+                    if (slot < S->max_band) {
+                        band_elem[slot] = (int)e; band_start[slot] = b; band_cnt[slot] = total;
+                        best[slot] = (unsigned long long)__double_as_longlong(reach);
+                        dmin[slot] = 0x7ff0000000000000ull;
+                        NItem it; it.p = (unsigned)(b + (long long)(skey & 0xfffffull)); it.ak = (unsigned)slot | (7u << 29); it.w2 = 0; it.w3 = 1u << 24;
+                        seed_q[slot] = it;
+                        bslot = slot;
+                    } else { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
                 }
                 base = b;
             }
             base = __shfl_sync(gmask, base, 0, PR_W);
+            bslot = __shfl_sync(gmask, bslot, 0, PR_W);
             if (base < 0 || total == 0) break;
             if (total <= PR_CAP) {
-                for (int i = lane; i < total; i += PR_W) { pair_face[base + i] = list[i]; pair_key[base + i] = 0x7ff0000000000000ull; }
+                for (int i = lane; i < total; i += PR_W) { pair_face[base + i] = list[i]; pair_key[base + i] = 0x7ff0000000000000ull; pair_band[base + i] = bslot; }
                 break;
             }
         }
@@ -857,7 +876,7 @@ struct dc_ctx {
     int *band_elem; long long *band_start; int *band_cnt;
     double *ecoef, *pbox; unsigned long long *best, *dmin;
     NItem *q[2], *nq; NLeafX *nqx;
-    int *pair_face; unsigned long long *pair_key;
+    int *pair_face; unsigned long long *pair_key; int *pair_band;
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
     int *cell_count, *cell_start, *cell_fill;
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
@@ -873,7 +892,7 @@ static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 struct WsLayout {
     size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
         off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq, off_nqx,
-        off_pair_face, off_pair_key, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
+        off_pair_face, off_pair_key, off_pair_band, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
         off_cell_count, off_cell_start, off_cell_fill, off_hfaces, off_hlabels, off_hsdist, total;
     long long max_band, qcap;
 };
@@ -915,6 +934,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     if (pf + pk < need_adj) pk = need_adj - pf;
     L.off_pair_face = take(pf);
     L.off_pair_key = take(pk);
+    L.off_pair_band = take((size_t)max_pairs * 4);
     L.off_fbox_orig = take((size_t)max_faces * 6 * 8);
     L.off_fbox = take((size_t)max_faces * 6 * 8);
     L.off_fcoef = take((size_t)max_faces * 28 * 8);
@@ -992,6 +1012,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->nqx = (NLeafX *)(c->ws + L.off_nqx);
     c->pair_face = (int *)(c->ws + L.off_pair_face);
     c->pair_key = (unsigned long long *)(c->ws + L.off_pair_key);
+    c->pair_band = (int *)(c->ws + L.off_pair_band);
     c->fbox_orig = (double *)(c->ws + L.off_fbox_orig);
     c->fbox = (double *)(c->ws + L.off_fbox);
     c->fcoef = (double *)(c->ws + L.off_fcoef);
@@ -1067,13 +1088,13 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
     k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->act_elem);
     k_pairs<<<c->num_sms * 16, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
-                                           c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key);
+                                           c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key,
+                                           c->pair_band, c->nq, c->best, c->dmin);
     CK(cudaEventRecord(c->ev[2], st));
     // ---- S5: wavefront narrow phase (dc_narrow.cuh)
     const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
     DcScalars *S = c->S;
-    k_np_stage<<<gw, NPW_THREADS, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fcoef,
-                                           c->ecoef, c->pbox, c->best, c->dmin, c->nq);
+    k_np_stage<<<gw, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox);
     // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
     // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
     const int gs = c->num_sms * 2 * 4;     // solve grids: grid-stride, 2 resident CTAs of 128 threads per SM
@@ -1081,8 +1102,8 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
                                              c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT);
     CK(cudaEventRecord(c->ev[10], st));
-    k_np_roots<<<gw, NPW_THREADS, 0, st>>>(S, c->band_start, c->band_cnt, c->pair_face, c->fbox, c->pbox, c->best,
-                                           c->q[0], &S->qn[0], c->qcap);
+    k_np_roots<<<c->num_sms * 8, 256, 0, st>>>(S, c->pair_band, c->pair_face, c->fbox, c->pbox, c->best, c->max_pairs,
+                                               c->q[0], &S->qn[0], c->qcap);
     // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
     // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
     const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;

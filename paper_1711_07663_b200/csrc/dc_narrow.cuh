@@ -3,14 +3,13 @@
 // Every kernel does one kind of operation and compacts its output into a global queue (warp-aggregated
 // atomics), so warps stay full and no kernel carries another's registers:
 //
-//   k_np_stage      warp / band element : gather the 27 nodes, monomial coefficients and Bezier boxes of the 6
-//                                         boundary patches -> ecoef, pbox; centre-centre distances of all
-//                                         (pair, patch) -> first upper bound best[b] and ONE seed item per element
+//   k_np_stage      thread / (element, patch) : monomial coefficients and Bezier box of a boundary patch -> ecoef, pbox
+//                                         (the first upper bound best[b] and the seed item come from k_pairs)
 //   k_np_newton     persistent warps    : projected Newton (Eq. 3-5 L256-L270 generalised to two patches, clamp
 //                                         L272-L278), one solve per lane in lockstep, lanes refilled from the
 //                                         queue; min into best / dmin / pair_key; the sub-leaves of an unconverged
 //                                         leaf go to an overflow queue
-//   k_np_roots      warp / band element : (pair, patch) whose boxes are within best + t_tie (A.2, L689-L709)
+//   k_np_roots      thread / pair       : (pair, patch) whose boxes are within best + t_tie (A.2, L689-L709)
 //                                         become the items of round 0
 //   k_np_bound      thread / item       : bound_node -> prune / 4 children / leaf (+ the leaf's first step)
 //   k_np_bound_tail one CTA             : the sparse late rounds, until one comes up empty
@@ -24,11 +23,6 @@
 #define NPW_THREADS 128
 #define DC_MAX_ROUNDS 25            /* 2 * 12 + 1 */
 
-struct __align__(16) NItem { unsigned p, ak, w2, w3; };
-// p : global pair index (face = pair_face[p], key slot = pair_key[p])
-// ak: band index b (29 bits) | boundary patch k << 29
-// w2: lP(4) | lQ(4)<<4 | iu(12)<<8 | iv(12)<<20
-// w3: is(12) | it(12)<<12 | flags(8)<<24      flags bit0: seed solve (no re-split on failure)
 
 // what a leaf carries beside its item (16 bytes): the starting point of its solve (the first step k_np_bound took from
 // the centre, local coordinates in [-1,1] as 16-bit fixed point: +-32767 = on the bound) and its lower bound (the solve
@@ -113,126 +107,48 @@ __device__ __forceinline__ void np_flush_counters(DcScalars *S, const NpCounters
 }
 
 // ------------------------------------------------------------------------------------------
-// Stage: one warp per band element.  ecoef [b][6][28] (27 monomial coefficients [coord][9] + the
-// higher-order constant K), pbox [b][6][6] (Bezier box of each boundary patch).
-#define ST_WARPS (NPW_THREADS / 32)
-__global__ void __launch_bounds__(NPW_THREADS) k_np_stage(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
-                                                          const int *__restrict__ band_elem, const long long *__restrict__ band_start,
-                                                          const int *__restrict__ band_cnt, const int *__restrict__ pair_face,
-                                                          const double *__restrict__ fcoef, double *__restrict__ ecoef,
-                                                          double *__restrict__ pbox, unsigned long long *__restrict__ best,
-                                                          unsigned long long *__restrict__ dmin, NItem *__restrict__ nq)
+// Stage: one thread per (band element, boundary patch).  ecoef [b][6][28] (27 monomial coefficients [coord][9] + the
+// higher-order constant K), pbox [b][6][6] (Bezier box of each boundary patch).  (best[b], dmin[b] and the seed item
+// are written by k_pairs, which meets every candidate pair anyway.)
+__global__ void __launch_bounds__(128) k_np_stage(const DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
+                                                  const int *__restrict__ band_elem, double *__restrict__ ecoef,
+                                                  double *__restrict__ pbox)
 {
-    __shared__ double s_nodes[ST_WARPS][81];
-    __shared__ double s_coef[ST_WARPS][6 * 28];
-    __shared__ double s_box[ST_WARPS][36];
-    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
     const int n_band = min(S->n_band, S->max_band);
-    const double reach = S->reach;
-    double *nd = s_nodes[wl], *cf = s_coef[wl], *bx = s_box[wl];
-    // the node gather (band_elem -> conn -> xyz: three dependent loads) of the NEXT element of this warp is issued
-    // before the current one is processed
-    double cx = 0.0, cy = 0.0, cz = 0.0;
-    if (warp < n_band && lane < 27) {
-        const int id = __ldg(conn + (size_t)band_elem[warp] * 27 + lane);
-        const double *p = xyz + (size_t)id * 3;
-        cx = __ldg(p); cy = __ldg(p + 1); cz = __ldg(p + 2);
-    }
-    for (int b = warp; b < n_band; b += nwarps) {
-        if (lane < 27) { nd[lane * 3 + 0] = cx; nd[lane * 3 + 1] = cy; nd[lane * 3 + 2] = cz; }
-        if (b + nwarps < n_band && lane < 27) {
-            const int id = __ldg(conn + (size_t)band_elem[b + nwarps] * 27 + lane);
-            const double *p = xyz + (size_t)id * 3;
-            cx = __ldg(p); cy = __ldg(p + 1); cz = __ldg(p + 2);
-        }
-        __syncwarp();
-        if (lane < 18) {
-            const int k = lane / 3, c = lane % 3;
-            double x[9], a[9];
+    const long long n = (long long)n_band * 6;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int b = (int)(i / 6), k = (int)(i - (long long)b * 6);
+        const int *cn = conn + (size_t)__ldg(band_elem + b) * 27;
+        // nodes of boundary patch k (c_face_node[k][a + 3 b] = base + sa a + sb b; the table itself is not used here: with a
+        // runtime k the compiler pairs its 36-byte rows into 64-bit constant loads, misaligned for odd k)
+        const int nbase = k == 1 ? 2 : (k == 3 ? 6 : (k == 5 ? 18 : 0)), sa = k < 2 ? 3 : 1, sb = k < 4 ? 9 : 3;
+        int id[9];
 #pragma unroll
-            for (int m = 0; m < 9; ++m) x[m] = nd[c_face_node[k][m] * 3 + c];
-            nodes_to_mono9(x, a);
+        for (int m = 0; m < 9; ++m) id[m] = __ldg(cn + nbase + sa * (m % 3) + sb * (m / 3));
+        double A[28], box[6];
 #pragma unroll
-            for (int m = 0; m < 9; ++m) cf[k * 28 + c * 9 + m] = a[m];
+        for (int c = 0; c < 3; ++c) {
+            double x[9];
+#pragma unroll
+            for (int m = 0; m < 9; ++m) x[m] = __ldg(xyz + (size_t)id[m] * 3 + c);
+            nodes_to_mono9(x, A + 9 * c);
             // Bezier box of the patch (convex-hull property)
 #pragma unroll
             for (int j = 0; j < 3; ++j) x[3 * j + 1] = bez_mid(x[3 * j], x[3 * j + 1], x[3 * j + 2]);
 #pragma unroll
-            for (int i = 0; i < 3; ++i) x[i + 3] = bez_mid(x[i], x[i + 3], x[i + 6]);
+            for (int q = 0; q < 3; ++q) x[q + 3] = bez_mid(x[q], x[q + 3], x[q + 6]);
             double lo = x[0], hi = x[0];
 #pragma unroll
             for (int m = 1; m < 9; ++m) { lo = dmin2(lo, x[m]); hi = dmax2(hi, x[m]); }
-            bx[k * 6 + c] = lo; bx[k * 6 + 3 + c] = hi;
+            box[c] = lo; box[3 + c] = hi;
         }
-        __syncwarp();
-        // constants K of the 6 patches (dc_geom.cuh higher_order_const): the 6 x 6 coefficient norms it needs are
-        // spread over the warp (a lane per norm) instead of 9 square roots in a row on 6 lanes
-        {
-            // weights of |A20| |A02| |A11| |A21| |A12| |A22| (m = 2, 6, 4, 5, 7, 8) in K
-            const int mm[6] = { 2, 6, 4, 5, 7, 8 };
-            const double ww[6] = { 1.0, 1.0, 1.0, 4.0, 4.0, 11.0 };
-            double part = 0.0, part2 = 0.0;
-            {
-                const int k = lane / 6, j = lane % 6;           // lanes 0..31 -> (patch, norm) 0..31
-                const double *A = cf + k * 28;
-                const int m = mm[j];
-                part = ww[j] * sqrt(A[m] * A[m] + A[9 + m] * A[9 + m] + A[18 + m] * A[18 + m]);
-            }
-            if (lane < 4) {                                     // (patch 5, norms 2..5) = items 32..35
-                const int j = lane + 2;
-                const double *A = cf + 5 * 28;
-                const int m = mm[j];
-                part2 = ww[j] * sqrt(A[m] * A[m] + A[9 + m] * A[9 + m] + A[18 + m] * A[18 + m]);
-            }
-            // sum the 6 norms of each patch: lanes 6k .. 6k+5 (patch 5: lanes 30, 31 + part2 of lanes 0..3)
-            double sum = part;
+        A[27] = higher_order_const(A);
+        double2 *out = reinterpret_cast<double2 *>(ecoef + (size_t)i * 28);
 #pragma unroll
-            for (int o = 1; o < 6; ++o) {
-                const double v = __shfl_down_sync(0xffffffffu, part, o);
-                if (lane % 6 + o < 6 && lane + o < 32) sum += v;
-            }
-            double tail = part2;
-            tail += __shfl_down_sync(0xffffffffu, tail, 2);
-            tail += __shfl_down_sync(0xffffffffu, tail, 1);
-            tail = __shfl_sync(0xffffffffu, tail, 0);
-            if (lane % 6 == 0 && lane < 30) cf[(lane / 6) * 28 + 27] = sum;
-            if (lane == 30) cf[5 * 28 + 27] = sum + tail;
-        }
-        __syncwarp();
-        for (int i = lane; i < 6 * 28; i += 32) ecoef[(size_t)b * (6 * 28) + i] = cf[i];
-        for (int i = lane; i < 36; i += 32) pbox[(size_t)b * 36 + i] = bx[i];
-        // centre-centre distances of every (pair, patch): attained => upper bound; the smallest seeds Newton.
-        // A lane per pair (its face centre is loaded once), the 6 patch centres come from shared memory.
-        const long long p0 = band_start[b];
-        const int npair = band_cnt[b];
-        unsigned long long key = ~0ull;
-        for (int pl = lane; pl < npair; pl += 32) {
-            const int f = __ldg(pair_face + p0 + pl);
-            const double *AQ = fcoef + (size_t)f * 28;
-            const double qx = __ldg(AQ), qy = __ldg(AQ + 9), qz = __ldg(AQ + 18);
+        for (int m = 0; m < 14; ++m) out[m] = make_double2(A[2 * m], A[2 * m + 1]);
+        double2 *ob = reinterpret_cast<double2 *>(pbox + (size_t)i * 6);
 #pragma unroll
-            for (int k = 0; k < 6; ++k) {
-                const double dx = cf[k * 28] - qx, dy = cf[k * 28 + 9] - qy, dz = cf[k * 28 + 18] - qz;
-                const double d2 = dx * dx + dy * dy + dz * dz;           // (squared: one sqrt per element, below)
-                const unsigned long long kk = (d2u(d2) & ~0xfffffull) | (unsigned long long)min(pl * 6 + k, 0xfffff);
-                key = kk < key ? kk : key;
-            }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, key, o); key = v < key ? v : key; }
-        if (lane == 0) {
-            // the truncated key is <= the attained squared distance: round up to stay an upper bound
-            const double dkey = sqrt(u2d((key & ~0xfffffull) + 0x100000ull)) * (1.0 + 4e-16);
-            best[b] = d2u(dmin2(reach, dkey));
-            dmin[b] = 0x7ff0000000000000ull;
-            const int t = (int)(key & 0xfffffull);
-            const int pl = t / 6, k = t - pl * 6;
-            NItem it; it.p = (unsigned)(p0 + pl); it.ak = (unsigned)b | ((unsigned)k << 29); it.w2 = 0; it.w3 = 1u << 24;
-            nq[b] = it;
-        }
-        __syncwarp();
+        for (int m = 0; m < 3; ++m) ob[m] = make_double2(box[2 * m], box[2 * m + 1]);
     }
 }
 
@@ -350,19 +266,33 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
             lb = __hiloint2double((int)st.y, (int)st.x);
             s.iters = (int)(st.z & 0xffff); s.ls = (int)(st.z >> 16); s.phase = (int)(st.w & 0xffff);
         }
-        const unsigned b = it.ak & 0x1fffffffu, k = it.ak >> 29;
+        const unsigned b = it.ak & 0x1fffffffu;
+        unsigned k = it.ak >> 29;
         const double bst0 = u2d(__ldcg(best + b));
         // dropped: the element is already CUT, or its best distance is below this leaf's lower bound by now
         if (!(bst0 > tau_exit) || lb > bst0 + t_tie) continue;
         double AP[28], AQ[28];
         {
-            const double2 *APg = reinterpret_cast<const double2 *>(ecoef + ((size_t)b * 6 + k) * 28);
             const double2 *AQg = reinterpret_cast<const double2 *>(fcoef + (size_t)__ldg(pair_face + it.p) * 28);
 #pragma unroll
-            for (int m = 0; m < 14; ++m) {
-                const double2 vp = __ldg(APg + m), vq = __ldg(AQg + m);
-                AP[2 * m] = vp.x; AP[2 * m + 1] = vp.y; AQ[2 * m] = vq.x; AQ[2 * m + 1] = vq.y;
+            for (int m = 0; m < 14; ++m) { const double2 vq = __ldg(AQg + m); AQ[2 * m] = vq.x; AQ[2 * m + 1] = vq.y; }
+            if (k == 7) {
+                // a seed names the pair with the nearest face BOX (k_pairs); its patch is the one whose centre is nearest
+                // to the face's centre
+                double dbest = INFINITY;
+                k = 0;
+#pragma unroll
+                for (int kk = 0; kk < 6; ++kk) {
+                    const double *c = ecoef + ((size_t)b * 6 + kk) * 28;
+                    const double dx = __ldg(c) - AQ[0], dy = __ldg(c + 9) - AQ[9], dz = __ldg(c + 18) - AQ[18];
+                    const double d2 = dx * dx + dy * dy + dz * dz;
+                    if (d2 < dbest) { dbest = d2; k = kk; }
+                }
+                it.ak = b | (k << 29);
             }
+            const double2 *APg = reinterpret_cast<const double2 *>(ecoef + ((size_t)b * 6 + k) * 28);
+#pragma unroll
+            for (int m = 0; m < 14; ++m) { const double2 vp = __ldg(APg + m); AP[2 * m] = vp.x; AP[2 * m + 1] = vp.y; }
         }
         auto cf = [&](int m) { return m < 27 ? AP[m] : AQ[m - 27]; };
         double uc, vc, hP, sc, tc, hQ;
@@ -454,62 +384,59 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
 }
 
 // ------------------------------------------------------------------------------------------
-// Roots: one warp per band element, lanes over its pairs.  (pair, patch k) survives when the
-// box distance (Algorithm A.2) of the patch's Bezier box and the face's Bezier box is
-// within best + t_tie; survivors become the items of round 0.
-__global__ void __launch_bounds__(NPW_THREADS) k_np_roots(DcScalars *S, const long long *__restrict__ band_start,
-                                                          const int *__restrict__ band_cnt, const int *__restrict__ pair_face,
-                                                          const double *__restrict__ fbox, const double *__restrict__ pbox,
-                                                          const unsigned long long *__restrict__ best,
-                                                          NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
+// Roots: one thread per candidate pair.  (pair, patch k) survives when the box distance (Algorithm A.2) of
+// the patch's Bezier box and the face's Bezier box is within best + t_tie; survivors become the items of round 0
+// (warp-aggregated append: a scan of the lanes' counts, one atomic per warp).
+__global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__restrict__ pair_band, const int *__restrict__ pair_face,
+                                                  const double *__restrict__ fbox, const double *__restrict__ pbox,
+                                                  const unsigned long long *__restrict__ best, long long max_pairs,
+                                                  NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
 {
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int n_band = min(S->n_band, S->max_band);
+    const long long n_pairs = min((long long)S->n_pairs, max_pairs);
+    const long long n_round = (n_pairs + 31) & ~31LL;
     const double t_tie = S->t_tie, tau_exit = S->tau_exit;
-    for (int b = warp; b < n_band; b += nwarps) {
-        const double bst = u2d(best[b]);
-        if (bst <= tau_exit) continue;                      // already CUT
-        const double cut = bst + t_tie, cut2 = cut * cut;
-        const long long p0 = band_start[b];
-        const int cnt = band_cnt[b];
-        const double *pb = pbox + (size_t)b * 36;
-        for (int base = 0; base < cnt; base += 32) {
-            const int pl = base + lane;
-            unsigned mask = 0;
-            if (pl < cnt) {
-                const int f = __ldg(pair_face + p0 + pl);
-                double fb[6];
-#pragma unroll
-                for (int m = 0; m < 6; ++m) fb[m] = __ldg(fbox + (size_t)f * 6 + m);
+    const int lane = threadIdx.x & 31;
+    for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < n_round; p += (long long)gridDim.x * blockDim.x) {
+        unsigned mask = 0;
+        int b = 0;
+        if (p < n_pairs) {
+            b = __ldg(pair_band + p);
+            const double bst = u2d(__ldg(best + b));
+            if (bst > tau_exit) {                                   // (else: already CUT)
+                const double cut = bst + t_tie, cut2 = cut * cut;
+                const double2 *fp = reinterpret_cast<const double2 *>(fbox + (size_t)__ldg(pair_face + p) * 6);
+                const double2 f0 = __ldg(fp), f1 = __ldg(fp + 1), f2 = __ldg(fp + 2);
+                const double fb[6] = { f0.x, f0.y, f1.x, f1.y, f2.x, f2.y };
+                const double2 *pb = reinterpret_cast<const double2 *>(pbox + (size_t)b * 36);
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
+                    const double2 b0 = __ldg(pb + 3 * k), b1 = __ldg(pb + 3 * k + 1), b2 = __ldg(pb + 3 * k + 2);
+                    const double bb[6] = { b0.x, b0.y, b1.x, b1.y, b2.x, b2.y };
                     double d2 = 0.0;
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
-                        const double g = dmax2(0.0, dmax2(fb[c] - __ldg(pb + k * 6 + 3 + c), __ldg(pb + k * 6 + c) - fb[3 + c]));
+                        const double g = dmax2(0.0, dmax2(fb[c] - bb[3 + c], bb[c] - fb[3 + c]));
                         d2 = fma(g, g, d2);
                     }
                     if (d2 <= cut2) mask |= 1u << k;
                 }
             }
-            const int mine = __popc(mask);
-            int incl = mine;
+        }
+        const int mine = __popc(mask);
+        int incl = mine;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-            const int total = __shfl_sync(0xffffffffu, incl, 31);
-            if (total == 0) continue;
-            int start = 0;
-            if (lane == 31) start = atomicAdd(qout_n, total);
-            start = __shfl_sync(0xffffffffu, start, 31);
-            long long slot = (long long)start + incl - mine;
-            if ((long long)start + total > qcap) { if (lane == 0) atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW); continue; }
-            while (mask) {
-                const int k = __ffs(mask) - 1; mask &= mask - 1;
-                NItem it; it.p = (unsigned)(p0 + pl); it.ak = (unsigned)b | ((unsigned)k << 29); it.w2 = 0; it.w3 = 0;
-                qout[slot++] = it;
-            }
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        if (total == 0) continue;
+        int start = 0;
+        if (lane == 31) start = atomicAdd(qout_n, total);
+        start = __shfl_sync(0xffffffffu, start, 31);
+        if ((long long)start + total > qcap) { if (lane == 0) atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW); continue; }
+        long long slot = (long long)start + incl - mine;
+        while (mask) {
+            const int k = __ffs(mask) - 1; mask &= mask - 1;
+            NItem it; it.p = (unsigned)p; it.ak = (unsigned)b | ((unsigned)k << 29); it.w2 = 0; it.w3 = 0;
+            qout[slot++] = it;
         }
     }
 }
