@@ -7,7 +7,7 @@
 //   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
 //   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound, k_np_bound_tail (FP64)
 //   S6 decide         k_np_decide
-//   S7 flood fill     k_uf_local, k_uf_union, k_uf_seed, k_uf_collect, k_seedless, k_uf_assign
+//   S7 flood fill     k_uf_tiles, k_uf_seed, k_uf_resolve, k_uf_assign, k_seedless, k_uf_fix
 //
 // PAPER.md citations are given where an operation is defined; the kernel design itself is new
 // (the paper's A.1-A.4 kernels were written for Kepler K80 and are prior art, not the blueprint).
@@ -24,7 +24,7 @@
 
 using namespace dcg;
 
-#define DC_MAX_SEEDLESS 32
+#define DC_MAX_SEEDLESS 1024           /* seedless components resolved per cut (each by one exhaustive query) */
 #define DC_GRID_MAX 64              /* face-bin cells per axis (Morton code: 6 bits per axis) */
 #define DC_NCELL (DC_GRID_MAX * DC_GRID_MAX * DC_GRID_MAX)
 #define DC_NQN 28                   /* >= DC_MAX_ROUNDS + 2 */
@@ -53,6 +53,8 @@ struct DcScalars {
     int n_band;                     // elements with >= 1 candidate pair (the narrow-phase band)
     int max_band;                   // capacity of the per-band-element arrays
     int n_seedless;
+    int uf_tile;                    // next tile of k_uf_tiles (tiles are taken in launch order)
+    int n_lroots;                   // tile-local roots listed by k_uf_tiles
     int status;
     int qn[DC_NQN];                 // items of round r (children queue, ping-pong buffers)
     int nn[DC_NQN];                 // leaves of round r (Newton queue)
@@ -362,7 +364,7 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
     S->reach = S->d_band + 2.0 * S->tau + S->t_tie;
     S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.25;
     S->max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
-    S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->status = 0; S->n_pairs = 0ull;
+    S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->uf_tile = 0; S->n_lroots = 0; S->status = 0; S->n_pairs = 0ull;
     for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; S->nh[i] = 0; }
     S->nh[DC_NQN] = 0;
     S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
@@ -630,66 +632,97 @@ __device__ __forceinline__ void uf_union(int *parent, int a, int b)
     }
 }
 
-// Pass 1: components INSIDE a tile of UF_TILE consecutive elements, in shared memory (neighbours mostly have
-// nearby ids, so most edges are settled here without touching global memory); every element then points at
-// its tile-local root.  Pass 2 (k_uf_union): only the edges that leave the tile go through the global forest.
+__device__ __forceinline__ int ld_acquire(const int *p) { int v; asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v; }
+__device__ __forceinline__ void st_release(int *p, int v) { asm volatile("st.release.gpu.global.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory"); }
+
+// One kernel for the whole forest.  Components INSIDE a tile of UF_TILE consecutive elements are found in shared memory
+// (neighbours mostly have nearby ids, so most edges are settled there); every element then points at its tile-local root.
+// Only the edges that leave the tile (towards LOWER tiles: each edge is handled by its upper end) go through the global
+// forest.  They need the lower tile's local roots: tiles are handed out in launch order by a counter, a tile publishes a
+// flag (the cut's epoch) once its local roots are written, and an upper tile waits for the flags of the lower tiles it
+// touches -- those started earlier and never wait for an upper tile, so the wait cannot deadlock (the chained-scan
+// argument).  Per tile, a (local root, other root) pair already united is remembered in shared memory, so a slab of
+// 1024 elements facing one component of the slab below costs one union, not a thousand.
 #define UF_TILE 1024
-__global__ void __launch_bounds__(UF_TILE) k_uf_local(const signed char *__restrict__ labels, const int *__restrict__ adj,
-                                                      long long n_elem, int *__restrict__ parent)
+__global__ void __launch_bounds__(UF_TILE) k_uf_tiles(DcScalars *S, const signed char *__restrict__ labels, const int *__restrict__ adj,
+                                                      long long n_elem, int *parent, int *tile_flag, int epoch,
+                                                      int *__restrict__ lroot_list)
 {
     __shared__ int sp[UF_TILE];
-    const int tid = threadIdx.x;
-    const long long base = (long long)blockIdx.x * UF_TILE, e = base + tid;
-    sp[tid] = tid;
+    __shared__ int s_last[UF_TILE];
+    __shared__ signed char s_lab[UF_TILE];
+    __shared__ int s_tile;
+    const int tid = threadIdx.x, lane = tid & 31;
+    if (tid == 0) s_tile = atomicAdd(&S->uf_tile, 1);
+    s_last[tid] = -1;
     __syncthreads();
-    if (e < n_elem && labels[e] != DC_CUT) {
-        int nbs[6];
-        const int2 *ap = reinterpret_cast<const int2 *>(adj + e * 6);
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { const int2 v = __ldg(ap + k); nbs[2 * k] = v.x; nbs[2 * k + 1] = v.y; }
-#pragma unroll
-        for (int k = 0; k < 6; ++k) {
-            const int nb = nbs[k];
-            if (nb >= base && nb < e && labels[nb] != DC_CUT) uf_union(sp, tid, nb - (int)base);
-        }
-    }
-    __syncthreads();
-    if (e < n_elem) parent[e] = (int)base + uf_find(sp, tid);
-}
-
-__global__ void k_uf_union(const signed char *__restrict__ labels, const int *__restrict__ adj, long long n_elem, int *parent)
-{
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = e < n_elem && labels[e] != DC_CUT;
-    const long long base = e & ~(long long)(UF_TILE - 1);
-    const int lane = threadIdx.x & 31;
+    const int tile = s_tile;
+    const long long base = (long long)tile * UF_TILE, e = base + tid;
+    const int lab = e < n_elem ? labels[e] : DC_CUT;
+    s_lab[tid] = (signed char)lab;
+    const bool live = lab != DC_CUT;
     int nbs[6] = { -1, -1, -1, -1, -1, -1 };
-    int mine = 0;
     if (live) {
         const int2 *ap = reinterpret_cast<const int2 *>(adj + e * 6);
 #pragma unroll
         for (int k = 0; k < 3; ++k) { const int2 v = __ldg(ap + k); nbs[2 * k] = v.x; nbs[2 * k + 1] = v.y; }
-        mine = ((volatile int *)parent)[e];              // its tile-local root (or an ancestor of it by now)
     }
-    // all the gathers of the six neighbours first (independent loads in flight together), the unions after
+    // Runs of consecutive ids that are neighbours (rows of a structured numbering) are merged inside the warp with one
+    // ballot: every lane starts hooked under the first lane of its run, and the run's edges to other runs are issued once
+    // per pair of runs, not once per element (a thousand threads hooking a row one element at a time was the cost here).
+    bool to_prev = false;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) to_prev = to_prev || nbs[k] == (int)e - 1;
+    const unsigned mlive = __ballot_sync(0xffffffffu, live);
+    to_prev = to_prev && live && lane > 0 && ((mlive >> (lane - 1)) & 1u);
+    const unsigned mconn = __ballot_sync(0xffffffffu, to_prev);
+    const int head = (tid & ~31) + (31 - __clz((~mconn) & (0xffffffffu >> (31 - lane))));
+    sp[tid] = head;
+    __syncthreads();
+    if (live) {
+        int hn[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const int nb = nbs[k];
+            const bool in_tile = nb >= base && nb < e && !(to_prev && nb == (int)e - 1) && s_lab[nb - (int)base] != DC_CUT;
+            hn[k] = in_tile ? sp[nb - (int)base] : -1;           // (its run's head, or already something above it)
+        }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const int ph = __shfl_up_sync(__activemask(), hn[k], 1);
+            if (hn[k] >= 0 && !(to_prev && ph == hn[k])) uf_union(sp, head, hn[k]);
+        }
+    }
+    __syncthreads();
+    const int lr = uf_find(sp, tid);
+    if (e < n_elem) parent[e] = (int)base + lr;
+    if (live && lr == tid) lroot_list[atomicAdd(&S->n_lroots, 1)] = (int)e;
+    __syncthreads();
+    if (tid == 0) st_release(tile_flag + tile, epoch);       // (release after the barrier: the tile's stores come before it)
+    // edges to lower tiles: all the gathers first (independent loads in flight together), the unions after
+    const int mine = (int)base + lr;
     int other[6];
     bool edge[6];
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
         const int nb = nbs[k];
         const bool cross = live && nb >= 0 && nb < base;
-        const int lab = cross ? labels[nb] : DC_CUT;
-        const int par = cross ? ((volatile int *)parent)[nb] : 0;
-        edge[k] = cross && lab != DC_CUT;
-        other[k] = edge[k] ? par : -1 - lane;
+        edge[k] = cross && labels[nb] != DC_CUT;
+        other[k] = -1 - lane;
+        if (edge[k]) {
+            const int *fl = tile_flag + nb / UF_TILE;
+            while (ld_acquire(fl) != epoch) { }
+            other[k] = ((volatile int *)parent)[nb];
+        }
     }
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-        // neighbouring elements mostly sit in the same tile-local components on both sides of a tile border: a lane
-        // whose (root, root) pair equals that of the lane before it leaves the union to that lane (its own would be a
-        // no-op after three dependent loads)
+        // a lane whose (root, root) pair equals that of the lane before it leaves the union to that lane; the others ask the
+        // tile's memory of the last root united with their local root
         const int pm = __shfl_up_sync(0xffffffffu, mine, 1), po = __shfl_up_sync(0xffffffffu, other[k], 1);
-        if (edge[k] && !(lane > 0 && pm == mine && po == other[k])) uf_union(parent, mine, other[k]);
+        if (edge[k] && !(lane > 0 && pm == mine && po == other[k])) {
+            if (atomicExch(&s_last[lr], other[k]) != other[k]) uf_union(parent, mine, other[k]);
+        }
     }
 }
 
@@ -703,22 +736,14 @@ __global__ void k_uf_seed(const DcScalars *S, const int *__restrict__ band_elem,
         const int lab = labels[e];
         if (lab == DC_HOLE || lab == DC_NORMAL) {
             const int r = uf_find(parent, e);
-            // byte-wide OR through a 32-bit atomic
-            unsigned *w = reinterpret_cast<unsigned *>(comp + (r & ~3));
-            atomicOr(w, (unsigned)(lab == DC_HOLE ? 1 : 2) << (8 * (r & 3)));
+            // byte-wide OR through a 32-bit atomic; tested first (two giant components take almost every seed: the
+            // atomics on their two words were the whole duration of this kernel)
+            const unsigned bit = lab == DC_HOLE ? 1u : 2u;
+            if ((((volatile unsigned char *)comp)[r] & bit) == 0) {
+                unsigned *w = reinterpret_cast<unsigned *>(comp + (r & ~3));
+                atomicOr(w, bit << (8 * (r & 3)));
+            }
         }
-    }
-}
-
-__global__ void k_uf_collect(DcScalars *S, const signed char *__restrict__ labels, long long n_elem,
-                             const int *__restrict__ parent, const unsigned char *__restrict__ comp)
-{
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n_elem) return;
-    if (labels[e] != DC_CUT && parent[e] == (int)e && comp[e] == 0) {
-        const int i = atomicAdd(&S->n_seedless, 1);
-        if (i < DC_MAX_SEEDLESS) S->seedless_elem[i] = (int)e;
-        else atomicOr(&S->status, DC_STATUS_SEEDLESS_OVERFLOW);
     }
 }
 
@@ -734,9 +759,10 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
     __shared__ unsigned long long s_best;
     __shared__ double s_d[SL_THREADS], s_c[SL_THREADS];
     const int ns = min(S->n_seedless, DC_MAX_SEEDLESS);
-    if ((int)blockIdx.x >= ns) return;
-    const int e = S->seedless_elem[blockIdx.x];
     const int tid = threadIdx.x;
+    for (int comp_i = blockIdx.x; comp_i < ns; comp_i += gridDim.x) {
+    const int e = S->seedless_elem[comp_i];
+    __syncthreads();
     if (tid < 27) {
         const int id = conn[(size_t)e * 27 + tid];
         for (int c = 0; c < 3; ++c) s_nodes[tid * 3 + c] = xyz[(size_t)id * 3 + c];
@@ -802,36 +828,94 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
         comp[e] = bc < 0.0 ? 1 : 2;
         atomicAdd(&S->c_seedless_total, 1ull);
     }
+    }
 }
 
-__global__ void k_uf_assign(DcScalars *S, long long n_elem, int *parent,
-                            const unsigned char *__restrict__ comp, signed char *__restrict__ labels,
-                            double *__restrict__ sdist)
+// Labels of the elements S6 left undecided.  An element points at its tile-local root (or, a hooked root or a band
+// element whose path k_uf_seed has halved, at some root above it), and every such root is in the list k_uf_tiles made:
+// k_uf_resolve walks the global forest once per listed root and leaves the component's seed bits at the root itself
+// (comp[] of a hooked root is otherwise unused), so k_uf_assign is a plain stream: labels, parent, comp[parent].
+// A component with no seed at all is listed (by its global root) for k_seedless and its elements are left to k_uf_fix.
+__device__ __forceinline__ void uf_label(DcScalars *S, long long e, int lab, int bits, signed char *labels, double *sdist, bool &conflict, int &out)
 {
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    int lab = -2;
-    bool conflict = false;
-    if (e < n_elem) {
-        lab = labels[e];
-        if (lab != DC_CUT) {
-            const int bits = comp[uf_find(parent, (int)e)];
-            if (lab < 0) {
-                conflict = bits == 3;
-                lab = (bits == 1) ? DC_HOLE : DC_NORMAL;
-                labels[e] = (signed char)lab;
-                sdist[e] = lab == DC_HOLE ? -S->d_band : S->d_band;
-            } else if (bits == 3) conflict = true;
-        }
-    }
+    out = lab;
+    if (lab < 0) {
+        if (bits == 0) return;                         // seedless: k_uf_fix
+        conflict = bits == 3;
+        out = (bits == 1) ? DC_HOLE : DC_NORMAL;
+        labels[e] = (signed char)out;
+        sdist[e] = out == DC_HOLE ? -S->d_band : S->d_band;
+    } else if (bits == 3) conflict = true;
+}
+// census of the labels: ballots, then shared-memory counters, then one atomic per counter and CTA (a warp-level atomic
+// on three global addresses was most of the duration of the old assign kernel)
+__device__ __forceinline__ void uf_census(DcScalars *S, int lab, bool conflict)
+{
+    __shared__ unsigned s_cnt[4];
+    if (threadIdx.x < 4) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
     const unsigned mc = __ballot_sync(0xffffffffu, lab == DC_CUT);
     const unsigned mh = __ballot_sync(0xffffffffu, lab == DC_HOLE);
     const unsigned mn = __ballot_sync(0xffffffffu, lab == DC_NORMAL);
     const unsigned mf = __ballot_sync(0xffffffffu, conflict);
     if ((threadIdx.x & 31) == 0) {
-        if (mc) atomicAdd(&S->c_cut, (unsigned long long)__popc(mc));
-        if (mh) atomicAdd(&S->c_hole, (unsigned long long)__popc(mh));
-        if (mn) atomicAdd(&S->c_normal, (unsigned long long)__popc(mn));
-        if (mf) { atomicAdd(&S->c_fill_conflicts, (unsigned long long)__popc(mf)); atomicOr(&S->status, DC_STATUS_FILL_CONFLICT); }
+        if (mc) atomicAdd(&s_cnt[0], __popc(mc));
+        if (mh) atomicAdd(&s_cnt[1], __popc(mh));
+        if (mn) atomicAdd(&s_cnt[2], __popc(mn));
+        if (mf) atomicAdd(&s_cnt[3], __popc(mf));
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (s_cnt[0]) atomicAdd(&S->c_cut, (unsigned long long)s_cnt[0]);
+        if (s_cnt[1]) atomicAdd(&S->c_hole, (unsigned long long)s_cnt[1]);
+        if (s_cnt[2]) atomicAdd(&S->c_normal, (unsigned long long)s_cnt[2]);
+        if (s_cnt[3]) { atomicAdd(&S->c_fill_conflicts, (unsigned long long)s_cnt[3]); atomicOr(&S->status, DC_STATUS_FILL_CONFLICT); }
+    }
+}
+__global__ void k_uf_resolve(DcScalars *S, const int *__restrict__ lroot_list, int *parent, unsigned char *comp)
+{
+    const int n = S->n_lroots;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int r = lroot_list[i];
+        const int g = uf_find(parent, r);
+        const int bits = ((volatile unsigned char *)comp)[g];
+        if (g != r) comp[r] = (unsigned char)bits;        // (global roots keep their own; nobody reads a hooked root's before this)
+        else if (bits == 0) {
+            const int k = atomicAdd(&S->n_seedless, 1);
+            if (k < DC_MAX_SEEDLESS) S->seedless_elem[k] = r;
+            else atomicOr(&S->status, DC_STATUS_SEEDLESS_OVERFLOW);
+        }
+    }
+}
+__global__ void k_uf_assign(DcScalars *S, long long n_elem, const int *__restrict__ parent,
+                            const unsigned char *__restrict__ comp, signed char *__restrict__ labels,
+                            double *__restrict__ sdist)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int lab = -2, out = -2;
+    bool conflict = false;
+    if (e < n_elem) {
+        lab = labels[e]; out = lab;
+        if (lab != DC_CUT) uf_label(S, e, lab, comp[parent[e]], labels, sdist, conflict, out);
+    }
+    uf_census(S, out, conflict);
+}
+
+// the elements of seedless components, once k_seedless has given those a sign (nothing to do on most cuts)
+__global__ void k_uf_fix(DcScalars *S, long long n_elem, int *parent, const unsigned char *__restrict__ comp,
+                         signed char *__restrict__ labels, double *__restrict__ sdist)
+{
+    if (S->n_seedless == 0) return;
+    for (long long e0 = (long long)blockIdx.x * blockDim.x; e0 < n_elem; e0 += (long long)gridDim.x * blockDim.x) {
+        const long long e = e0 + threadIdx.x;
+        bool conflict = false;
+        int out = -2;
+        if (e < n_elem && labels[e] < 0) {
+            int bits = comp[uf_find(parent, (int)e)];
+            if (bits == 0) bits = 2;                    // (more seedless components than DC_MAX_SEEDLESS: status bit set)
+            uf_label(S, e, -1, bits, labels, sdist, conflict, out);
+        }
+        uf_census(S, out, conflict);
     }
 }
 
@@ -871,7 +955,7 @@ struct dc_ctx {
     DcScalars *S;
     double *ebox;             // [6][n_elem]
     int *adj_own;             // [n_elem][6] (derived) or NULL
-    int *parent; unsigned char *comp;
+    int *parent; unsigned char *comp; int *tile_flag; int epoch;
     int *act_elem;
     int *band_elem; long long *band_start; int *band_cnt;
     double *ecoef, *pbox; unsigned long long *best, *dmin;
@@ -890,7 +974,7 @@ struct dc_ctx {
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
+    size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_tile_flag, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
         off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq, off_nqx,
         off_pair_face, off_pair_key, off_pair_band, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
         off_cell_count, off_cell_start, off_cell_fill, off_hfaces, off_hlabels, off_hsdist, total;
@@ -914,6 +998,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_adj = take((size_t)n_elem * 6 * 4);
     L.off_parent = take((size_t)n_elem * 4);
     L.off_comp = take((size_t)n_elem + 4);
+    L.off_tile_flag = take((size_t)(n_elem / UF_TILE + 2) * 4);
     L.off_act_elem = take((size_t)n_elem * 4);
     L.max_band = band_capacity(n_elem, max_pairs);
     L.qcap = queue_capacity(max_pairs);
@@ -997,6 +1082,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->adj_own = (int *)(c->ws + L.off_adj);
     c->parent = (int *)(c->ws + L.off_parent);
     c->comp = c->ws + L.off_comp;
+    c->tile_flag = (int *)(c->ws + L.off_tile_flag);
     c->act_elem = (int *)(c->ws + L.off_act_elem);
     c->max_band = L.max_band; c->qcap = L.qcap;
     c->band_elem = (int *)(c->ws + L.off_band_elem);
@@ -1029,6 +1115,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     for (int i = 0; i < 12; ++i) CK(cudaEventCreate(&c->ev[i]));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
+    CK(cudaMemsetAsync(c->tile_flag, 0, (size_t)(n_elem / UF_TILE + 2) * 4, st));
     int rc = run_elem_boxes(c, st);
     if (rc != DC_OK) { delete c; return rc; }
     if (adj6_dev) c->adj = adj6_dev;
@@ -1145,12 +1232,13 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
-    k_uf_local<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(labels_dev, c->adj, ne, c->parent);
-    k_uf_union<<<nblk(ne, 256), 256, 0, st>>>(labels_dev, c->adj, ne, c->parent);
+    c->epoch = c->epoch == 0x7fffffff ? 1 : c->epoch + 1;
+    k_uf_tiles<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(c->S, labels_dev, c->adj, ne, c->parent, c->tile_flag, c->epoch, c->act_elem);
     k_uf_seed<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
-    k_uf_collect<<<nblk(ne, 256), 256, 0, st>>>(c->S, labels_dev, ne, c->parent, c->comp);
-    k_seedless<<<DC_MAX_SEEDLESS, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
+    k_uf_resolve<<<c->num_sms * 4, 256, 0, st>>>(c->S, c->act_elem, c->parent, c->comp);
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
+    k_seedless<<<32, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
+    k_uf_fix<<<c->num_sms * 4, 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
     c->launches_classify = 21 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);

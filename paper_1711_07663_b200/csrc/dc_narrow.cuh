@@ -345,11 +345,13 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
             // ---- result of the finished solve (an attained distance is an upper bound whether converged or not)
             cnt.newton++; cnt.iters += s.iters;
             atomicMin(best + b, d2u(R.dist));
-            if (R.dist > tau_exit) {
+            // (a seed only tightens best[b]: its pair comes back as a leaf, and which pair is the seed depends on the
+            // arrival order of the faces in their bins -- results must not: dmin and the keys come from leaves alone)
+            if (R.dist > tau_exit && !seed) {
                 atomicMin(dmin + b, d2u(R.dist));
                 const unsigned long long key = (d2u(R.dist) & ~0xffull) | (unsigned long long)cos_code(R.cosv);
                 atomicMin(pair_key + it.p, key);
-                if (!R.converged && !seed) {
+                if (!R.converged) {
                     // unconverged: the distance above stands as an upper bound and the leaf is quartered (a seed solve is
                     // never split: the roots cover its pair)
                     cnt.fail++;
