@@ -117,26 +117,30 @@ __device__ __forceinline__ double higher_order_const(const double *A /*[27]*/)
 }
 
 // value and first derivatives of one coordinate at (u,v)
-__device__ __forceinline__ void eval_d1(const double *A, double u, double v, double &p, double &pu, double &pv)
+// (coefficients come through an accessor A(m), m = i + 3 j: registers, shared memory or a pointer)
+template <class CF>
+__device__ __forceinline__ void eval_d1(CF A, double u, double v, double &p, double &pu, double &pv)
 {
     const double u2 = u + u, v2 = v + v;
-    const double r0 = fma(u, fma(u, A[2], A[1]), A[0]);
-    const double r1 = fma(u, fma(u, A[5], A[4]), A[3]);
-    const double r2 = fma(u, fma(u, A[8], A[7]), A[6]);
-    const double d0 = fma(u2, A[2], A[1]);
-    const double d1 = fma(u2, A[5], A[4]);
-    const double d2 = fma(u2, A[8], A[7]);
+    const double a0 = A(0), a1 = A(1), a2 = A(2), a3 = A(3), a4 = A(4), a5 = A(5), a6 = A(6), a7 = A(7), a8 = A(8);
+    const double r0 = fma(u, fma(u, a2, a1), a0);
+    const double r1 = fma(u, fma(u, a5, a4), a3);
+    const double r2 = fma(u, fma(u, a8, a7), a6);
+    const double d0 = fma(u2, a2, a1);
+    const double d1 = fma(u2, a5, a4);
+    const double d2 = fma(u2, a8, a7);
     p = fma(v, fma(v, r2, r1), r0);
     pv = fma(v2, r2, r1);
     pu = fma(v, fma(v, d2, d1), d0);
 }
 
 // value of one coordinate at (u,v)
-__device__ __forceinline__ double eval_d0(const double *A, double u, double v)
+template <class CF>
+__device__ __forceinline__ double eval_d0(CF A, double u, double v)
 {
-    const double r0 = fma(u, fma(u, A[2], A[1]), A[0]);
-    const double r1 = fma(u, fma(u, A[5], A[4]), A[3]);
-    const double r2 = fma(u, fma(u, A[8], A[7]), A[6]);
+    const double r0 = fma(u, fma(u, A(2), A(1)), A(0));
+    const double r1 = fma(u, fma(u, A(5), A(4)), A(3));
+    const double r2 = fma(u, fma(u, A(8), A(7)), A(6));
     return fma(v, fma(v, r2, r1), r0);
 }
 
@@ -176,6 +180,10 @@ __device__ __forceinline__ void scalar_range(const double *g, double uc, double 
     }
 }
 
+#ifndef DC_CD_SWEEPS
+#define DC_CD_SWEEPS 3
+#endif
+
 // reciprocal of a positive normal-range double: hardware seed + two Newton steps (no slow path)
 __device__ __forceinline__ double rcp_pos(double x)
 {
@@ -186,16 +194,40 @@ __device__ __forceinline__ double rcp_pos(double x)
     return y;
 }
 
-#ifndef DC_CD_SWEEPS
-#define DC_CD_SWEEPS 3
-#endif
+// Closest pair of the first-order model min |r + J a|, a in [-1,1]^4, J = [h P_u, h P_v, -h Q_s, -h Q_t]: DC_CD_SWEEPS
+// sweeps of exact coordinate minimisation with clamping (rho = r + J a only ever shrinks).  nrm[i] = |J_i|^2.
+__device__ __forceinline__ void model_closest_pair(const double *r, const double *pu, const double *pv, const double *qs,
+                                                   const double *qt, double n0, double n1, double n2, double n3,
+                                                   double hP, double hQ, double *a)
+{
+    const double sc4[4] = { hP, hP, -hQ, -hQ };
+    const double *col[4] = { pu, pv, qs, qt };
+    const double nrm[4] = { n0, n1, n2, n3 };
+    double inv[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { inv[i] = nrm[i] > 1e-300 ? rcp_pos(nrm[i]) * sc4[i] : 0.0; a[i] = 0.0; }
+    double rho[3] = { r[0], r[1], r[2] };
+#pragma unroll
+    for (int sw = 0; sw < DC_CD_SWEEPS; ++sw)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const double *J = col[i];
+            const double dot = J[0] * rho[0] + J[1] * rho[1] + J[2] * rho[2];      // (J_i . rho) / h_i
+            double t = fma(-dot, inv[i], a[i]);
+            t = dmax2(-1.0, dmin2(1.0, t));
+            const double da = (t - a[i]) * sc4[i];
+            rho[0] = fma(J[0], da, rho[0]); rho[1] = fma(J[1], da, rho[1]); rho[2] = fma(J[2], da, rho[2]);
+            a[i] = t;
+        }
+}
 
 struct NodeOut {
     double ub, lb; bool leaf, splitP;
     double x0[4];                                  // closest pair of the first-order model, local coordinates
 };
 
-__device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ, double KP, double KQ,
+template <class CP, class CQ>
+__device__ __forceinline__ NodeOut bound_node(CP AP, CQ AQ, double KP, double KQ,
                                               double uc, double vc, double hP, double sc, double tc, double hQ,
                                               double theta2)
 {
@@ -203,8 +235,8 @@ __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double p, q;
-        eval_d1(AP + 9 * c, uc, vc, p, pu[c], pv[c]);
-        eval_d1(AQ + 9 * c, sc, tc, q, qs[c], qt[c]);
+        eval_d1([&](int m) { return AP(9 * c + m); }, uc, vc, p, pu[c], pv[c]);
+        eval_d1([&](int m) { return AQ(9 * c + m); }, sc, tc, q, qs[c], qt[c]);
         r[c] = p - q;
     }
     NodeOut o;
@@ -222,36 +254,17 @@ __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ
         o.leaf = okP && okQ;
         o.splitP = S1P >= S1Q;
     }
-    // closest pair of the first-order model: exact coordinate minimisation with clamping, rho = r_c + J a
-    double a[4] = { 0.0, 0.0, 0.0, 0.0 };
-    {
-        const double sc4[4] = { hP, hP, -hQ, -hQ };
-        const double *col[4] = { pu, pv, qs, qt };
-        const double nrm[4] = { hP2 * npu, hP2 * npv, hQ2 * nqs, hQ2 * nqt };
-        double inv[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) inv[i] = nrm[i] > 1e-300 ? rcp_pos(nrm[i]) * sc4[i] : 0.0;
-        double rho[3] = { r[0], r[1], r[2] };
-#pragma unroll
-        for (int sw = 0; sw < DC_CD_SWEEPS; ++sw)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const double *J = col[i];
-                const double dot = J[0] * rho[0] + J[1] * rho[1] + J[2] * rho[2];      // (J_i . rho) / h_i
-                double t = fma(-dot, inv[i], a[i]);
-                t = dmax2(-1.0, dmin2(1.0, t));
-                const double da = (t - a[i]) * sc4[i];
-                rho[0] = fma(J[0], da, rho[0]); rho[1] = fma(J[1], da, rho[1]); rho[2] = fma(J[2], da, rho[2]);
-                a[i] = t;
-            }
-    }
+    // closest pair of the first-order model
+    double a[4];
+    model_closest_pair(r, pu, pv, qs, qt, hP2 * npu, hP2 * npv, hQ2 * nqs, hQ2 * nqt, hP, hQ, a);
 #pragma unroll
     for (int i = 0; i < 4; ++i) o.x0[i] = a[i];
     // the true patches at x0
     const double u0 = fma(hP, a[0], uc), v0 = fma(hP, a[1], vc), s0 = fma(hQ, a[2], sc), t0 = fma(hQ, a[3], tc);
     double r0[3];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) r0[c] = eval_d0(AP + 9 * c, u0, v0) - eval_d0(AQ + 9 * c, s0, t0);
+    for (int c = 0; c < 3; ++c)
+        r0[c] = eval_d0([&](int m) { return AP(9 * c + m); }, u0, v0) - eval_d0([&](int m) { return AQ(9 * c + m); }, s0, t0);
     const double d20 = r0[0] * r0[0] + r0[1] * r0[1] + r0[2] * r0[2];
     // direction of the bound: the closest pair's (the centre's if the patches touch there)
     const bool use0 = d20 > 0.0;
@@ -264,8 +277,8 @@ __device__ __forceinline__ NodeOut bound_node(const double *AP, const double *AQ
     double gP[9], gQ[9];
 #pragma unroll
     for (int m = 1; m < 9; ++m) {
-        gP[m] = fma(n[2], AP[18 + m], fma(n[1], AP[9 + m], n[0] * AP[m]));
-        gQ[m] = fma(n[2], AQ[18 + m], fma(n[1], AQ[9 + m], n[0] * AQ[m]));
+        gP[m] = fma(n[2], AP(18 + m), fma(n[1], AP(9 + m), n[0] * AP(m)));
+        gQ[m] = fma(n[2], AQ(18 + m), fma(n[1], AQ(9 + m), n[0] * AQ(m)));
     }
     double loP, hiP, loQ, hiQ;
     scalar_range(gP, uc, vc, hP, loP, hiP);

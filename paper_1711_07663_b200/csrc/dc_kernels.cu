@@ -794,7 +794,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                 const NItem it = st[--top];
                 double uc, vc, hP, sc, tc, hQ;
                 nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                const NodeOut nb = bound_node(AP, AQ, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
+                const NodeOut nb = bound_node([&](int m) { return AP[m]; }, [&](int m) { return AQ[m]; }, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
                 double best = u2d(s_best);
                 if (nb.ub < best) { atomicMin(&s_best, d2u(nb.ub)); best = nb.ub; }
                 if (nb.lb > best + t_tie) continue;

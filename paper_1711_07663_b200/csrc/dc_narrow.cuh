@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(128) k_np_stage(const DcScalars *S, const doub
 #ifndef NW_OVF_MAXIT
 #define NW_OVF_MAXIT 20              /* evaluations a sub-leaf of an unconverged leaf may take (a quarter of the box) */
 #endif
-#define NW_SEED_MAXIT 8              /* evaluations a seed solve may take */
+#define NW_SEED_MAXIT 5              /* evaluations a seed solve may take */
 #ifndef NW_BUDGET1
 #define NW_BUDGET1 20                 /* busy lanes below which a warp of pass 1 hands its stragglers on */
 #endif
@@ -298,7 +298,17 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
         double uc, vc, hP, sc, tc, hQ;
         nitem_box(it, uc, vc, hP, sc, tc, hQ);
         double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };
-        if (MODE == 0) {
+        if (MODE == 0 && !nqx) {
+            // a seed (a whole patch pair, centre (0,0)): its own first-order model from the coefficients themselves
+            const double r[3] = { cf(0) - cf(27), cf(9) - cf(36), cf(18) - cf(45) };
+            const double pu[3] = { cf(1), cf(10), cf(19) }, pv[3] = { cf(3), cf(12), cf(21) };
+            const double qs[3] = { cf(28), cf(37), cf(46) }, qt[3] = { cf(30), cf(39), cf(48) };
+            double a[4];
+            model_closest_pair(r, pu, pv, qs, qt, pu[0] * pu[0] + pu[1] * pu[1] + pu[2] * pu[2], pv[0] * pv[0] + pv[1] * pv[1] + pv[2] * pv[2],
+                               qs[0] * qs[0] + qs[1] * qs[1] + qs[2] * qs[2], qt[0] * qt[0] + qt[1] * qt[1] + qt[2] * qt[2], 1.0, 1.0, a);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) s.x[j] = a[j];
+        } else if (MODE == 0) {
             // start at the closest pair of the leaf's first-order model (on a bound when the fixed point says so)
             const double q15 = 1.0 / 32767.0;
             const double cen[4] = { uc, vc, sc, tc }, hw[4] = { hP, hP, hQ, hQ };
@@ -394,8 +404,10 @@ __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__res
                                                   const unsigned long long *__restrict__ best, long long max_pairs,
                                                   NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
 {
+    __shared__ int s_wsum[8];
+    __shared__ int s_base, s_total;
     const long long n_pairs = min((long long)S->n_pairs, max_pairs);
-    const long long n_round = (n_pairs + 31) & ~31LL;
+    const long long n_round = (n_pairs + 255) & ~255LL;          // (uniform trip count inside a CTA: barriers below)
     const double t_tie = S->t_tie, tau_exit = S->tau_exit;
     const int lane = threadIdx.x & 31;
     for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < n_round; p += (long long)gridDim.x * blockDim.x) {
@@ -428,12 +440,22 @@ __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__res
         int incl = mine;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        // one atomic per CTA and round (a returning atomic on ONE address costs about a third of a nanosecond of the whole
+        // GPU's time: one per warp was a third of this kernel)
+        if (lane == 31) s_wsum[threadIdx.x >> 5] = incl;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int t = 0;
+#pragma unroll
+            for (int w2 = 0; w2 < 8; ++w2) { const int v = s_wsum[w2]; s_wsum[w2] = t; t += v; }
+            s_base = t ? atomicAdd(qout_n, t) : 0;
+            s_total = t;
+        }
+        __syncthreads();
+        const int cbase = s_base, start = cbase + s_wsum[threadIdx.x >> 5], total = s_total;
+        __syncthreads();
         if (total == 0) continue;
-        int start = 0;
-        if (lane == 31) start = atomicAdd(qout_n, total);
-        start = __shfl_sync(0xffffffffu, start, 31);
-        if ((long long)start + total > qcap) { if (lane == 0) atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW); continue; }
+        if ((long long)cbase + total > qcap) { if (threadIdx.x == 0) atomicOr(&S->status, DC_STATUS_QUEUE_OVERFLOW); continue; }
         long long slot = (long long)start + incl - mine;
         while (mask) {
             const int k = __ffs(mask) - 1; mask &= mask - 1;
@@ -479,7 +501,8 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                     const double2 vq = __ldg(reinterpret_cast<const double2 *>(AQg) + m);
                     AP[2 * m] = vp.x; AP[2 * m + 1] = vp.y; AQ[2 * m] = vq.x; AQ[2 * m + 1] = vq.y;
                 }
-                const NodeOut o = bound_node(AP, AQ, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
+                const NodeOut o = bound_node([&](int m) { return AP[m]; }, [&](int m) { return AQ[m]; }, AP[27], AQ[27],
+                                             uc, vc, hP, sc, tc, hQ, theta2);
                 cnt.nodes++;
                 if (o.ub < bst) { atomicMin(best + b, d2u(o.ub)); bst = o.ub; }
                 const bool alive = o.ub > tau_exit && o.lb <= bst + t_tie;
