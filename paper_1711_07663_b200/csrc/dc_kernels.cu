@@ -2,9 +2,9 @@
 //
 // Step names follow SURVEY.md 8(a) / DESIGN.md:
 //   S1 face prep      k_face_boxes, k_setup_surface
-//   S3 face bins      k_face_hist, k_scan_sums, k_scan_cells, k_face_scatter        (Morton-ordered uniform bins)
+//   S3 face bins      k_face_hist, k_scan_sums, k_scan_cells, k_cell_occ, k_face_scatter   (uniform bins, rows along x contiguous)
 //   S2 element boxes  k_elem_boxes                                    (HBM-bound stream)
-//   S4 candidates     k_filter (thread/element), k_pairs (warp/active element, warp-aggregated append)
+//   S4 candidates     k_filter (thread/element), k_pairs (16 lanes/active element, one append per element)
 //   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound, k_np_bound_tail (FP64)
 //   S6 decide         k_np_decide
 //   S7 flood fill     k_uf_tiles, k_uf_seed, k_uf_resolve, k_uf_assign, k_seedless, k_uf_fix
@@ -25,7 +25,8 @@
 using namespace dcg;
 
 #define DC_MAX_SEEDLESS 1024           /* seedless components resolved per cut (each by one exhaustive query) */
-#define DC_GRID_MAX 64              /* face-bin cells per axis (Morton code: 6 bits per axis) */
+#define DC_GRID_MAX 64              /* face-bin cells per axis; cell (x,y,z) has code x + 64 (y + 64 z): a row along x is contiguous */
+#define DC_OCC (DC_GRID_MAX / 4)    /* coarse occupancy grid: 4 x 4 x 4 cells per entry */
 #define DC_NCELL (DC_GRID_MAX * DC_GRID_MAX * DC_GRID_MAX)
 #define DC_NQN 28                   /* >= DC_MAX_ROUNDS + 2 */
 #define DC_GRID_ROUNDS 4             /* branch-and-bound rounds launched as grids; the rest run inside one CTA */
@@ -70,18 +71,7 @@ struct DcScalars {
 __device__ __forceinline__ void atomic_min_d(unsigned long long *addr, double v) { atomicMin(addr, enc_ord(v)); }
 __device__ __forceinline__ void atomic_max_d(unsigned long long *addr, double v) { atomicMax(addr, enc_ord(v)); }
 
-__device__ __forceinline__ unsigned morton3(unsigned x, unsigned y, unsigned z)
-{
-    auto spread = [](unsigned v) {
-        v &= 0x3ffu;
-        v = (v | (v << 16)) & 0x030000ffu;
-        v = (v | (v << 8)) & 0x0300f00fu;
-        v = (v | (v << 4)) & 0x030c30c3u;
-        v = (v | (v << 2)) & 0x09249249u;
-        return v;
-    };
-    return spread(x) | (spread(y) << 1) | (spread(z) << 2);
-}
+__device__ __forceinline__ int cell_code(int x, int y, int z) { return x + DC_GRID_MAX * (y + DC_GRID_MAX * z); }
 
 // Bezier control values of a 1-D quadratic through nodes (-1,0,1): b0 = x0, b1 = 2 x1 - (x0+x2)/2,
 // b2 = x2 (convex-hull property => conservative boxes; Lagrange NODES do not bound the patch).
@@ -172,7 +162,7 @@ __device__ __forceinline__ int cell_coord(const DcScalars *S, double x, int c)
     return i < 0 ? 0 : (i >= S->dims[c] ? S->dims[c] - 1 : i);
 }
 
-// S3: histogram of faces over cells keyed by the Morton code of the box-centre cell
+// S3: histogram of faces over cells keyed by the code of the box-centre cell
 __global__ void k_face_hist(const DcScalars *S, const double *__restrict__ fbox_orig, int n_face,
                             int *__restrict__ fcell, int *cell_count)
 {
@@ -182,12 +172,12 @@ __global__ void k_face_hist(const DcScalars *S, const double *__restrict__ fbox_
 #pragma unroll
     for (int c = 0; c < 3; ++c)
         ic[c] = cell_coord(S, 0.5 * (fbox_orig[(size_t)f * 6 + c] + fbox_orig[(size_t)f * 6 + 3 + c]), c);
-    const int code = (int)morton3(ic[0], ic[1], ic[2]);
+    const int code = cell_code(ic[0], ic[1], ic[2]);
     fcell[f] = code;
     atomicAdd(&cell_count[code], 1);
 }
 
-// exclusive scan over the DC_NCELL Morton-ordered cells in two coalesced passes: per-chunk sums (one CTA of
+// exclusive scan over the DC_NCELL cells in two coalesced passes: per-chunk sums (one CTA of
 // 256 threads per 1024 cells, int4 loads), then every CTA adds the sums of the chunks before it to a local scan.
 #define SCAN_CHUNK 1024
 #define SCAN_NCHUNK (DC_NCELL / SCAN_CHUNK)
@@ -232,6 +222,22 @@ __global__ void __launch_bounds__(256) k_scan_cells(const int *__restrict__ cell
     o.x = before + woff + incl - mine; o.y = o.x + v.x; o.z = o.y + v.y; o.w = o.z + v.z;
     reinterpret_cast<int4 *>(cell_start)[blockIdx.x * 256 + threadIdx.x] = o;
     if (blockIdx.x == SCAN_NCHUNK - 1 && threadIdx.x == 255) cell_start[DC_NCELL] = o.w + v.w;
+}
+
+// coarse occupancy: does any face sit in the 4 x 4 x 4 cells of a coarse entry (k_filter's first look: most elements
+// near the surface's box are in empty space)
+__global__ void k_cell_occ(const int *__restrict__ cell_start, unsigned char *__restrict__ occ)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= DC_OCC * DC_OCC * DC_OCC) return;
+    const int X = t % DC_OCC, Y = (t / DC_OCC) % DC_OCC, Z = t / (DC_OCC * DC_OCC);
+    int n = 0;
+    for (int z = 4 * Z; z < 4 * Z + 4; ++z)
+        for (int y = 4 * Y; y < 4 * Y + 4; ++y) {
+            const int c0 = cell_code(4 * X, y, z);
+            n += cell_start[c0 + 4] - cell_start[c0];
+        }
+    occ[t] = n > 0;
 }
 
 // scatter faces into cell order; write sorted boxes and monomial coefficients (stride 28 doubles)
@@ -373,71 +379,52 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
 }
 
 // ------------------------------------------------------------------------------------------
-// S4a: one thread per element.  Initialises the per-element state of this cut and appends the
-// elements whose inflated box overlaps a non-empty 4x4x4 block of face cells to the active list
-// (warp-aggregated atomic append).  A block of 64 cells is one contiguous range of the Morton order.
-// faces of the Morton-aligned block of 2^s x 2^s x 2^s cells with block coordinates (bx, by, bz): ONE contiguous range
-__device__ __forceinline__ int block_faces(const int *__restrict__ cell_start, int bx, int by, int bz, int s, int &first)
+// S4a: one thread per element.  Initialises the per-element state of this cut and appends the elements whose inflated
+// box meets a face cell that is not empty to the active list (warp-aggregated atomic append).  Coarse to fine: most
+// elements near the surface's box sit in empty space, and the (at most 27, usually 8) coarse occupancy bytes say so;
+// only the others look at the cell rows k_pairs will walk (a row of cells along x is ONE contiguous face range).
+__device__ __forceinline__ bool filter_test(const DcScalars *S, const int *__restrict__ cell_start,
+                                            const unsigned char *__restrict__ occ, const double *lo, const double *hi)
 {
-    const unsigned c0 = morton3(bx, by, bz) << (3 * s);
-    first = __ldg(cell_start + c0);
-    return __ldg(cell_start + c0 + (1u << (3 * s))) - first;
-}
-// block level of a query over the cells [i0, i1]: the finest one with at most 4 blocks per axis (64 ranges, two
-// per lane); the blocks then cover at most (4 / 3)^3 ... 2^3 times the cells of the query, whatever its size
-__device__ __forceinline__ int block_level(const int *i0, const int *i1)
-{
-    int s = 0;
-    while (s < 7 && (((i1[0] >> s) - (i0[0] >> s)) > 3 || ((i1[1] >> s) - (i0[1] >> s)) > 3 || ((i1[2] >> s) - (i0[2] >> s)) > 3)) ++s;
-    return s;
+    double d2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double g = dmax2(0.0, dmax2(S->smin[c] - hi[c], lo[c] - S->smax[c]));
+        d2 = fma(g, g, d2);
+    }
+    const double reach = S->reach;
+    if (!(d2 <= reach * reach)) return false;
+    const double pad = reach + S->fhalf;
+    int i0[3], i1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c); }
+    bool maybe = false;
+    for (int z = i0[2] >> 2; z <= (i1[2] >> 2) && !maybe; ++z)
+        for (int y = i0[1] >> 2; y <= (i1[1] >> 2) && !maybe; ++y)
+            for (int x = i0[0] >> 2; x <= (i1[0] >> 2); ++x)
+                if (__ldg(occ + x + DC_OCC * (y + DC_OCC * z))) { maybe = true; break; }
+    if (!maybe) return false;
+    for (int z = i0[2]; z <= i1[2]; ++z)
+        for (int y = i0[1]; y <= i1[1]; ++y) {
+            const int c0 = cell_code(0, y, z);
+            if (__ldg(cell_start + c0 + i1[0] + 1) - __ldg(cell_start + c0 + i0[0]) > 0) return true;
+        }
+    return false;
 }
 
 __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
                          signed char *__restrict__ labels, int *__restrict__ parent,
                          unsigned char *__restrict__ comp, const int *__restrict__ cell_start,
-                         int *__restrict__ act_elem)
+                         const unsigned char *__restrict__ occ, int *__restrict__ act_elem)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     bool active = false;
     if (e < n_elem) {
-        labels[e] = -1; comp[e] = 0;       // (parent[] is initialised by k_uf_local)
+        labels[e] = -1; comp[e] = 0;       // (parent[] is initialised by k_uf_tiles)
         double lo[3], hi[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) { lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e]; }
-        double d2 = 0.0;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const double g = dmax2(0.0, dmax2(S->smin[c] - hi[c], lo[c] - S->smax[c]));
-            d2 = fma(g, g, d2);
-        }
-        const double reach = S->reach;
-        if (d2 <= reach * reach) {
-            const double pad = reach + S->fhalf;
-            int i0[3], i1[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c); }
-            // coarse to fine: most elements near the surface AABB sit in empty space, and at most 8 blocks two levels up
-            // say so; only the others look at the (<= 64) blocks k_pairs will walk
-            const int sl = block_level(i0, i1);
-            bool maybe = false;
-            {
-                int sc = sl;
-                while (sc < 7 && (((i1[0] >> sc) - (i0[0] >> sc)) > 1 || ((i1[1] >> sc) - (i0[1] >> sc)) > 1 || ((i1[2] >> sc) - (i0[2] >> sc)) > 1)) ++sc;
-                for (int z = i0[2] >> sc; z <= (i1[2] >> sc) && !maybe; ++z)
-                    for (int y = i0[1] >> sc; y <= (i1[1] >> sc) && !maybe; ++y)
-                        for (int x = i0[0] >> sc; x <= (i1[0] >> sc); ++x) {
-                            int first;
-                            if (block_faces(cell_start, x, y, z, sc, first) > 0) { maybe = true; break; }
-                        }
-            }
-            if (maybe)
-                for (int z = i0[2] >> sl; z <= (i1[2] >> sl) && !active; ++z)
-                    for (int y = i0[1] >> sl; y <= (i1[1] >> sl) && !active; ++y)
-                        for (int x = i0[0] >> sl; x <= (i1[0] >> sl); ++x) {
-                            int first;
-                            if (block_faces(cell_start, x, y, z, sl, first) > 0) { active = true; break; }
-                        }
-        }
+        active = filter_test(S, cell_start, occ, lo, hi);
     }
     const unsigned m = __ballot_sync(0xffffffffu, active);
     if (m) {
@@ -449,13 +436,12 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
     }
 }
 
-// S4b: one warp per active element.  The 4x4x4 cell blocks its inflated box overlaps (at most 27 for an
-// element smaller than a block) are one contiguous face range each in the Morton order: one lane per block
-// fetches its range, the ranges are concatenated by a warp scan, and the lanes then walk the concatenation
-// 32 faces at a time (coalesced face-box loads, every lane busy) applying the box test of Algorithm A.2
-// (PAPER.md L689-L709).  Survivors are staged in shared memory and written as ONE contiguous segment of
-// the pair list (one atomic per element); an element with more survivors than the stage holds re-walks its
-// ranges and writes directly.  pair_key is initialised to +inf for S5.
+// S4b: a group of 16 lanes per active element.  The cells its inflated box overlaps are (ny x nz) ROWS along x, one
+// contiguous face range each: one lane per row fetches its range, the ranges are concatenated by a scan over the
+// group, and the lanes then walk the concatenation 16 faces at a time (coalesced face-box loads, every lane busy)
+// applying the box test of Algorithm A.2.  Survivors are staged in shared memory and written as
+// ONE contiguous segment of the pair list (one atomic per element); an element with more survivors than the stage
+// holds re-walks its ranges and writes directly.  pair_key is initialised to +inf for S5.
 __device__ __forceinline__ double box_dist2(const double *lo, const double *hi, const double *fb)
 {
     double d2 = 0.0;
@@ -497,16 +483,13 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
     for (int a = warp; a < n_active; a += nwarps) {
         const long long e = act_elem[a];
         double lo[3], hi[3];
-        int b0[3], nb[3], i0[3], i1[3];
+        int i0[3], i1[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             lo[c] = ebox[(size_t)c * n_elem + e]; hi[c] = ebox[(size_t)(3 + c) * n_elem + e];
             i0[c] = cell_coord(S, lo[c] - pad, c); i1[c] = cell_coord(S, hi[c] + pad, c);
         }
-        const int sl = block_level(i0, i1);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) { b0[c] = i0[c] >> sl; nb[c] = (i1[c] >> sl) - b0[c] + 1; }
-        const int nblk = nb[0] * nb[1] * nb[2];
+        const int ny = i1[1] - i0[1] + 1, nblk = ny * (i1[2] - i0[2] + 1);      // rows of cells along x
         long long base = 0;
         int total = 0, bslot = 0;
         unsigned long long skey = ~0ull;
@@ -515,7 +498,11 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
             for (int bbase = 0; bbase < nblk; bbase += PR_W) {
                 const int bi = bbase + lane;
                 int cnt = 0, first = 0;
-                if (bi < nblk) cnt = block_faces(cell_start, b0[0] + bi % nb[0], b0[1] + (bi / nb[0]) % nb[1], b0[2] + bi / (nb[0] * nb[1]), sl, first);
+                if (bi < nblk) {
+                    const int c0 = cell_code(0, i0[1] + bi % ny, i0[2] + bi / ny);
+                    first = __ldg(cell_start + c0 + i0[0]);
+                    cnt = __ldg(cell_start + c0 + i1[0] + 1) - first;
+                }
                 int incl = cnt;
 #pragma unroll
                 for (int o = 1; o < PR_W; o <<= 1) { const int v = __shfl_up_sync(gmask, incl, o, PR_W); if (lane >= o) incl += v; }
@@ -962,7 +949,7 @@ struct dc_ctx {
     NItem *q[2], *nq; NLeafX *nqx;
     int *pair_face; unsigned long long *pair_key; int *pair_band;
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
-    int *cell_count, *cell_start, *cell_fill;
+    int *cell_count, *cell_start, *cell_fill; unsigned char *occ;
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
     cudaEvent_t ev[12];
     cudaStream_t last_stream;
@@ -977,7 +964,7 @@ struct WsLayout {
     size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_tile_flag, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
         off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq, off_nqx,
         off_pair_face, off_pair_key, off_pair_band, off_fbox_orig, off_fbox, off_fcoef, off_fcell, off_fperm,
-        off_cell_count, off_cell_start, off_cell_fill, off_hfaces, off_hlabels, off_hsdist, total;
+        off_cell_count, off_cell_start, off_cell_fill, off_occ, off_hfaces, off_hlabels, off_hsdist, total;
     long long max_band, qcap;
 };
 
@@ -1028,6 +1015,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_cell_count = take((size_t)(DC_NCELL + 1) * 4);
     L.off_cell_start = take((size_t)(DC_NCELL + 1) * 4);
     L.off_cell_fill = take((size_t)(DC_NCELL + 8 + SCAN_NCHUNK) * 4);   // + the scan's chunk sums
+    L.off_occ = take((size_t)DC_OCC * DC_OCC * DC_OCC);
     L.off_hfaces = take((size_t)max_faces * 27 * 8);
     L.off_hlabels = take((size_t)n_elem);
     L.off_hsdist = take((size_t)n_elem * 8);
@@ -1107,6 +1095,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->cell_count = (int *)(c->ws + L.off_cell_count);
     c->cell_start = (int *)(c->ws + L.off_cell_start);
     c->cell_fill = (int *)(c->ws + L.off_cell_fill);
+    c->occ = c->ws + L.off_occ;
     c->h_faces_dev = (double *)(c->ws + L.off_hfaces);
     c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
     c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
@@ -1150,11 +1139,12 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
     k_face_hist<<<nblk(nf, 128), 128, 0, st>>>(c->S, c->fbox_orig, nf, c->fcell, c->cell_count);
     k_scan_sums<<<SCAN_NCHUNK, 256, 0, st>>>(c->cell_count, c->cell_fill + DC_NCELL + 8);
     k_scan_cells<<<SCAN_NCHUNK, 256, 0, st>>>(c->cell_count, c->cell_fill + DC_NCELL + 8, c->cell_start);
+    k_cell_occ<<<(DC_OCC * DC_OCC * DC_OCC + 127) / 128, 128, 0, st>>>(c->cell_start, c->occ);
     k_face_scatter<<<nblk(nf, 128), 128, 0, st>>>(face_nodes_dev, c->fbox_orig, c->fcell, c->cell_start, c->cell_fill,
                                                    nf, c->fperm, c->fbox, c->fcoef);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[9], st));
-    c->launches_surface = 7;
+    c->launches_surface = 8;
     c->have_surface = true;
     return DC_OK;
 }
@@ -1173,7 +1163,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     if (P.flags & DC_FLAG_RECOMPUTE_BOXES) { int rc = run_elem_boxes(c, st); if (rc) return rc; }
     CK(cudaEventRecord(c->ev[1], st));
     k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
-    k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->act_elem);
+    k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->occ, c->act_elem);
     k_pairs<<<c->num_sms * 16, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
                                            c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key,
                                            c->pair_band, c->nq, c->best, c->dmin);
