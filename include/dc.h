@@ -98,7 +98,12 @@ typedef struct {
     double l_ref, tau_cut, d_band;
     float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
                                     4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface,
-                                    7 the k_np_newton launches of S5 (seed, leaf and overflow solves: the dominant kernel) */
+                                    7 every k_np_solve launch of S5 (seeds + leaf passes + overflow rounds, the latter
+                                      with their two short k_np_bound passes) */
+    float ms_kernel[8];          /* the kernels of S5/S6 one by one (CUDA events on the caller's stream):
+                                    0 k_np_stage, 1 k_np_solve on the seeds, 2 k_np_roots, 3 k_np_bound (all rounds + tail),
+                                    4 k_np_compact, 5 k_np_solve leaf passes 1-3, 6 overflow rounds (2 x bound + solve),
+                                    7 k_np_decide */
     int status;                  /* DC_STATUS_* bits */
     int n_launches;              /* kernels launched by the last dc_set_cut_surface + dc_classify */
 } dc_stats;
@@ -128,7 +133,7 @@ int dc_create_grid(dc_ctx **out, int device,
 /*
  * Set the cutting surface (L171-L175: "each partition gathers all of its potential cutting
  * surfaces"; L215 "outward-oriented normal").  Runs S1 (face Bezier boxes, monomial
- * coefficients, surface AABB -> L_ref) and S3 (Morton-ordered uniform face bins).
+ * coefficients, surface AABB -> L_ref) and S3 (uniform face bins, a row of cells contiguous).
  *   face_nodes_dev [n_face][9][3] f64 dev, m = i + 3 j, normal x_s cross x_t points OUT of the body.
  */
 int dc_set_cut_surface(dc_ctx *ctx, long long n_face, const double *face_nodes_dev, void *stream);

@@ -39,13 +39,13 @@ class dc_stats(C.Structure):
                 ("n_seedless_components", C.c_longlong), ("n_fill_conflicts", C.c_longlong),
                 ("pairs_needed", C.c_longlong), ("queue_peak", C.c_longlong),
                 ("l_ref", C.c_double), ("tau_cut", C.c_double), ("d_band", C.c_double),
-                ("ms_stage", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int)]
+                ("ms_stage", C.c_float * 8), ("ms_kernel", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int)]
 
     def as_dict(self) -> dict:
         d = {}
         for k, _ in self._fields_:
             v = getattr(self, k)
-            d[k] = list(v) if k == "ms_stage" else v
+            d[k] = list(v) if k in ("ms_stage", "ms_kernel") else v
         return d
 
 

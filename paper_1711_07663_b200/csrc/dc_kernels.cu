@@ -951,7 +951,7 @@ struct dc_ctx {
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm;
     int *cell_count, *cell_start, *cell_fill; unsigned char *occ;
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
-    cudaEvent_t ev[12];
+    cudaEvent_t ev[12], evk[10];    // evk: boundaries between the kernels of S5/S6
     cudaStream_t last_stream;
     bool have_surface, have_cut;
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
@@ -1102,6 +1102,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     for (int i = 0; i < 12; ++i) CK(cudaEventCreate(&c->ev[i]));
+    for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->evk[i]));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
     CK(cudaMemsetAsync(c->tile_flag, 0, (size_t)(n_elem / UF_TILE + 2) * 4, st));
@@ -1183,6 +1184,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
                                                c->q[0], &S->qn[0], c->qcap);
     // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
     // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
+    CK(cudaEventRecord(c->evk[0], st));
     const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     const int rounds = 2 * max_level + 1;
     const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
@@ -1202,12 +1204,14 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     NItem *ovf1 = (NItem *)c->nqx + c->qcap / 2;
     const long long cap_ovf1 = c->qcap / 2;
     k_np_compact<<<c->num_sms * 8, 256, 0, st>>>(S, &S->nn[0], c->qcap, c->nq, c->nqx, c->best, lq, lqx, &S->nn[5]);
+    CK(cudaEventRecord(c->evk[1], st));
     k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[5], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
                                              c->best, c->dmin, c->pair_key, contA, &S->nh[0], capA, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET1, NW_MAXIT);
     k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[0], capA, nullptr, nullptr, contA, c->pair_face, c->fcoef, c->ecoef,
                                              c->best, c->dmin, c->pair_key, contB, &S->nh[1], capB, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET2, NW_MAXIT);
     k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[1], capB, nullptr, nullptr, contB, c->pair_face, c->fcoef, c->ecoef,
                                              c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, ovf1, &S->nn[1], cap_ovf1, 0, NW_MAXIT);
+    CK(cudaEventRecord(c->evk[2], st));
     // The sub-leaves of unconverged solves come back through one bound pass (best[b] is final or nearly so: most of them
     // are pruned) and one solve launch, twice; the last launch finishes whatever still fails on the lane that held it.
     k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
@@ -1326,7 +1330,16 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
         if (cudaEventElapsedTime(&ms, c->ev[3], c->ev[4]) == cudaSuccess) o->ms_stage[4] = ms;
         if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[4]) == cudaSuccess) o->ms_stage[5] = ms;
         if (cudaEventElapsedTime(&ms, c->ev[5], c->ev[6]) == cudaSuccess) o->ms_stage[7] = ms;
-        if (cudaEventElapsedTime(&ms, c->ev[7], c->ev[10]) == cudaSuccess) o->ms_stage[7] += ms;
+        if (cudaEventElapsedTime(&ms, c->ev[7], c->ev[10]) == cudaSuccess) { o->ms_stage[7] += ms; o->ms_kernel[1] = ms; }
+        if (cudaEventElapsedTime(&ms, c->ev[2], c->ev[7]) == cudaSuccess) o->ms_kernel[0] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[10], c->evk[0]) == cudaSuccess) o->ms_kernel[2] = ms;
+        if (cudaEventElapsedTime(&ms, c->evk[0], c->ev[5]) == cudaSuccess) o->ms_kernel[3] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[5], c->evk[1]) == cudaSuccess) o->ms_kernel[4] = ms;
+        if (cudaEventElapsedTime(&ms, c->evk[1], c->evk[2]) == cudaSuccess) o->ms_kernel[5] = ms;
+        if (cudaEventElapsedTime(&ms, c->evk[2], c->ev[6]) == cudaSuccess) o->ms_kernel[6] = ms;
+        if (cudaEventElapsedTime(&ms, c->ev[6], c->ev[3]) == cudaSuccess) o->ms_kernel[7] = ms;
+        // (ms_stage[7]: every k_np_solve launch = seeds + leaf passes + overflow rounds; the compaction pass is not in it)
+        o->ms_stage[7] = o->ms_kernel[1] + o->ms_kernel[5] + o->ms_kernel[6];
     }
     if (c->have_surface) {
         float ms;
@@ -1343,6 +1356,7 @@ extern "C" void dc_destroy(dc_ctx *c)
     cudaSetDevice(c->device);
     if (c->last_stream || true) cudaStreamSynchronize(c->last_stream);
     for (int i = 0; i < 12; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 10; ++i) if (c->evk[i]) cudaEventDestroy(c->evk[i]);
     if (c->S_host) cudaFreeHost(c->S_host);
     delete c;
 }
