@@ -154,17 +154,24 @@ __device__ __forceinline__ void mono_to_bern(double a0, double a1, double a2, do
 // range [lo, hi] of the non-constant part of the scalar biquadratic g (g[0] ignored) over the sub-rectangle
 // (uc, vc, h): re-centre and scale to [-1,1]^2, convert to the Bernstein basis, take the smallest and the largest
 // of the 9 coefficients (the function lies in their convex hull).
+template <bool ROOT>
 __device__ __forceinline__ void scalar_range(const double *g, double uc, double vc, double h, double &lo, double &hi)
 {
-    const double h2 = h * h, uc2 = uc + uc, vc2 = vc + vc;
-    // rows j = 0,1,2 (powers of v) re-centred in u: R_j0, R_j1, R_j2
-    const double R01 = h * fma(uc2, g[2], g[1]), R02 = h2 * g[2];
-    const double R10 = fma(uc, fma(uc, g[5], g[4]), g[3]), R11 = h * fma(uc2, g[5], g[4]), R12 = h2 * g[5];
-    const double R20 = fma(uc, fma(uc, g[8], g[7]), g[6]), R21 = h * fma(uc2, g[8], g[7]), R22 = h2 * g[8];
-    // columns re-centred in v: c[j][i], constant term dropped
-    const double c01 = fma(vc, fma(vc, R21, R11), R01), c02 = fma(vc, fma(vc, R22, R12), R02);
-    const double c10 = h * fma(vc2, R20, R10), c11 = h * fma(vc2, R21, R11), c12 = h * fma(vc2, R22, R12);
-    const double c20 = h2 * R20, c21 = h2 * R21, c22 = h2 * R22;
+    double c01, c02, c10, c11, c12, c20, c21, c22;
+    if (ROOT) {
+        // the whole patch (centre (0,0), half-width 1): the coefficients are already the local ones
+        c01 = g[1]; c02 = g[2]; c10 = g[3]; c11 = g[4]; c12 = g[5]; c20 = g[6]; c21 = g[7]; c22 = g[8];
+    } else {
+        const double h2 = h * h, uc2 = uc + uc, vc2 = vc + vc;
+        // rows j = 0,1,2 (powers of v) re-centred in u: R_j0, R_j1, R_j2
+        const double R01 = h * fma(uc2, g[2], g[1]), R02 = h2 * g[2];
+        const double R10 = fma(uc, fma(uc, g[5], g[4]), g[3]), R11 = h * fma(uc2, g[5], g[4]), R12 = h2 * g[5];
+        const double R20 = fma(uc, fma(uc, g[8], g[7]), g[6]), R21 = h * fma(uc2, g[8], g[7]), R22 = h2 * g[8];
+        // columns re-centred in v: c[j][i], constant term dropped
+        c01 = fma(vc, fma(vc, R21, R11), R01); c02 = fma(vc, fma(vc, R22, R12), R02);
+        c10 = h * fma(vc2, R20, R10); c11 = h * fma(vc2, R21, R11); c12 = h * fma(vc2, R22, R12);
+        c20 = h2 * R20; c21 = h2 * R21; c22 = h2 * R22;
+    }
     // Bernstein in u (rows), then in v (columns)
     double r0[3], r1[3], r2[3];
     mono_to_bern(0.0, c01, c02, r0[0], r0[1], r0[2]);
@@ -226,7 +233,10 @@ struct NodeOut {
     double x0[4];                                  // closest pair of the first-order model, local coordinates
 };
 
-template <class CP, class CQ>
+// ROOT: the node is a whole patch pair (round 0 of the branch and bound, 97 % of the nodes at config 2): the centre is
+// (0,0) and the half-widths are 1, so the centre values and first derivatives ARE coefficients (no evaluation) and the
+// scalar ranges need no re-centring.
+template <bool ROOT, class CP, class CQ>
 __device__ __forceinline__ NodeOut bound_node(CP AP, CQ AQ, double KP, double KQ,
                                               double uc, double vc, double hP, double sc, double tc, double hQ,
                                               double theta2)
@@ -235,8 +245,13 @@ __device__ __forceinline__ NodeOut bound_node(CP AP, CQ AQ, double KP, double KQ
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double p, q;
-        eval_d1([&](int m) { return AP(9 * c + m); }, uc, vc, p, pu[c], pv[c]);
-        eval_d1([&](int m) { return AQ(9 * c + m); }, sc, tc, q, qs[c], qt[c]);
+        if (ROOT) {
+            p = AP(9 * c); pu[c] = AP(9 * c + 1); pv[c] = AP(9 * c + 3);
+            q = AQ(9 * c); qs[c] = AQ(9 * c + 1); qt[c] = AQ(9 * c + 3);
+        } else {
+            eval_d1([&](int m) { return AP(9 * c + m); }, uc, vc, p, pu[c], pv[c]);
+            eval_d1([&](int m) { return AQ(9 * c + m); }, sc, tc, q, qs[c], qt[c]);
+        }
         r[c] = p - q;
     }
     NodeOut o;
@@ -281,8 +296,8 @@ __device__ __forceinline__ NodeOut bound_node(CP AP, CQ AQ, double KP, double KQ
         gQ[m] = fma(n[2], AQ(18 + m), fma(n[1], AQ(9 + m), n[0] * AQ(m)));
     }
     double loP, hiP, loQ, hiQ;
-    scalar_range(gP, uc, vc, hP, loP, hiP);
-    scalar_range(gQ, sc, tc, hQ, loQ, hiQ);
+    scalar_range<ROOT>(gP, uc, vc, hP, loP, hiP);
+    scalar_range<ROOT>(gQ, sc, tc, hQ, loQ, hiQ);
     o.lb = fma(n[2], r[2], fma(n[1], r[1], n[0] * r[0])) + loP - hiQ;
     return o;
 }

@@ -781,7 +781,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                 const NItem it = st[--top];
                 double uc, vc, hP, sc, tc, hQ;
                 nitem_box(it, uc, vc, hP, sc, tc, hQ);
-                const NodeOut nb = bound_node([&](int m) { return AP[m]; }, [&](int m) { return AQ[m]; }, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
+                const NodeOut nb = bound_node<false>([&](int m) { return AP[m]; }, [&](int m) { return AQ[m]; }, AP[27], AQ[27], uc, vc, hP, sc, tc, hQ, theta2);
                 double best = u2d(s_best);
                 if (nb.ub < best) { atomicMin(&s_best, d2u(nb.ub)); best = nb.ub; }
                 if (nb.lb > best + t_tie) continue;
@@ -1188,9 +1188,11 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     const int rounds = 2 * max_level + 1;
     const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
-    for (int r = 0; r < grid_rounds; ++r)
-        k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                               c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
+    k_np_bound<true><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                 c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
+    for (int r = 1; r < grid_rounds; ++r)
+        k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                      c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
     if (rounds > grid_rounds)
         k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                        c->nq, c->nqx, &S->nn[0], c->qcap);
@@ -1214,11 +1216,11 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     CK(cudaEventRecord(c->evk[2], st));
     // The sub-leaves of unconverged solves come back through one bound pass (best[b] is final or nearly so: most of them
     // are pruned) and one solve launch, twice; the last launch finishes whatever still fails on the lane that held it.
-    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
+    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
                                            nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[2], c->qcap, 1);
     k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[2], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
                                              c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, c->nq, &S->nn[3], c->qcap, 0, NW_OVF_MAXIT);
-    k_np_bound<<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
+    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
                                            nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[4], c->qcap, 1);
     k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[4], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
                                              c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_OVF_MAXIT);

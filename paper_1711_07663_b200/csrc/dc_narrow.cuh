@@ -468,6 +468,7 @@ __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__res
 // ------------------------------------------------------------------------------------------
 // Bound: one thread per item of qin[0 .. n): prune, or 4 children -> qout, or leaf -> the ONE leaf queue nq
 // (all rounds append to it; the Newton kernel runs once, after the last round).  Items i0, i0 + stride, ...
+template <bool ROOT>
 __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem *__restrict__ qin,
                                                const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
@@ -501,7 +502,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
                     const double2 vq = __ldg(reinterpret_cast<const double2 *>(AQg) + m);
                     AP[2 * m] = vp.x; AP[2 * m + 1] = vp.y; AQ[2 * m] = vq.x; AQ[2 * m + 1] = vq.y;
                 }
-                const NodeOut o = bound_node([&](int m) { return AP[m]; }, [&](int m) { return AQ[m]; }, AP[27], AQ[27],
+                const NodeOut o = bound_node<ROOT>([&](int m) { return AP[m]; }, [&](int m) { return AQ[m]; }, AP[27], AQ[27],
                                              uc, vc, hP, sc, tc, hQ, theta2);
                 cnt.nodes++;
                 if (o.ub < bst) { atomicMin(best + b, d2u(o.ub)); bst = o.ub; }
@@ -533,7 +534,8 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
     }
 }
 
-__global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
+template <bool ROOT>
+__global__ void __launch_bounds__(NPW_THREADS, ROOT ? 3 : 2) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
@@ -543,7 +545,7 @@ __global__ void __launch_bounds__(NPW_THREADS) k_np_bound(DcScalars *S, const in
     if (n == 0) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
     NpCounters cnt = { 0, 0, 0, 0, 0 };
-    np_bound_items(S, n, qin, pair_face, fcoef, ecoef, best, qout, qout_n, nq, nqx, nq_n, qcap,
+    np_bound_items<ROOT>(S, n, qin, pair_face, fcoef, ecoef, best, qout, qout_n, nq, nqx, nq_n, qcap,
                    blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, cnt, force_leaf != 0);
     np_flush_counters(S, cnt);
 }
@@ -561,7 +563,7 @@ __global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S,
         const int n = min(*(volatile int *)&S->qn[r], (int)min(qcap, (long long)0x7fffffff));
         if (n == 0) break;
         if (threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
-        np_bound_items(S, n, (r & 1) ? q1 : q0, pair_face, fcoef, ecoef, best, (r & 1) ? q0 : q1, &S->qn[r + 1], nq, nqx, nq_n, qcap,
+        np_bound_items<false>(S, n, (r & 1) ? q1 : q0, pair_face, fcoef, ecoef, best, (r & 1) ? q0 : q1, &S->qn[r + 1], nq, nqx, nq_n, qcap,
                        threadIdx.x, NP_TAIL_THREADS, cnt);
         __threadfence();
         __syncthreads();
