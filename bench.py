@@ -53,6 +53,7 @@ UNIT = "pair tests/s"
 # algorithmic fp64 flops per operation of the narrow phase (FMA = 2)
 FLOP_PER_BNB_NODE = 850.0       # centre evals with first derivatives 183, norms + leaf rule 45, model closest pair 250, true patches there 120,
 #                                 2 x 8 projected coefficients 80, 2 Bernstein ranges 170
+FLOP_PER_BNB_ROOT = 585.0       # a whole patch pair (round 0): no centre evaluation (-180), no re-centring in the two ranges (-85)
 FLOP_PER_NEWTON_EVAL = 560.0    # 6 jets x 36 + (r, g, H) 3 x 43 + LDL^T 4x4 ~75 + trial point and its value 6 x 16 + 17 + tests ~35
 FLOP_PER_NEWTON_FINISH = 40.0   # normal, cosine, distance of a finished solve
 # S2 algorithmic bytes: every conn row (108 B) and every node (24 B) read once, one box (48 B) written per element
@@ -502,13 +503,15 @@ def main():
     traffic = stored_traffic(cfg)
     step_ms = float(med[5] + med[6])
     # dominant kernel by time: k_np_bound (all rounds: four grids and the one-CTA tail; round 0 holds 97 % of the nodes)
-    bound_flops = s_last.n_bnb_nodes * FLOP_PER_BNB_NODE
+    n_root = min(int(s_last.n_root_nodes), int(s_last.n_bnb_nodes))
+    bound_flops = n_root * FLOP_PER_BNB_ROOT + (s_last.n_bnb_nodes - n_root) * FLOP_PER_BNB_NODE
     bound_ms = float(medk[3])
     ach_b = bound_flops / (bound_ms * 1e-3) / 1e12 if bound_ms > 0 else 0.0
     roofline = {"kernel": "k_np_bound (S5 branch and bound: 4 grid rounds + tail, round 0 = 97 % of the nodes)", "bound": "alu",
                 "achieved": ach_b, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach_b / fp64_peak if fp64_peak > 0 else None,
                 "traffic": traffic.get("k_np_bound"),
-                "algorithmic_flops_per_cut": bound_flops, "flop_per_node": FLOP_PER_BNB_NODE, "nodes_per_cut": int(s_last.n_bnb_nodes),
+                "algorithmic_flops_per_cut": bound_flops, "flop_per_node": FLOP_PER_BNB_NODE, "flop_per_root_node": FLOP_PER_BNB_ROOT,
+                "nodes_per_cut": int(s_last.n_bnb_nodes), "root_nodes_per_cut": n_root,
                 "ms_per_cut": bound_ms, "peak_source": fp64_src, "share_of_step": bound_ms / step_ms if step_ms > 0 else None}
     # every k_np_solve launch (seeds, three leaf passes, two overflow rounds -- the latter with their two short bound passes)
     newton_flops = s_last.n_newton_iters * FLOP_PER_NEWTON_EVAL + s_last.n_newton * FLOP_PER_NEWTON_FINISH

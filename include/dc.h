@@ -56,12 +56,23 @@ extern "C" {
 #define DC_ERR_UNSUPPORTED (-3) /* device is not sm_100, or input violates a documented precondition */
 #define DC_ERR_CUDA (-4)        /* a CUDA runtime call failed */
 #define DC_ERR_STATE (-5)       /* call order: dc_classify before dc_set_cut_surface, ... */
+#define DC_ERR_RESULT (-6)      /* a device-side consistency check failed (DC_STATUS_FILL_CONFLICT,
+                                   DC_STATUS_SEEDLESS_OVERFLOW): labels were written but are not to be trusted */
 
 /* dc_stats.status bits (device-side conditions) */
 #define DC_STATUS_PAIR_OVERFLOW 1   /* candidate pair list exceeded max_pairs: results invalid */
 #define DC_STATUS_QUEUE_OVERFLOW 2  /* narrow-phase work queue spill area exhausted: results invalid */
 #define DC_STATUS_FILL_CONFLICT 4   /* a flood-fill component has seeds of both signs */
-#define DC_STATUS_SEEDLESS_OVERFLOW 8 /* more seedless components than DC_MAX_SEEDLESS */
+#define DC_STATUS_SEEDLESS_OVERFLOW 8 /* more seedless components than the library resolves (1024): dc_get_stats
+                                         returns DC_ERR_RESULT */
+#define DC_STATUS_BAND_OVERFLOW 16  /* more elements with candidate pairs than the workspace holds (max_pairs / 8,
+                                       at least 65 536): results invalid; dc_stats.band_needed says how many there
+                                       were -- size max_pairs >= 8 * band_needed */
+#define DC_STATUS_SURFACE_SMALL 32  /* the whole cutting surface is smaller than an element (longest edge of its box <
+                                       max element box diagonal / sqrt 3): a surface component may lie strictly inside
+                                       one element, where the distance to the element's BOUNDARY patches is not the
+                                       distance to the element (reading A7); dc_get_stats returns DC_ERR_UNSUPPORTED.
+                                       Labels and distances are still those of the boundary-patch definition. */
 
 /* dc_params.flags */
 #define DC_FLAG_RECOMPUTE_BOXES 1   /* redo step S2 (element boxes from raw nodes) inside dc_classify
@@ -95,6 +106,10 @@ typedef struct {
     long long n_fill_conflicts;
     long long pairs_needed;      /* pair slots S4 wanted (> max_pairs on overflow) */
     long long queue_peak;        /* max narrow-phase queue depth seen (items) */
+    long long n_root_nodes;      /* (pair, patch) items of branch-and-bound round 0 (whole patch pairs) */
+    long long band_needed;       /* elements with candidate pairs (> the band capacity on DC_STATUS_BAND_OVERFLOW) */
+    long long queue_needed;      /* largest narrow-phase queue any round wanted (> the capacity max(2^20, max_pairs) on
+                                    DC_STATUS_QUEUE_OVERFLOW: size max_pairs >= queue_needed) */
     double l_ref, tau_cut, d_band;
     float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
                                     4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface,
@@ -166,7 +181,10 @@ int dc_get_adjacency(dc_ctx *ctx, int *out_dev, void *stream);
  * Synchronises.  Returns the number of pairs (or a negative error).  For tests. */
 long long dc_get_pairs(dc_ctx *ctx, int *elem_host, int *face_host, long long cap);
 
-/* Synchronises the stream of the last call and fills *host_out. */
+/* Synchronises the stream of the last call and fills *host_out (also when it returns an error).  Returns
+ * DC_ERR_WORKSPACE on DC_STATUS_PAIR/QUEUE/BAND_OVERFLOW (pairs_needed / band_needed say what was wanted),
+ * DC_ERR_RESULT on DC_STATUS_FILL_CONFLICT / DC_STATUS_SEEDLESS_OVERFLOW, DC_ERR_UNSUPPORTED on
+ * DC_STATUS_SURFACE_SMALL, DC_OK otherwise. */
 int dc_get_stats(dc_ctx *ctx, dc_stats *host_out);
 
 void dc_destroy(dc_ctx *ctx);
@@ -185,7 +203,7 @@ const char *dc_error_string(int code);
 int dc_union_labels(long long n_elem, const signed char *a_dev, const signed char *b_dev,
                     signed char *out_dev, void *stream);
 
-/* Algorithm 3.1 steps 6-7 (PAPER.md L126-L131) for one grid.
+/* Algorithm 3.1 steps 6-7 (PAPER.md L121-L125) for one grid.
  *   iblank_prev_dev [n_elem] int8 dev  in   I_{t-}: the blanking used for the previous time step (step 1)
  *   labels_t_dev, labels_tplus_dev      in   dc_classify labels of the cuts at t (step 5) and t + dt (step 3)
  *   iblank_out_dev  [n_elem] int8 dev  out  the blanking of this step: wall  -> hole at t OR at t + dt  (6.1),

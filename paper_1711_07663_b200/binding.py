@@ -14,8 +14,9 @@ from typing import Optional
 from ._build import LIB
 
 DC_HOLE, DC_NORMAL, DC_CUT = 0, 1, 2
-DC_OK, DC_ERR_ARG, DC_ERR_WORKSPACE, DC_ERR_UNSUPPORTED, DC_ERR_CUDA, DC_ERR_STATE = 0, -1, -2, -3, -4, -5
+DC_OK, DC_ERR_ARG, DC_ERR_WORKSPACE, DC_ERR_UNSUPPORTED, DC_ERR_CUDA, DC_ERR_STATE, DC_ERR_RESULT = 0, -1, -2, -3, -4, -5, -6
 DC_STATUS_PAIR_OVERFLOW, DC_STATUS_QUEUE_OVERFLOW, DC_STATUS_FILL_CONFLICT, DC_STATUS_SEEDLESS_OVERFLOW = 1, 2, 4, 8
+DC_STATUS_BAND_OVERFLOW, DC_STATUS_SURFACE_SMALL = 16, 32
 DC_FLAG_RECOMPUTE_BOXES = 1
 DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
 
@@ -38,6 +39,7 @@ class dc_stats(C.Structure):
                 ("n_normal", C.c_longlong), ("n_ambiguous", C.c_longlong), ("n_sign_ambiguous", C.c_longlong),
                 ("n_seedless_components", C.c_longlong), ("n_fill_conflicts", C.c_longlong),
                 ("pairs_needed", C.c_longlong), ("queue_peak", C.c_longlong),
+                ("n_root_nodes", C.c_longlong), ("band_needed", C.c_longlong), ("queue_needed", C.c_longlong),
                 ("l_ref", C.c_double), ("tau_cut", C.c_double), ("d_band", C.c_double),
                 ("ms_stage", C.c_float * 8), ("ms_kernel", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int)]
 
@@ -119,7 +121,7 @@ def dc_classify_host(ctx, params: Optional[dc_params], n_face, faces_host_ptr, l
 def dc_get_stats(ctx, allow_status: bool = False) -> dc_stats:
     st = dc_stats()
     rc = _lib.dc_get_stats(ctx, C.byref(st))
-    if rc != DC_OK and not (allow_status and rc == DC_ERR_WORKSPACE):
+    if rc != DC_OK and not (allow_status and rc in (DC_ERR_WORKSPACE, DC_ERR_RESULT, DC_ERR_UNSUPPORTED)):
         raise DcError(rc, "dc_get_stats (status=%d, pairs_needed=%d)" % (st.status, st.pairs_needed))
     return st
 

@@ -1,5 +1,5 @@
 // dc_blank.cuh -- the blanking logic that consumes direct cuts: union of holes and AB faces,
-// Algorithm 3.1 steps 6-7 (L126-L131).  Pure label arithmetic: one thread per element, streaming (HBM bound:
+// Algorithm 3.1 steps 6-7 (L121-L125).  Pure label arithmetic: one thread per element, streaming (HBM bound:
 // 3-4 bytes per element in, 1 out), lists by warp-aggregated atomic append.
 #pragma once
 

@@ -24,8 +24,8 @@ namespace dcg {
 
 // min / max of two finite doubles as one compare and a select (fmin / fmax expand to a NaN-aware sequence about
 // twice as long; every value compared on the hot path is finite)
-__host__ __device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
-__host__ __device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double dmin2(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax2(double a, double b) { return a > b ? a : b; }
 
 // ---------------------------------------------------------------------------------------------
 // 1-D quadratic through nodes (-1, 0, +1): a0 + a1 t + a2 t^2
@@ -56,14 +56,10 @@ __device__ __forceinline__ unsigned long long enc_ord(double x)
     unsigned long long b = (unsigned long long)__double_as_longlong(x);
     return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
 }
-__device__ __host__ __forceinline__ double dec_ord(unsigned long long e)
+__device__ __forceinline__ double dec_ord(unsigned long long e)
 {
-    unsigned long long b = (e & 0x8000000000000000ull) ? (e & 0x7fffffffffffffffull) : ~e;
-#ifdef __CUDA_ARCH__
+    const unsigned long long b = (e & 0x8000000000000000ull) ? (e & 0x7fffffffffffffffull) : ~e;
     return __longlong_as_double((long long)b);
-#else
-    double d; memcpy(&d, &b, 8); return d;
-#endif
 }
 
 // 8-bit code of the sign cosine: bit 7 = negative, bits 0-6 = round(|cos| * 127)

@@ -56,6 +56,7 @@ struct DcScalars {
     int n_seedless;
     int uf_tile;                    // next tile of k_uf_tiles (tiles are taken in launch order)
     int n_lroots;                   // tile-local roots listed by k_uf_tiles
+    int surface_small;              // DC_STATUS_SURFACE_SMALL (kept apart from status: k_setup_classify resets that later)
     int status;
     int qn[DC_NQN];                 // items of round r (children queue, ping-pong buffers)
     int nn[DC_NQN];                 // leaves of round r (Newton queue)
@@ -368,9 +369,18 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
     S->tol_d = 1e-13 * lref;
     S->d_band = P.d_band > 0.0 ? P.d_band : sqrt(__longlong_as_double((long long)S->grid_max_diag2));
     S->reach = S->d_band + 2.0 * S->tau + S->t_tie;
+    {
+        // precondition of reading A7 (SURVEY 8(a) note ii), checked where it is cheap: the WHOLE surface against the
+        // largest element (a cube of diagonal D has edge D / sqrt 3)
+        double ext = 0.0;
+        for (int c = 0; c < 3; ++c) ext = dmax2(ext, S->smax[c] - S->smin[c]);
+        const double dg = sqrt(__longlong_as_double((long long)S->grid_max_diag2));
+        S->surface_small = ext < dg * 0.5773502691896258 ? 1 : 0;
+    }
     S->theta = P.theta_leaf > 0.0 ? P.theta_leaf : 0.25;
     S->max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
-    S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->uf_tile = 0; S->n_lroots = 0; S->status = 0; S->n_pairs = 0ull;
+    S->n_active = 0; S->n_band = 0; S->n_seedless = 0; S->uf_tile = 0; S->n_lroots = 0; S->n_pairs = 0ull;
+    S->status = S->surface_small ? DC_STATUS_SURFACE_SMALL : 0;
     for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; S->nh[i] = 0; }
     S->nh[DC_NQN] = 0;
     S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
@@ -561,7 +571,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                         NItem it; it.p = (unsigned)(b + (long long)(skey & 0xfffffull)); it.ak = (unsigned)slot | (7u << 29); it.w2 = 0; it.w3 = 1u << 24;
                         seed_q[slot] = it;
                         bslot = slot;
-                    } else { atomicOr(&S->status, DC_STATUS_PAIR_OVERFLOW); b = -1; }
+                    } else { atomicOr(&S->status, DC_STATUS_BAND_OVERFLOW); b = -1; }
                 }
                 base = b;
             }
@@ -1026,7 +1036,8 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
 extern "C" size_t dc_workspace_bytes(long long n_nodes, long long n_elem, long long max_faces, long long max_pairs)
 {
     if (n_nodes <= 0 || n_elem <= 0 || max_faces <= 0 || max_pairs <= 0) return 0;
-    if (n_elem > 300000000LL || n_nodes > 2000000000LL) return 0;
+    // (element, node, face and pair indices are 32-bit on the device; a work item keeps the band index in 29 bits)
+    if (n_elem > 300000000LL || n_nodes > 2000000000LL || max_faces >= (1LL << 31) || max_pairs >= (1LL << 31)) return 0;
     return ws_layout(n_nodes, n_elem, max_faces, max_pairs).total;
 }
 
@@ -1043,24 +1054,13 @@ static int run_elem_boxes(dc_ctx *c, cudaStream_t st)
     return DC_OK;
 }
 
-extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const double *xyz_dev,
-                              long long n_elem, const int *conn27_dev, const int *adj6_dev,
-                              void *workspace_dev, size_t workspace_bytes,
-                              long long max_faces, long long max_pairs, void *stream)
+extern "C" void dc_destroy(dc_ctx *c);
+
+static int create_grid_body(dc_ctx *c, int num_sms, int device, long long n_nodes, const double *xyz_dev,
+                            long long n_elem, const int *conn27_dev, const int *adj6_dev,
+                            void *workspace_dev, size_t workspace_bytes, long long max_faces, long long max_pairs, cudaStream_t st)
 {
-    if (!out || !xyz_dev || !conn27_dev || !workspace_dev) return DC_ERR_ARG;
-    const size_t need = dc_workspace_bytes(n_nodes, n_elem, max_faces, max_pairs);
-    if (need == 0) return DC_ERR_ARG;
-    if (workspace_bytes < need) return DC_ERR_WORKSPACE;
-    if (((uintptr_t)workspace_dev & 255) != 0) return DC_ERR_ARG;
-    CK(cudaSetDevice(device));
-    cudaDeviceProp prop;
-    CK(cudaGetDeviceProperties(&prop, device));
-    if (prop.major != 10) return DC_ERR_UNSUPPORTED;   // sm_100a only: no fallback path exists
-    dc_ctx *c = new (std::nothrow) dc_ctx();
-    if (!c) return DC_ERR_ARG;
-    memset(c, 0, sizeof *c);
-    c->device = device; c->num_sms = prop.multiProcessorCount;
+    c->device = device; c->num_sms = num_sms;
     c->n_nodes = n_nodes; c->n_elem = n_elem; c->max_faces = max_faces; c->max_pairs = max_pairs;
     c->xyz = xyz_dev; c->conn = conn27_dev;
     c->ws = (unsigned char *)workspace_dev; c->ws_bytes = workspace_bytes;
@@ -1099,7 +1099,6 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     c->h_faces_dev = (double *)(c->ws + L.off_hfaces);
     c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
     c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
-    cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     for (int i = 0; i < 12; ++i) CK(cudaEventCreate(&c->ev[i]));
     for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->evk[i]));
@@ -1107,7 +1106,7 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
     CK(cudaMemsetAsync(c->tile_flag, 0, (size_t)(n_elem / UF_TILE + 2) * 4, st));
     int rc = run_elem_boxes(c, st);
-    if (rc != DC_OK) { delete c; return rc; }
+    if (rc != DC_OK) return rc;
     if (adj6_dev) c->adj = adj6_dev;
     else {
         int *first = (int *)(c->ws + L.off_pair_face);
@@ -1118,6 +1117,30 @@ extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const
         CK(cudaGetLastError());
         c->adj = c->adj_own;
     }
+    return DC_OK;
+}
+
+
+extern "C" int dc_create_grid(dc_ctx **out, int device, long long n_nodes, const double *xyz_dev,
+                              long long n_elem, const int *conn27_dev, const int *adj6_dev,
+                              void *workspace_dev, size_t workspace_bytes,
+                              long long max_faces, long long max_pairs, void *stream)
+{
+    if (!out || !xyz_dev || !conn27_dev || !workspace_dev) return DC_ERR_ARG;
+    const size_t need = dc_workspace_bytes(n_nodes, n_elem, max_faces, max_pairs);
+    if (need == 0) return DC_ERR_ARG;
+    if (workspace_bytes < need) return DC_ERR_WORKSPACE;
+    if (((uintptr_t)workspace_dev & 255) != 0) return DC_ERR_ARG;
+    CK(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10 || prop.minor != 0) return DC_ERR_UNSUPPORTED;   // sm_100a only (the one cubin built): no fallback path exists
+    dc_ctx *c = new (std::nothrow) dc_ctx();
+    if (!c) return DC_ERR_ARG;
+    memset(c, 0, sizeof *c);
+    const int rc = create_grid_body(c, prop.multiProcessorCount, device, n_nodes, xyz_dev, n_elem, conn27_dev, adj6_dev,
+                                    workspace_dev, workspace_bytes, max_faces, max_pairs, (cudaStream_t)stream);
+    if (rc != DC_OK) { dc_destroy(c); return rc; }     // (events, pinned buffer and the context itself: one cleanup path)
     *out = c;
     return DC_OK;
 }
@@ -1283,21 +1306,26 @@ extern "C" long long dc_get_pairs(dc_ctx *c, int *elem_host, int *face_host, lon
     CK(cudaStreamSynchronize(c->last_stream));
     CK(cudaMemcpy(c->S_host, c->S, sizeof(DcScalars), cudaMemcpyDeviceToHost));
     const int na = c->S_host->n_band < (int)c->max_band ? c->S_host->n_band : (int)c->max_band;
-    int *ae = new int[na > 0 ? na : 1]; long long *as = new long long[na > 0 ? na : 1]; int *ac = new int[na > 0 ? na : 1];
-    int *perm = new int[c->n_face];
-    cudaMemcpy(ae, c->band_elem, (size_t)na * 4, cudaMemcpyDeviceToHost);
-    cudaMemcpy(as, c->band_start, (size_t)na * 8, cudaMemcpyDeviceToHost);
-    cudaMemcpy(ac, c->band_cnt, (size_t)na * 4, cudaMemcpyDeviceToHost);
-    cudaMemcpy(perm, c->fperm, (size_t)c->n_face * 4, cudaMemcpyDeviceToHost);
     long long np = (long long)c->S_host->n_pairs; if (np > c->max_pairs) np = c->max_pairs;
-    int *pf = new int[np > 0 ? np : 1];
-    cudaMemcpy(pf, c->pair_face, (size_t)np * 4, cudaMemcpyDeviceToHost);
-    long long n = 0;
-    for (int a = 0; a < na; ++a)
-        for (int i = 0; i < ac[a]; ++i) {
-            if (n < cap) { elem_host[n] = ae[a]; face_host[n] = perm[pf[as[a] + i]]; }
-            ++n;
-        }
+    int *ae = new (std::nothrow) int[na > 0 ? na : 1]; long long *as = new (std::nothrow) long long[na > 0 ? na : 1];
+    int *ac = new (std::nothrow) int[na > 0 ? na : 1]; int *perm = new (std::nothrow) int[c->n_face > 0 ? c->n_face : 1];
+    int *pf = new (std::nothrow) int[np > 0 ? np : 1];
+    long long n = DC_ERR_ARG;
+    if (ae && as && ac && perm && pf) {
+        n = DC_ERR_CUDA;
+        if (cudaMemcpy(ae, c->band_elem, (size_t)na * 4, cudaMemcpyDeviceToHost) == cudaSuccess &&
+            cudaMemcpy(as, c->band_start, (size_t)na * 8, cudaMemcpyDeviceToHost) == cudaSuccess &&
+            cudaMemcpy(ac, c->band_cnt, (size_t)na * 4, cudaMemcpyDeviceToHost) == cudaSuccess &&
+            cudaMemcpy(perm, c->fperm, (size_t)c->n_face * 4, cudaMemcpyDeviceToHost) == cudaSuccess &&
+            cudaMemcpy(pf, c->pair_face, (size_t)np * 4, cudaMemcpyDeviceToHost) == cudaSuccess) {
+            n = 0;
+            for (int a = 0; a < na; ++a)
+                for (int i = 0; i < ac[a]; ++i) {
+                    if (n < cap && as[a] + i < np) { elem_host[n] = ae[a]; face_host[n] = perm[pf[as[a] + i]]; }
+                    ++n;
+                }
+        } else fprintf(stderr, "libdc: dc_get_pairs: a device-to-host copy failed: %s\n", cudaGetErrorString(cudaGetLastError()));
+    }
     delete[] ae; delete[] as; delete[] ac; delete[] perm; delete[] pf;
     return n;
 }
@@ -1321,6 +1349,8 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
     o->n_ambiguous = (long long)S.c_ambiguous; o->n_sign_ambiguous = (long long)S.c_sign_ambiguous;
     o->n_seedless_components = S.n_seedless; o->n_fill_conflicts = (long long)S.c_fill_conflicts;
     o->queue_peak = (long long)S.c_queue_peak;
+    o->n_root_nodes = S.qn[0]; o->band_needed = S.n_band;
+    for (int i = 0; i < DC_NQN; ++i) { if (S.qn[i] > o->queue_needed) o->queue_needed = S.qn[i]; if (S.nn[i] > o->queue_needed) o->queue_needed = S.nn[i]; }
     o->l_ref = S.l_ref; o->tau_cut = S.tau; o->d_band = S.d_band;
     o->status = S.status;
     o->n_launches = (c->have_surface ? c->launches_surface : 0) + (c->have_cut ? c->launches_classify : 0);
@@ -1348,7 +1378,9 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
         if (cudaEventElapsedTime(&ms, c->ev[8], c->ev[9]) == cudaSuccess) { o->ms_stage[0] = ms; o->ms_stage[6] = ms; }
     }
     (void)cudaGetLastError();
-    if (S.status & (DC_STATUS_PAIR_OVERFLOW | DC_STATUS_QUEUE_OVERFLOW)) return DC_ERR_WORKSPACE;
+    if (S.status & (DC_STATUS_PAIR_OVERFLOW | DC_STATUS_QUEUE_OVERFLOW | DC_STATUS_BAND_OVERFLOW)) return DC_ERR_WORKSPACE;
+    if (S.status & (DC_STATUS_FILL_CONFLICT | DC_STATUS_SEEDLESS_OVERFLOW)) return DC_ERR_RESULT;
+    if (S.status & DC_STATUS_SURFACE_SMALL) return DC_ERR_UNSUPPORTED;
     return DC_OK;
 }
 
@@ -1369,9 +1401,10 @@ extern "C" const char *dc_error_string(int code)
     case DC_OK: return "ok";
     case DC_ERR_ARG: return "bad argument";
     case DC_ERR_WORKSPACE: return "workspace too small or device-side list overflow";
-    case DC_ERR_UNSUPPORTED: return "unsupported device or input (libdc needs an sm_100 GPU)";
+    case DC_ERR_UNSUPPORTED: return "unsupported device (libdc needs an sm_100 GPU) or input (cutting surface smaller than an element)";
     case DC_ERR_CUDA: return "CUDA runtime error";
     case DC_ERR_STATE: return "call order error";
+    case DC_ERR_RESULT: return "device-side consistency check failed (fill conflict or too many seedless components): results not to be trusted";
     default: return "unknown error";
     }
 }

@@ -14,19 +14,10 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
-#include <string.h>
 
 namespace dcn {
 
-#ifdef __CUDA_ARCH__
-#define __longlong_as_double_hd(x) __longlong_as_double(x)
-#else
-static inline double __longlong_as_double_hd(long long x) { double d; memcpy(&d, &x, 8); return d; }
-#endif
-
-#ifndef DCN_HD
-#define DCN_HD __host__ __device__ __forceinline__
-#endif
+#define DCN_HD __device__ __forceinline__      /* device only: there is no host build of the solver */
 
 // (compare-and-select min / max of finite doubles: see dc_geom.cuh)
 DCN_HD double dmin2(double a, double b) { return a < b ? a : b; }
@@ -36,15 +27,11 @@ DCN_HD double dmax2(double a, double b) { return a > b ? a : b; }
 // the compiler emits for 1.0 / x carries a range check and a call; the pivots it is used on are >= floor > 0)
 DCN_HD double rcp_fast(double x)
 {
-#ifdef __CUDA_ARCH__
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     y = fma(fma(-x, y, 1.0), y, y);
     y = fma(fma(-x, y, 1.0), y, y);
     return y;
-#else
-    return 1.0 / x;
-#endif
 }
 
 #ifndef NW_MAXIT
@@ -186,7 +173,7 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
             }
             const double ahit = pd != 0.0 ? rn / pd : INFINITY;
             const bool stretch = indefinite && ahit > 1.0 && ahit < INFINITY;
-            const double q = __longlong_as_double_hd((long long)(1023 - 2 * (s.ls > 0 ? s.ls - 1 : 0)) << 52);   // 4^-(ls-1)
+            const double q = __longlong_as_double((long long)(1023 - 2 * (s.ls > 0 ? s.ls - 1 : 0)) << 52);   // 4^-(ls-1)
             if (s.ls == 0) alpha = stretch ? ahit : 1.0;
             // a rejected trial is followed by UNCLAMPED ones: up to the first bound (a clamped step is not a
             // descent step when the clamped variable is coupled to the others), then quarters of that
@@ -235,11 +222,7 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
         const double den2 = rr * nn;
         R.dist = sqrt(rr_out);
         // (the cosine only decides a sign and a 7-bit magnitude: reciprocal square root instead of sqrt and divide)
-#ifdef __CUDA_ARCH__
         R.cosv = den2 > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) * rsqrt(den2) : 0.0;
-#else
-        R.cosv = den2 > 0.0 ? (r[0] * nx + r[1] * ny + r[2] * nz) / sqrt(den2) : 0.0;
-#endif
         R.converged = converged;
     }
     return finished;

@@ -204,13 +204,42 @@ def test_surface_outside_and_enclosing_the_grid(B):
     assert np.abs(s - ref.sdist).max() <= 1e-14 and st.n_seedless_components == 1
 
 
-def test_single_element_grid(B):
-    w = make_config(0, N=1, n=2)           # one hex [-1,1]^3 containing the whole sphere
-    # documented precondition (no surface component inside one element) is violated on purpose only
-    # for the distance: the boundary-patch distance is still what both sides compute.
+def test_single_element_grid_is_reported_unsupported(B):
+    """One hex [-1,1]^3 containing the whole sphere: the documented precondition (no surface component inside one
+    element, reading A7 / SURVEY.md 8(a) note ii) is violated; dc_get_stats says DC_ERR_UNSUPPORTED
+    (DC_STATUS_SURFACE_SMALL), and the labels / distances written are still those of the boundary-patch definition,
+    which is what the oracle computes too."""
+    w = make_config(0, N=1, n=2)
     ref = O.classify(w.xyz, w.conn27, w.faces)
-    l, s, st = gpu_cut(B, w)
+    dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face)
+    dcut.set_cut_surface(w.faces)
+    labels, sdist = dcut.classify()
+    with pytest.raises(B.DcError) as ei:
+        dcut.stats()
+    assert ei.value.code == B.DC_ERR_UNSUPPORTED
+    st = dcut.stats(allow_status=True)
+    assert st.status == B.DC_STATUS_SURFACE_SMALL
+    l, s = labels.cpu().numpy(), sdist.cpu().numpy()
+    dcut.close()
     assert np.array_equal(l, ref.labels) and np.abs(s - ref.sdist).max() <= TOL_REL * st.l_ref
+
+
+def test_many_seedless_components(B):
+    """A grid of 216 hexes that are not connected to one another at all (adjacency all -1) and far from the surface:
+    216 seedless components, each resolved by its own exhaustive nearest-face query (the library used to stop at 32)."""
+    w = make_config(0, N=6, n=2)
+    adj = np.full_like(w.adj6, -1)
+    faces = w.faces * 0.25 + np.array([3.0, 0.0, 0.0])          # a small sphere outside the grid
+    ref = O.classify(w.xyz, w.conn27, faces)
+    dcut = B.DirectCut(w.xyz, w.conn27, adj, max_faces=len(faces))
+    dcut.set_cut_surface(faces)
+    labels, sdist = dcut.classify()
+    st = dcut.stats(allow_status=True)
+    l, s = labels.cpu().numpy(), sdist.cpu().numpy()
+    dcut.close()
+    assert st.n_pairs == 0 and st.n_seedless_components == w.n_elem
+    assert (st.status & ~B.DC_STATUS_SURFACE_SMALL) == 0
+    assert (l == NORMAL).all() and np.array_equal(l, ref.labels) and np.abs(s - ref.sdist).max() <= 1e-14
 
 
 # ------------------------------------------------------------------------------ error behaviour (include/dc.h)
@@ -231,9 +260,42 @@ def test_error_codes(B):
     st = dcut.stats(allow_status=True)
     assert st.status & B.DC_STATUS_PAIR_OVERFLOW and st.pairs_needed > 64
     dcut.close()
+    assert B.dc_workspace_bytes(10, 10, 1 << 31, 100) == 0 and B.dc_workspace_bytes(10, 10, 100, 1 << 31) == 0
     # the reported size is sufficient
     l, s, st2 = gpu_cut(B, w, max_pairs=int(st.pairs_needed))
     assert st2.status == 0 and st2.n_pairs == st.pairs_needed
+
+
+def test_band_overflow_is_reported_with_the_size_needed(B):
+    """Few, large faces against a fine grid: many band elements with two or three pairs each, so the band arrays
+    (capacity max_pairs / 8, at least 65 536) fill before the pair list does: DC_STATUS_BAND_OVERFLOW, and
+    dc_stats.band_needed says what to ask for."""
+    w = make_config(1, N=112, n=3)           # 1.4 M elements vs 54 faces
+    dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face, max_pairs=400000)
+    dcut.set_cut_surface(w.faces)
+    dcut.classify()
+    with pytest.raises(B.DcError) as ei:
+        dcut.stats()
+    assert ei.value.code == B.DC_ERR_WORKSPACE
+    st = dcut.stats(allow_status=True)
+    dcut.close()
+    assert st.status & B.DC_STATUS_BAND_OVERFLOW and not (st.status & B.DC_STATUS_PAIR_OVERFLOW)
+    assert st.band_needed > 65536 and st.pairs_needed <= 400000
+    # following the sizes reported leads to a valid cut (this workload's whole faces make up to 6 root items per pair:
+    # the queues, sized by max_pairs too, are the next thing to fill, and say so the same way; a queue that overflowed
+    # hides what the later rounds would have wanted, hence the loop)
+    need = 8 * int(st.band_needed)
+    for attempt in range(4):
+        dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face, max_pairs=need)
+        dcut.set_cut_surface(w.faces); dcut.classify()
+        st1 = dcut.stats(allow_status=True)
+        dcut.close()
+        assert not (st1.status & (B.DC_STATUS_BAND_OVERFLOW | B.DC_STATUS_PAIR_OVERFLOW))
+        if st1.status == 0:
+            break
+        assert st1.status & B.DC_STATUS_QUEUE_OVERFLOW and st1.queue_needed > max(need, 1 << 20)
+        need = int(st1.queue_needed)
+    assert st1.status == 0 and st1.band_needed == st.band_needed and st1.n_cut > 1000
 
 
 # ------------------------------------------------------------------------------ coarse grid, fine surface
