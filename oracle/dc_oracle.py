@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dc_oracle.c")
+_SRC_PAPER = os.path.join(_HERE, "paper_oracle.c")     # the paper's approximate mode (oracle/paper_oracle.py)
 _LIB = os.path.join(_HERE, "liboracle_dc.so")
 
 HOLE, NORMAL, CUT = 0, 1, 2
@@ -41,10 +42,10 @@ class OrcStats(C.Structure):
 def build(force: bool = False) -> str:
     """gcc -O2 (no fast-math) -> oracle/liboracle_dc.so; rebuilt when the source is newer."""
     if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_PAPER))):
         return _LIB
     tmp = _LIB + ".tmp%d" % os.getpid()
-    subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+    subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", tmp, _SRC, _SRC_PAPER, "-lm"])
     os.replace(tmp, _LIB)
     return _LIB
 

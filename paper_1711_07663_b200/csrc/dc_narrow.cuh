@@ -587,7 +587,10 @@ __global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, con
         const double dmin = u2d(dmin_arr[b]);
         if (u2d(best[b]) <= tau_exit) { labels[e] = DC_CUT; sdist[e] = 0.0; }
         else if (dmin <= tau) { labels[e] = DC_CUT; sdist[e] = 0.0; if (dmin >= tau - amb) ++n_amb; }
-        else if (dmin < INFINITY) {
+        else if (dmin <= d_band) {
+            // (an element whose distance exceeds the band keeps label -1 and takes its sign from the flood fill: beyond
+            // best[b] = reach the branch and bound has pruned freely, so the faces it did solve need not include the
+            // nearest one, and on a body thinner than the band a far-side face could win the sign)
             if (dmin <= tau + amb) ++n_amb;
             int bestmag = -1, neg = 0, npos = 0, nneg = 0;
             const long long p0 = band_start[b];
