@@ -23,6 +23,7 @@ nodes + connectivity + adjacency, surface faces) are resident in HBM before the 
   cpu_baseline: the oracle (oracle/dc_oracle.c, as it stands) on this box's host cores on a bounded
             uniform sample of the same workload's elements, each against ALL faces; `value` counts the SAME
             candidate pairs as the GPU line (those of the sampled elements), per oracle second.
+  paper_mode: the paper's own approximate cut (DC_FLAG_PAPER_MODE) on the same context: ms, labels differing from the exact mode.
   per_config: the other BASELINE.json configs (0, 1, 3 incl. the sum over its 32 steps, 4), a few seconds each,
             every one with its own clock record over a timed region of at least 200 ms.
 
@@ -330,6 +331,31 @@ def time_cuts(dcut, face_sets, params, n_cuts: int, stream, torch):
     return ev0.elapsed_time(ev1)
 
 
+def measure_paper_mode(dcut, faces, B, stream, torch, np, n_cuts: int = 10):
+    """the paper's own approximate cut (DC_FLAG_PAPER_MODE: A.1, A.3, A.4, 16 -> 4 faces, linear
+    triangles, L215) on the same context: ms per full cut, and how its labels and distances differ from the exact mode's
+    (which is element-by-element equal to the oracle in the -m gpu tests)."""
+    p_exact = B.dc_params(); p_exact.flags = B.DC_FLAG_RECOMPUTE_BOXES
+    p_paper = B.dc_params(); p_paper.flags = B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_PAPER_MODE
+    dcut.set_cut_surface(faces); dcut.classify(p_exact)
+    lab0 = dcut.labels.clone(); sd0 = dcut.sdist.clone()
+    st0 = dcut.stats()
+    for _ in range(2):
+        dcut.set_cut_surface(faces); dcut.classify(p_paper)
+    ms = time_cuts(dcut, [faces], p_paper, n_cuts, stream, torch) / n_cuts
+    st = dcut.stats()
+    lab1, sd1 = dcut.labels, dcut.sdist
+    diff = lab1 != lab0
+    out = {"ms_per_full_cut": ms, "ms_S5_S6": float(st.ms_stage[3]), "ms_S5_S6_exact_mode": float(st0.ms_stage[3]),
+           "labels_differing_from_exact": int(diff.sum().item()), "band_elements": int(st.band_needed),
+           "cut_in_exact_only": int(((lab0 == 2) & (lab1 != 2)).sum().item()), "cut_in_paper_only": int(((lab1 == 2) & (lab0 != 2)).sum().item()),
+           "hole_normal_swapped": int((diff & (lab0 != 2) & (lab1 != 2)).sum().item()),
+           "max_abs_dsdist_over_lref": float((sd1 - sd0).abs().max().item() / st.l_ref),
+           "census_hole_cut_normal": [int(st.n_hole), int(st.n_cut), int(st.n_normal)]}
+    dcut.set_cut_surface(faces); dcut.classify(p_exact)
+    return out
+
+
 def measure_other_config(cfg: int, B, local_rank: int, torch, np, min_ms: float = 200.0):
     """One of the other BASELINE.json configs: full cut and re-cut, each over a timed region of at least `min_ms` with its
     own clock record; config 3: every one of its 32 steps and their sum (re-cut path: the grid is fixed)."""
@@ -372,6 +398,8 @@ def measure_other_config(cfg: int, B, local_rank: int, torch, np, min_ms: float 
                          "ms_sum_32_steps_recut": float(per_step.sum()),
                          "ms_step1_full_cut": float(first_full),
                          "ms_sum_32_steps_step1_full": float(per_step[1:].sum() + first_full)}
+    if cfg != 3:
+        out["paper_mode"] = measure_paper_mode(dcut, face_sets[0], B, stream, torch, np)
     dcut.close()
     del dcut, face_sets
     torch.cuda.empty_cache()
@@ -597,6 +625,8 @@ def main():
                                 "gpu_box_tests_per_s": float(s_last.n_box_tests) / (ms_per_step * 1e-3),
                                 "parity_on_sample": {"label_mismatches": mism, "ambiguous": int(amb.sum()),
                                                      "max_abs_dsdist_over_lref": err / ref.stats["l_ref"]}}
+    if rank == 0 and world == 1 and cfg != 3 and not args.no_per_config:
+        line["paper_mode"] = measure_paper_mode(dcut, face_sets[0], B, stream, torch, np)
     dcut.close()
     del dcut
     torch.cuda.empty_cache()

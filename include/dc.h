@@ -77,6 +77,12 @@ extern "C" {
 /* dc_params.flags */
 #define DC_FLAG_RECOMPUTE_BOXES 1   /* redo step S2 (element boxes from raw nodes) inside dc_classify
                                        instead of using the boxes cached by dc_create_grid */
+#define DC_FLAG_PAPER_MODE 2        /* the paper's own APPROXIMATE cut for the elements with candidate faces, in place of the
+                                       exact narrow phase (S5, S6): Algorithms A.1, A.3, A.4 with N_F^1 = 16
+                                       and N_F^2 = 4 nearest faces kept (L209, L213), the nearest-corner 3-face shortcut (L213),
+                                       linear triangles (Fig. 11) and the normal averaging of L215.  Labels and distances are
+                                       those of that method (its linearisation error included): for comparison with the exact
+                                       mode, not for parity with the exact oracle.  S4 and S7 are unchanged. */
 
 typedef struct dc_ctx dc_ctx;
 

@@ -18,6 +18,7 @@ DC_OK, DC_ERR_ARG, DC_ERR_WORKSPACE, DC_ERR_UNSUPPORTED, DC_ERR_CUDA, DC_ERR_STA
 DC_STATUS_PAIR_OVERFLOW, DC_STATUS_QUEUE_OVERFLOW, DC_STATUS_FILL_CONFLICT, DC_STATUS_SEEDLESS_OVERFLOW = 1, 2, 4, 8
 DC_STATUS_BAND_OVERFLOW, DC_STATUS_SURFACE_SMALL = 16, 32
 DC_FLAG_RECOMPUTE_BOXES = 1
+DC_FLAG_PAPER_MODE = 2
 DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
 
 EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify",

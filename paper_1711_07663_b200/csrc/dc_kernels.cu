@@ -603,6 +603,7 @@ __constant__ int c_face_node[6][9] = {
 };
 
 #include "dc_narrow.cuh"
+#include "dc_paper.cuh"
 
 // ------------------------------------------------------------------------------------------
 // S7: flood fill = connected components of the face-adjacency graph of non-CUT elements
@@ -1192,6 +1193,30 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
                                            c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key,
                                            c->pair_band, c->nq, c->best, c->dmin);
     CK(cudaEventRecord(c->ev[2], st));
+    const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
+    const int rounds = 2 * max_level + 1;
+    const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
+    if (P.flags & DC_FLAG_PAPER_MODE) {
+        // ---- the paper's approximate cut of the band elements (dc_paper.cuh) in place of S5/S6; its work arrays live in the
+        // memory of the exact mode's per-element coefficients (1344 bytes per band element there, 656 here)
+        DcScalars *S = c->S;
+        PmWork W;
+        unsigned char *base = (unsigned char *)c->ecoef;
+        const size_t mb = (size_t)c->max_band;
+        W.sel1 = (int *)base; base += mb * PM_NF1 * 4;
+        W.corner = (int *)base; base += mb * PM_NF1 * 4;
+        W.sel2 = (int *)base; base += mb * PM_NF2 * 4;
+        W.d1 = (double *)base; base += mb * PM_NF1 * 8;
+        W.d2 = (double *)base; base += mb * PM_NF2 * 3 * 8;
+        W.v2 = (double *)base;
+        const int g = c->num_sms * 8;
+        k_pm_rank<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fperm, c->face_nodes, W);
+        k_pm_pass1<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->face_nodes, W);
+        k_pm_select<<<g, 128, 0, st>>>(S, W);
+        k_pm_pass2<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->face_nodes, W);
+        k_pm_decide<<<g, 128, 0, st>>>(S, c->band_elem, c->face_nodes, W, labels_dev, sdist_dev);
+        CK(cudaEventRecord(c->ev[3], st));
+    } else {
     // ---- S5: wavefront narrow phase (dc_narrow.cuh)
     const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
     DcScalars *S = c->S;
@@ -1208,9 +1233,6 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
     // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
     CK(cudaEventRecord(c->evk[0], st));
-    const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
-    const int rounds = 2 * max_level + 1;
-    const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
     k_np_bound<true><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                  c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
     for (int r = 1; r < grid_rounds; ++r)
@@ -1251,6 +1273,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
+    }
     c->epoch = c->epoch == 0x7fffffff ? 1 : c->epoch + 1;
     k_uf_tiles<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(c->S, labels_dev, c->adj, ne, c->parent, c->tile_flag, c->epoch, c->act_elem);
     k_uf_seed<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
@@ -1260,7 +1283,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_fix<<<c->num_sms * 4, 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
-    c->launches_classify = 21 + grid_rounds + (rounds > grid_rounds ? 1 : 0) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
+    c->launches_classify = ((P.flags & DC_FLAG_PAPER_MODE) ? 13 : 21 + grid_rounds + (rounds > grid_rounds ? 1 : 0)) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
 }
