@@ -111,3 +111,49 @@ def test_fullsize_sampled_parity_and_invariants(B, nproc, config):
         ids3 = ids[(mar < 1.5 * h) | (np.arange(ids.size) % 3 == 0)][:600]
         check_sample(w, faces, ids3, labels, sdist, st, nproc, zero_amb=False)
     dcut.close()
+
+
+MAX_AMBIGUOUS_PER_STEP = 2          # stated bound on the oracle's ambiguous elements in a sample of a spin step (measured: 0)
+
+
+def test_config3_every_spin_step_at_full_size(B, nproc):
+    """Config 3 = the config-2 grid re-cut by the surface rotated by s degrees, s = 1..32 (reading A13), on ONE context
+    (cached element boxes: the path the moving-body loop uses): every step against the oracle on 2000
+    elements (half near the rotated surface, chosen from the ANALYTIC shape in the body frame, half at random), labels
+    bit-exact off the ambiguous band, distances within 1e-10 L_ref, plus the invariants that hold at any size."""
+    w = make_config(2)
+    cen = centroids(w)
+    dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face)
+    p = B.dc_params()
+    h = 2.0 / w.N
+    rng = np.random.default_rng(33)
+    cand = rng.choice(w.n_elem, size=300000, replace=False)
+    d_band = None
+    worst, n_amb_total = 0.0, 0
+    for s in range(1, 33):
+        faces = w.spin_faces(s)
+        dcut.set_cut_surface(faces)
+        labels, sdist = dcut.classify(p)
+        st = dcut.stats()
+        labels, sdist = labels.cpu().numpy().copy(), sdist.cpu().numpy().copy()
+        assert st.status == 0 and st.n_fill_conflicts == 0 and st.n_depth_exceeded == 0 and st.n_sign_ambiguous == 0
+        assert st.n_cut + st.n_hole + st.n_normal == w.n_elem
+        Rm = rotation_about_axis(w.meta["spin_axis"], np.deg2rad(float(s)))      # faces = w.faces @ Rm.T
+        mar = w.surf_margin(cen[cand] @ Rm)                                      # centroids in the body frame
+        near = cand[mar < 1.5 * h]
+        ids = np.unique(np.concatenate([rng.choice(near, size=1000, replace=False), rng.choice(w.n_elem, size=1000, replace=False)]))
+        if d_band is None:
+            d_band = O.auto_d_band(w.xyz, w.conn27, faces)
+        assert abs(st.d_band - d_band) <= 1e-14
+        ref = O.classify(w.xyz, w.conn27, faces, elem_ids=ids, nproc=nproc, d_band=d_band)
+        amb = (ref.flags & O.FLAG_AMBIGUOUS) != 0
+        assert amb.sum() <= MAX_AMBIGUOUS_PER_STEP and ref.stats["n_depth_exceeded"] == 0
+        n_amb_total += int(amb.sum())
+        bad = (labels[ids] != ref.labels) & ~amb
+        assert bad.sum() == 0, "step %d: label mismatches at elements %s" % (s, ids[bad][:10])
+        err = np.abs(sdist[ids] - ref.sdist)[~amb].max()
+        assert err <= TOL_REL * ref.stats["l_ref"], "step %d: max |dsdist| %.3e" % (s, err)
+        worst = max(worst, err / ref.stats["l_ref"])
+        assert (ref.labels == CUT).sum() > 50 and (ref.labels == HOLE).sum() > 50
+    dcut.close()
+    print("config 3: 32 steps x ~2000 elements: max |dsdist| / L_ref %.2e, ambiguous elements (oracle) %d" % (worst, n_amb_total))
