@@ -5,7 +5,8 @@
 //   S3 face bins      k_face_hist, k_scan_sums, k_scan_cells, k_cell_occ, k_face_scatter   (uniform bins, rows along x contiguous)
 //   S2 element boxes  k_elem_boxes                                    (HBM-bound stream)
 //   S4 candidates     k_filter (thread/element), k_pairs (16 lanes/active element, one append per element)
-//   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_newton, k_np_roots, k_np_bound, k_np_bound_tail (FP64)
+//   S5 narrow phase   dc_narrow.cuh: k_np_stage, k_np_solve, k_np_roots, k_np_bound, k_np_bound_tail, k_np_compact (FP64)
+//   (DC_FLAG_PAPER_MODE: dc_paper.cuh, the paper's approximate A.1 / A.3 / A.4 in place of S5 and S6)
 //   S6 decide         k_np_decide
 //   S7 flood fill     k_uf_tiles, k_uf_seed, k_uf_resolve, k_uf_assign, k_seedless, k_uf_fix
 //
@@ -799,7 +800,7 @@ __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const dou
                 bool leaf = nb.leaf, splitP = false;
                 if (!leaf) leaf = !choose_split(it, nb.splitP, max_level, splitP);
                 if (leaf || top + 4 > 80) {
-                    // the same lockstep iteration as k_np_newton, run to the end by this thread (an unconverged
+                    // the same iteration as k_np_solve, run to the end by this thread (an unconverged
                     // solve still yields an attained distance; a seedless component only needs the sign)
                     dcn::NwState s; s.x[0] = uc; s.x[1] = vc; s.x[2] = sc; s.x[3] = tc; s.iters = 0; s.ls = 0; s.phase = 1;
                     const double lo[4] = { uc - hP, vc - hP, sc - hQ, tc - hQ }, hi[4] = { uc + hP, vc + hP, sc + hQ, tc + hQ };

@@ -4,20 +4,22 @@
 // atomics), so warps stay full and no kernel carries another's registers:
 //
 //   k_np_stage      thread / (element, patch) : monomial coefficients and Bezier box of a boundary patch -> ecoef, pbox
-//                                         (the first upper bound best[b] and the seed item come from k_pairs)
-//   k_np_newton     persistent warps    : projected Newton (Eq. 3-5 L256-L270 generalised to two patches, clamp
-//                                         L272-L278), one solve per lane in lockstep, lanes refilled from the
-//                                         queue; min into best / dmin / pair_key; the sub-leaves of an unconverged
-//                                         leaf go to an overflow queue
+//                                         (best[b] = reach and the seed item come from k_pairs)
+//   k_np_solve      thread / leaf       : projected Newton (Eq. 3-5 L256-L270 generalised to two patches, clamp
+//                                         L272-L278), both patches' coefficients in registers; a pass hands its
+//                                         stragglers to the next pass through a continuation queue; min into best /
+//                                         dmin / pair_key; the sub-leaves of an unconverged leaf go to an overflow queue
 //   k_np_roots      thread / pair       : (pair, patch) whose boxes are within best + t_tie (A.2, L689-L709)
 //                                         become the items of round 0
-//   k_np_bound      thread / item       : bound_node -> prune / 4 children / leaf (+ the leaf's first step)
+//   k_np_bound      thread / item       : bound_node -> prune / 4 children / leaf (+ the leaf's starting point and
+//                                         lower bound); <ROOT> for round 0
 //   k_np_bound_tail one CTA             : the sparse late rounds, until one comes up empty
+//   k_np_compact    thread / leaf       : drops the leaves whose lower bound the element's best distance has passed
 //   k_np_decide     thread / band elem  : S6 (L215 nearest face and its normal; tie rule L294)
 //
-// Launch order (dc_classify): stage, newton(seeds), roots, bound x 4, bound_tail, newton(leaves),
-// [bound(overflow), newton] x 2, decide.  Every item of bound round r has lP + lQ = r, so 2 max_level + 1
-// rounds always terminate the branch and bound.
+// Launch order (dc_classify): stage, solve(seeds), roots, bound<ROOT>, bound x 3, bound_tail, compact, solve(leaves),
+// solve(continuations) x 2, [bound(overflow), solve] x 2, decide.  Every item of bound round r has lP + lQ = r, so
+// 2 max_level + 1 rounds always terminate the branch and bound.
 #pragma once
 
 #define NPW_THREADS 128
