@@ -45,23 +45,27 @@ def num(s: str) -> float:
 
 def do_full(path: str, cfg: int, tag: str):
     rows = list(csv.reader(open(path)))
-    hdr = rows[0]
+    hdr, units = rows[0], rows[1]
     ix = {n: i for i, n in enumerate(hdr)}
-    cols = [("gpu__time_duration.sum", "us", 1e-3), ("launch__registers_per_thread", "regs", 1.0),
+    # ncu scales each column (us / ms, Mbyte / Gbyte ...): bring times to us and bytes to MB
+    scale_of = {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6, "byte": 1e-6, "Kbyte": 1e-3, "Mbyte": 1.0, "Gbyte": 1e3}
+    cols = [("gpu__time_duration.sum", "us", None), ("launch__registers_per_thread", "regs", 1.0),
             ("sm__warps_active.avg.pct_of_peak_sustained_active", "warps act %", 1.0),
-            ("smsp__issue_active.avg.pct", "issue %", 1.0),
+            ("smsp__issue_active.avg.pct_of_peak_sustained_active", "issue %", 1.0),
             ("sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active", "fp64 pipe %", 1.0),
             ("smsp__thread_inst_executed_per_inst_executed.ratio", "lanes/inst", 1.0),
-            ("dram__bytes_read.sum", "DRAM rd MB", 1e-6), ("dram__bytes_write.sum", "DRAM wr MB", 1e-6),
+            ("dram__bytes_read.sum", "DRAM rd MB", None), ("dram__bytes_write.sum", "DRAM wr MB", None),
             ("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "DRAM %", 1.0),
             ("smsp__sass_thread_inst_executed_op_dfma_pred_on.sum", "dfma", 1.0),
             ("smsp__sass_thread_inst_executed_op_dadd_pred_on.sum", "dadd", 1.0),
             ("smsp__sass_thread_inst_executed_op_dmul_pred_on.sum", "dmul", 1.0)]
-    cols = [c for c in cols if c[0] in ix]
+    cols = [(c[0], c[1], c[2] if c[2] is not None else scale_of.get(units[ix[c[0]]], 1.0)) for c in cols if c[0] in ix]
     out = ["# Round 2: `ncu --set full` of the kernels of one cut, config %d" % cfg, "",
            "Commands (B200, under gpurun; the plain run exited 0 first, same call):", "", "```",
            BENCH_CMD % cfg + " > gpurun_out/plain.log 2>&1 &&",
-           "ncu --set full --clock-control none --import-source on -k regex:'k_' --launch-skip <launches of 3 warm-up cuts> -c <launches of one cut> \\",
+           "ncu --set full --metrics smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,"
+           "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum \\",
+           "    --clock-control none --import-source on -k regex:'k_' --launch-skip 105 -c 35 \\",
            "    -f -o gpurun_out/prof_%s " % tag + BENCH_CMD % cfg,
            "ncu -i gpurun_out/prof_%s.ncu-rep --page raw --csv > raw.csv" % tag,
            "python -m paper_1711_07663_b200.profile_summary full raw.csv %d %s" % (cfg, tag), "```", "",
