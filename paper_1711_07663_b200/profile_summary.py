@@ -74,10 +74,14 @@ def do_full(path: str, cfg: int, tag: str):
            "| kernel | " + " | ".join(c[1] for c in cols if c[1] not in ("dfma", "dadd", "dmul")) + " | executed FP64 GFLOP |",
            "|---|" + "---:|" * (len([c for c in cols if c[1] not in ("dfma", "dadd", "dmul")]) + 1)]
     traffic = {}
+    started = False
     for r in rows[2:]:
         if len(r) < len(hdr):
             continue
         name = short(r[ix["Kernel Name"]])
+        started = started or name == "k_reset_surface"          # (rows before the cut's first kernel belong to the cut before)
+        if not started:
+            continue
         vals = {c[1]: num(r[ix[c[0]]]) * c[2] for c in cols}
         gf = (2 * vals.get("dfma", 0.0) + vals.get("dadd", 0.0) + vals.get("dmul", 0.0)) / 1e9
         out.append("| %s | " % name + " | ".join("%.1f" % vals[c[1]] for c in cols if c[1] not in ("dfma", "dadd", "dmul")) + " | %.3f |" % gf)
