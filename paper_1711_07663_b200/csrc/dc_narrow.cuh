@@ -23,6 +23,7 @@
 #pragma once
 
 #define NPW_THREADS 128
+#define DC_STATUS_INVALID (DC_STATUS_PAIR_OVERFLOW | DC_STATUS_QUEUE_OVERFLOW | DC_STATUS_BAND_OVERFLOW)
 #define DC_MAX_ROUNDS 25            /* 2 * 12 + 1 */
 
 
@@ -201,6 +202,7 @@ __global__ void __launch_bounds__(256) k_np_compact(const DcScalars *S, const in
                                                     const unsigned long long *__restrict__ best,
                                                     NItem *__restrict__ nq_out, NLeafX *__restrict__ nqx_out, int *__restrict__ n_out)
 {
+    if (S->status & DC_STATUS_INVALID) return;
     const int n = min(*n_in, (int)min(in_cap, (long long)0x7fffffff));
     const double tau_exit = S->tau_exit, t_tie = S->t_tie;
     const int n_round = (n + 31) & ~31;
@@ -240,6 +242,7 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
                                                            NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap,
                                                            int budget, int maxit)
 {
+    if (S->status & DC_STATUS_INVALID) return;
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
     const double tau_exit = S->tau_exit, tol_d2 = S->tol_d * S->tol_d, t_tie = S->t_tie;
     const double tau_exit2 = tau_exit > 0.0 ? tau_exit * tau_exit : -1.0;
@@ -408,6 +411,7 @@ __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__res
 {
     __shared__ int s_wsum[8];
     __shared__ int s_base, s_total;
+    if (S->status & DC_STATUS_INVALID) return;       // an overflow upstream left holes in the lists: nothing here can be trusted (or safely read)
     const long long n_pairs = min((long long)S->n_pairs, max_pairs);
     const long long n_round = (n_pairs + 255) & ~255LL;          // (uniform trip count inside a CTA: barriers below)
     const double t_tie = S->t_tie, tau_exit = S->tau_exit;
@@ -543,6 +547,7 @@ __global__ void __launch_bounds__(NPW_THREADS, ROOT ? 3 : 2) k_np_bound(DcScalar
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
                                                           NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap, int force_leaf)
 {
+    if (S->status & DC_STATUS_INVALID) return;
     const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
     if (n == 0) return;
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(&S->c_queue_peak, (unsigned long long)n);
@@ -560,6 +565,7 @@ __global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S,
                                                                    const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                                    NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
 {
+    if (S->status & DC_STATUS_INVALID) return;
     NpCounters cnt = { 0, 0, 0, 0, 0 };
     for (int r = r_begin; r < r_end; ++r) {
         const int n = min(*(volatile int *)&S->qn[r], (int)min(qcap, (long long)0x7fffffff));
