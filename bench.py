@@ -24,6 +24,7 @@ nodes + connectivity + adjacency, surface faces) are resident in HBM before the 
             uniform sample of the same workload's elements, each against ALL faces; `value` counts the SAME
             candidate pairs as the GPU line (those of the sampled elements), per oracle second.
   paper_mode: the paper's own approximate cut (DC_FLAG_PAPER_MODE) on the same context: ms, labels differing from the exact mode.
+  donor_search: the paper's other GPU algorithm (4.3: ADT stack search + Newton point containment), 1 M points.
   per_config: the other BASELINE.json configs (0, 1, 3 incl. the sum over its 32 steps, 4), a few seconds each,
             every one with its own clock record over a timed region of at least 200 ms.
 
@@ -627,6 +628,18 @@ def main():
                                                      "max_abs_dsdist_over_lref": err / ref.stats["l_ref"]}}
     if rank == 0 and world == 1 and cfg != 3 and not args.no_per_config:
         line["paper_mode"] = measure_paper_mode(dcut, face_sets[0], B, stream, torch, np)
+        # the paper's other GPU algorithm (4.3): ADT stack search + Newton point containment, 1 M query points
+        t0 = time.perf_counter(); dcut.build_adt(); t_build = time.perf_counter() - t0
+        q = (torch.rand((1 << 20, 3), dtype=torch.float64, device="cuda:%d" % local_rank) * 1.9 - 0.95)
+        dcut.find_donors(q)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(5):
+            donor, _ref = dcut.find_donors(q)
+        e1.record(stream); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 5
+        line["donor_search"] = {"points": int(q.shape[0]), "ms": ms, "points_per_s": q.shape[0] / (ms * 1e-3),
+                                "found": int((donor >= 0).sum().item()), "adt_build_host_s": t_build}
     dcut.close()
     del dcut
     torch.cuda.empty_cache()

@@ -230,6 +230,27 @@ int dc_unblank(int mode, int cut_is_hole, long long n_elem, const signed char *i
 int dc_ab_faces(long long n_elem, const signed char *iblank_dev, const int *adj6_dev,
                 unsigned char *ab_mask_dev, long long *count_dev, void *stream);
 
+/* ---- donor search for receptor points (PAPER.md 4.3 L229-L278; SURVEY.md 8(f) "(later)") ---------------------------
+ * dc_adt_build: alternating digital tree over the element boxes of S2, built on the HOST (L233: once, during
+ *   preprocessing; valid under rigid motion of the grid) into caller-owned device memory of dc_adt_bytes(n_elem)
+ *   bytes, 16-byte aligned; synchronises `stream`.  Balanced (median splits), so the search needs a LIFO of
+ *   height + 1 entries (L241-L247).
+ * dc_find_donors: for each point x [n_pts][3] f64 dev -- given in the frame the grid has been MOVED to,
+ *   x = R x_grid + o with rot9_host (row-major R, NULL = identity) and off3_host (NULL = 0) -- the element that
+ *   contains it and its reference coordinates: stack-based tree search appending candidate elements (boxes that hold
+ *   the point, at most 16 kept), then Newton on the isoparametric map of each candidate (Eq. 1-5, reference
+ *   coordinates limited to [-1,1] + 1e-10, at most 10 iterations, L272-L278); converged = |x_p - x(X)| <= 1e-12 x
+ *   element box diagonal.
+ *     donor_dev [n_pts] i32 dev   out  element id, -1 if no element contains the point
+ *     ref_dev   [n_pts][3] f64 dev out reference coordinates in the donor (0 if none)
+ *     scratch_dev                      dc_donor_scratch_bytes(n_pts) bytes of device scratch
+ *   A point on a face shared by two elements may be given either (both contain it).  Enqueued on `stream`. */
+size_t dc_adt_bytes(long long n_elem);
+size_t dc_donor_scratch_bytes(long long n_pts);
+int dc_adt_build(dc_ctx *ctx, void *adt_dev, size_t adt_bytes, void *stream);
+int dc_find_donors(dc_ctx *ctx, long long n_pts, const double *pts_dev, const double *rot9_host, const double *off3_host,
+                   int *donor_dev, double *ref_dev, void *scratch_dev, size_t scratch_bytes, void *stream);
+
 /* FP64 FMA peak microbenchmark (register-resident DFMA chains on every SM): returns measured
  * TFLOP/s (2 flop per FMA) or a negative error.  Used by bench.py for the "alu" roofline. */
 double dc_measure_fp64_tflops(int device, int iters);

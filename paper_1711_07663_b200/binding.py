@@ -24,7 +24,8 @@ DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
 EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify",
            "dc_classify_host", "dc_get_element_boxes", "dc_get_adjacency", "dc_get_pairs",
            "dc_get_stats", "dc_destroy", "dc_error_string", "dc_measure_fp64_tflops", "dc_version",
-           "dc_union_labels", "dc_unblank", "dc_ab_faces"]
+           "dc_union_labels", "dc_unblank", "dc_ab_faces",
+           "dc_adt_bytes", "dc_donor_scratch_bytes", "dc_adt_build", "dc_find_donors"]
 
 
 class dc_params(C.Structure):
@@ -80,6 +81,12 @@ _lib.dc_version.restype = C.c_int
 _lib.dc_union_labels.argtypes = [C.c_longlong, _vp, _vp, _vp, _vp]
 _lib.dc_unblank.argtypes = [C.c_int, C.c_int, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp, C.c_longlong, _vp, _vp]
 _lib.dc_ab_faces.argtypes = [C.c_longlong, _vp, _vp, _vp, _vp, _vp]
+_lib.dc_adt_bytes.argtypes = [C.c_longlong]
+_lib.dc_adt_bytes.restype = C.c_size_t
+_lib.dc_donor_scratch_bytes.argtypes = [C.c_longlong]
+_lib.dc_donor_scratch_bytes.restype = C.c_size_t
+_lib.dc_adt_build.argtypes = [_vp, _vp, C.c_size_t, _vp]
+_lib.dc_find_donors.argtypes = [_vp, C.c_longlong, _vp, C.POINTER(C.c_double), C.POINTER(C.c_double), _vp, _vp, _vp, C.c_size_t, _vp]
 
 
 class DcError(RuntimeError):
@@ -262,6 +269,31 @@ class DirectCut:
         if n < 0:
             raise DcError(int(n), "dc_get_pairs")
         return e[:n], f[:n]
+
+    def build_adt(self):
+        """dc_adt_build: the donor-search tree over the element boxes (host build, once)."""
+        t = self.torch
+        nbytes = int(_lib.dc_adt_bytes(self.n_elem))
+        self.adt = t.empty(nbytes + 16, dtype=t.uint8, device=self.xyz.device)
+        off = (-self.adt.data_ptr()) % 16
+        _ck(_lib.dc_adt_build(self.ctx, self.adt.data_ptr() + off, nbytes, self._stream()), "dc_adt_build")
+
+    def find_donors(self, pts, rot=None, offset=None):
+        """dc_find_donors: pts [n][3] (torch CUDA f64 or numpy) -> (donor int32 [n], ref f64 [n][3]) on the device."""
+        t = self.torch
+        if not (isinstance(pts, t.Tensor) and pts.is_cuda):
+            pts = t.as_tensor(pts, dtype=t.float64).contiguous().to(self.xyz.device)
+        pts = pts.contiguous()
+        n = int(pts.shape[0])
+        donor = t.empty(n, dtype=t.int32, device=pts.device)
+        ref = t.empty((n, 3), dtype=t.float64, device=pts.device)
+        sb = int(_lib.dc_donor_scratch_bytes(n))
+        scratch = t.empty(max(sb, 4), dtype=t.uint8, device=pts.device)
+        R = (C.c_double * 9)(*[float(x) for x in rot.reshape(-1)]) if rot is not None else None
+        o = (C.c_double * 3)(*[float(x) for x in offset]) if offset is not None else None
+        _ck(_lib.dc_find_donors(self.ctx, n, pts.data_ptr(), R, o, donor.data_ptr(), ref.data_ptr(), scratch.data_ptr(), sb,
+                                self._stream()), "dc_find_donors")
+        return donor, ref
 
     def close(self):
         if getattr(self, "ctx", None):

@@ -18,6 +18,8 @@
 #include <stdio.h>
 #include <string.h>
 #include <new>
+#include <algorithm>
+#include <vector>
 
 #include "../../include/dc.h"
 #include "dc_geom.cuh"
@@ -941,6 +943,8 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, doubl
     if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+#include "dc_donor.cuh"
+
 // ==========================================================================================
 // host side
 // ==========================================================================================
@@ -968,6 +972,7 @@ struct dc_ctx {
     bool have_surface, have_cut;
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
     DcScalars *S_host;        // pinned
+    const AdtNode *adt; int adt_nodes;   // donor search tree (dc_adt_build), caller's memory
 };
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -1463,5 +1468,50 @@ extern "C" double dc_measure_fp64_tflops(int device, int iters)
 
 #include "dc_blank.cuh"
 
-extern "C" int dc_version(void) { return 2; }
+// ---- donor search (dc_donor.cuh)
+extern "C" size_t dc_adt_bytes(long long n_elem) { return n_elem > 0 ? (size_t)n_elem * sizeof(AdtNode) : 0; }
+extern "C" size_t dc_donor_scratch_bytes(long long n_pts) { return n_pts > 0 ? (size_t)n_pts * (DC_DONOR_CAND + 1) * 4 : 0; }
+
+extern "C" int dc_adt_build(dc_ctx *c, void *adt_dev, size_t adt_bytes, void *stream)
+{
+    if (!c || !adt_dev) return DC_ERR_ARG;
+    if (adt_bytes < dc_adt_bytes(c->n_elem) || ((uintptr_t)adt_dev & 15) != 0) return DC_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(c->device));
+    CK(cudaStreamSynchronize(st));
+    const long long n = c->n_elem;
+    std::vector<double> soa((size_t)n * 6), box((size_t)n * 6);
+    CK(cudaMemcpy(soa.data(), c->ebox, (size_t)n * 6 * 8, cudaMemcpyDeviceToHost));
+    for (long long e = 0; e < n; ++e) for (int k = 0; k < 6; ++k) box[(size_t)e * 6 + k] = soa[(size_t)k * n + e];
+    std::vector<int> ids((size_t)n);
+    for (long long e = 0; e < n; ++e) ids[(size_t)e] = (int)e;
+    std::vector<AdtNode> nodes((size_t)n);
+    dcadt::Builder B; B.box = box.data(); B.nodes = nodes.data(); B.next = 0;
+    B.build(ids.data(), 0, (int)n, 0);
+    CK(cudaMemcpy(adt_dev, nodes.data(), (size_t)n * sizeof(AdtNode), cudaMemcpyHostToDevice));
+    c->adt = (const AdtNode *)adt_dev; c->adt_nodes = (int)n;
+    return DC_OK;
+}
+
+extern "C" int dc_find_donors(dc_ctx *c, long long n_pts, const double *pts_dev, const double *rot9_host, const double *off3_host,
+                              int *donor_dev, double *ref_dev, void *scratch_dev, size_t scratch_bytes, void *stream)
+{
+    if (!c || !pts_dev || !donor_dev || !ref_dev || !scratch_dev || n_pts < 0) return DC_ERR_ARG;
+    if (!c->adt) return DC_ERR_STATE;
+    if (scratch_bytes < dc_donor_scratch_bytes(n_pts)) return DC_ERR_WORKSPACE;
+    if (n_pts == 0) return DC_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(c->device));
+    const double I[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 }, Z[3] = { 0, 0, 0 };
+    const double *R = rot9_host ? rot9_host : I, *o = off3_host ? off3_host : Z;
+    int *cand = (int *)scratch_dev, *cand_n = cand + (size_t)n_pts * DC_DONOR_CAND;
+    k_adt_search<<<nblk(n_pts, 128), 128, 0, st>>>(c->adt, c->adt_nodes, c->ebox, c->n_elem, pts_dev, n_pts, R[0], R[1], R[2], R[3], R[4],
+                                                   R[5], R[6], R[7], R[8], o[0], o[1], o[2], 1e-12, cand, cand_n);
+    k_donor_newton<<<nblk(n_pts, 128), 128, 0, st>>>(c->xyz, c->conn, c->ebox, c->n_elem, pts_dev, n_pts, R[0], R[1], R[2], R[3], R[4],
+                                                     R[5], R[6], R[7], R[8], o[0], o[1], o[2], cand, cand_n, donor_dev, ref_dev);
+    CK(cudaGetLastError());
+    return DC_OK;
+}
+
+extern "C" int dc_version(void) { return 3; }
 
