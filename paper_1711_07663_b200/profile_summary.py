@@ -56,6 +56,10 @@ def do_full(path: str, cfg: int, tag: str):
             ("smsp__thread_inst_executed_per_inst_executed.ratio", "lanes/inst", 1.0),
             ("dram__bytes_read.sum", "DRAM rd MB", None), ("dram__bytes_write.sum", "DRAM wr MB", None),
             ("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "DRAM %", 1.0),
+            ("smsp__average_warps_issue_stalled_long_scoreboard_per_issue_active.ratio", "stall long-sb", 1.0),
+            ("smsp__average_warps_issue_stalled_wait_per_issue_active.ratio", "stall wait", 1.0),
+            ("smsp__average_warps_issue_stalled_barrier_per_issue_active.ratio", "stall barrier", 1.0),
+            ("smsp__inst_executed.sum", "warp inst M", 1e-6),
             ("smsp__sass_thread_inst_executed_op_dfma_pred_on.sum", "dfma", 1.0),
             ("smsp__sass_thread_inst_executed_op_dadd_pred_on.sum", "dadd", 1.0),
             ("smsp__sass_thread_inst_executed_op_dmul_pred_on.sum", "dmul", 1.0)]
@@ -70,7 +74,9 @@ def do_full(path: str, cfg: int, tag: str):
            "ncu -i gpurun_out/prof_%s.ncu-rep --page raw --csv > raw.csv" % tag,
            "python -m paper_1711_07663_b200.profile_summary full raw.csv %d %s" % (cfg, tag), "```", "",
            "Sources: `src_sha16 = %s` (bench.py `config.src_sha16`).  Executed FP64 flops = 2 dfma + dadd + dmul "
-           "(`smsp__sass_thread_inst_executed_op_*_pred_on.sum`, SURVEY.md 8(d)); the algorithmic ones are in the bench line." % source_hash(), "",
+           "(`smsp__sass_thread_inst_executed_op_*_pred_on.sum`, SURVEY.md 8(d)); the algorithmic ones are in the bench line.  "
+           "Stall columns: warps stalled per issue slot (`smsp__average_warps_issue_stalled_*_per_issue_active.ratio`): long scoreboard = "
+           "waiting for global / L2 data, wait = fixed-latency dependency, barrier = `__syncthreads`." % source_hash(), "",
            "| kernel | " + " | ".join(c[1] for c in cols if c[1] not in ("dfma", "dadd", "dmul")) + " | executed FP64 GFLOP |",
            "|---|" + "---:|" * (len([c for c in cols if c[1] not in ("dfma", "dadd", "dmul")]) + 1)]
     traffic = {}
