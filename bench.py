@@ -294,15 +294,17 @@ def run_reference(args, rank: int, world: int):
         nproc = 1
         n_sample = int(max(16, share / per_elem))
     cores = nproc
-    times, own_pairs, cand = [], [], []
+    times, own_pairs, cand_per_elem = [], [], None
     for it in range(args.warmup + args.steps):
         ids, ref, sec = oracle_sample(w, n_sample, nproc, seed=1000 + it)
         if it >= args.warmup:
             times.append(sec); own_pairs.append(ref.stats["n_pair_tests"])
-            reach = ref.stats["d_band"] + 2.0 * ref.stats["tau_cut"] + 1e-9 * ref.stats["l_ref"]
-            cand.append(candidate_pairs_by_oracle_boxes(w, ids, reach))       # (outside the timed interval)
+            if cand_per_elem is None:
+                # (outside the timed interval, once: the samples are uniform, so one of them gives the candidates per element)
+                reach = ref.stats["d_band"] + 2.0 * ref.stats["tau_cut"] + 1e-9 * ref.stats["l_ref"]
+                cand_per_elem = candidate_pairs_by_oracle_boxes(w, ids, reach) / float(len(ids))
     tot = sum(times)
-    value = sum(cand) / tot
+    value = cand_per_elem * len(ids) * len(times) / tot
     ms_cut = 1e3 * (tot / len(times)) * (w.n_elem / float(len(ids)))
     sample = "%d uniformly sampled elements of %d per step, each against all %d faces" % (len(ids), w.n_elem, w.n_face)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
