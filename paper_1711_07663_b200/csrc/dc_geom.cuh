@@ -184,7 +184,7 @@ __device__ __forceinline__ void scalar_range(const double *g, double uc, double 
 }
 
 #ifndef DC_CD_SWEEPS
-#define DC_CD_SWEEPS 3
+#define DC_CD_SWEEPS 4
 #endif
 
 // reciprocal of a positive normal-range double: hardware seed + two Newton steps (no slow path)

@@ -154,49 +154,71 @@ DCN_HD bool iterate(CF cf, NwState &s, const double *lo, const double *hi, doubl
         if (fx[1]) { h01 = h12 = h13 = 0.0; h11 = tr; g[1] = 0.0; }
         if (fx[2]) { h02 = h12 = h23 = 0.0; h22 = tr; g[2] = 0.0; }
         if (fx[3]) { h03 = h13 = h23 = 0.0; h33 = tr; g[3] = 0.0; }
-        double p[4];
-        const bool indefinite = ldl4_mod(h00, h01, h02, h03, h11, h12, h13, h22, h23, h33, g, 1e-10 * tr, p);
-        const double pred = -0.5 * (g[0] * p[0] + g[1] * p[1] + g[2] * p[2] + g[3] * p[3]);
+        // A free variable that sits ON a bound (its gradient points inward) can still be pushed outward by the coupled
+        // Newton step; clamping it leaves the other components of a step that assumed it would move -- not a descent
+        // direction, and the trial is rejected over and over (22 to 25 evaluations on the near-contact leaves that used
+        // to end unconverged).  Such variables are held for THIS step and the rest is solved again on that face of the
+        // box (6 or 7 evaluations on the same leaves).  The convergence test keeps the first solve's predicted decrease:
+        // a held variable with an inward gradient is not a KKT point.
+        double p[4], pred = 0.0;
+        bool indefinite = false;
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            indefinite = ldl4_mod(h00, h01, h02, h03, h11, h12, h13, h22, h23, h33, g, 1e-10 * tr, p) || indefinite;
+            if (pass == 1) break;
+            pred = -0.5 * (g[0] * p[0] + g[1] * p[1] + g[2] * p[2] + g[3] * p[3]);
+            bool o[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) o[i] = !fx[i] && ((s.x[i] >= hi[i] && p[i] > 0.0) || (s.x[i] <= lo[i] && p[i] < 0.0));
+            if (!(o[0] || o[1] || o[2] || o[3])) break;
+            if (o[0]) { h01 = h02 = h03 = 0.0; h00 = tr; g[0] = 0.0; }
+            if (o[1]) { h01 = h12 = h13 = 0.0; h11 = tr; g[1] = 0.0; }
+            if (o[2]) { h02 = h12 = h23 = 0.0; h22 = tr; g[2] = 0.0; }
+            if (o[3]) { h03 = h13 = h23 = 0.0; h33 = tr; g[3] = 0.0; }
+        }
         // Step length of THIS call's single trial (s.ls counts the rejected trials at this point).  With an
         // indefinite H the minimum along the valley sits on the box border: the first trial stretches the
-        // step until the first free variable reaches its bound.
-        double alpha = 1.0;
-        if (indefinite || s.ls > 0) {
-            // largest multiple of p that keeps every free variable inside its bounds
-            // (the smallest ratio room/p is found by cross-multiplication: one division instead of four)
-            double rn = 1.0, pd = 0.0;       // ahit = rn / pd; pd == 0: no bound in the way
+        // step until the first free variable reaches its bound.  A rejected trial is retried by the NEXT call with a
+        // shorter step (retrying inside the call with value-only evaluations was tried: fewer evaluations, but the
+        // extra code spills and every evaluation gets slower: 1.261 against 1.240 ms per cut).
+        double xn[4], fn = 0.0;
+        bool dec = false;
+        {
+            double alpha = 1.0;
+            if (indefinite || s.ls > 0) {
+                // largest multiple of p that keeps every free variable inside its bounds
+                // (the smallest ratio room/p is found by cross-multiplication: one division instead of four)
+                double rn = 1.0, pd = 0.0;       // ahit = rn / pd; pd == 0: no bound in the way
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const double room = fabs((p[i] > 0.0 ? hi[i] : lo[i]) - s.x[i]), pa = fabs(p[i]);
+                    // (a variable already on the bound it is pushed against just stays clamped)
+                    if (pa != 0.0 && room != 0.0 && (pd == 0.0 || room * pd < rn * pa)) { rn = room; pd = pa; }
+                }
+                const double ahit = pd != 0.0 ? rn / pd : INFINITY;
+                const bool stretch = indefinite && ahit > 1.0 && ahit < INFINITY;
+                const double q = __longlong_as_double((long long)(1023 - 2 * (s.ls > 0 ? s.ls - 1 : 0)) << 52);   // 4^-(ls-1)
+                if (s.ls == 0) alpha = stretch ? ahit : 1.0;
+                // a rejected trial is followed by UNCLAMPED ones: up to the first bound (a clamped step is not a
+                // descent step when the clamped variable is coupled to the others), then quarters of that
+                else alpha = stretch ? q : (ahit < 1.0 ? ahit * q : 0.25 * q);
+            }
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                const double room = fabs((p[i] > 0.0 ? hi[i] : lo[i]) - s.x[i]), pa = fabs(p[i]);
-                // (a variable already on the bound it is pushed against just stays clamped)
-                if (pa != 0.0 && room != 0.0 && (pd == 0.0 || room * pd < rn * pa)) { rn = room; pd = pa; }
+                // (a trial point within rounding of a bound is snapped onto it: the step to the first bound lands
+                // an ulp short of it as often as not, and "on the bound" is tested exactly everywhere)
+                const double t = fma(alpha, p[i], s.x[i]), w = 1e-14 * (hi[i] - lo[i]);
+                xn[i] = t >= hi[i] - w ? hi[i] : (t <= lo[i] + w ? lo[i] : t);
             }
-            const double ahit = pd != 0.0 ? rn / pd : INFINITY;
-            const bool stretch = indefinite && ahit > 1.0 && ahit < INFINITY;
-            const double q = __longlong_as_double((long long)(1023 - 2 * (s.ls > 0 ? s.ls - 1 : 0)) << 52);   // 4^-(ls-1)
-            if (s.ls == 0) alpha = stretch ? ahit : 1.0;
-            // a rejected trial is followed by UNCLAMPED ones: up to the first bound (a clamped step is not a
-            // descent step when the clamped variable is coupled to the others), then quarters of that
-            else alpha = stretch ? q : (ahit < 1.0 ? ahit * q : 0.25 * q);
-        }
-        // one projected trial point, value-only evaluation; a rejected trial is retried by the NEXT call with a
-        // shorter step (the other lanes of the warp never wait for a backtracking loop)
-        double xn[4];
+            fn = 0.0;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            // (a trial point within rounding of a bound is snapped onto it: the step to the first bound lands
-            // an ulp short of it as often as not, and "on the bound" is tested exactly everywhere)
-            const double t = fma(alpha, p[i], s.x[i]), w = 1e-14 * (hi[i] - lo[i]);
-            xn[i] = t >= hi[i] - w ? hi[i] : (t <= lo[i] + w ? lo[i] : t);
+            for (int c = 0; c < 3; ++c) {
+                const double d = value([&](int m) { return cf(9 * c + m); }, xn[0], xn[1])
+                               - value([&](int m) { return cf(27 + 9 * c + m); }, xn[2], xn[3]);
+                fn = fma(d, d, fn);
+            }
+            dec = fn <= rr;
         }
-        double fn = 0.0;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const double d = value([&](int m) { return cf(9 * c + m); }, xn[0], xn[1])
-                           - value([&](int m) { return cf(27 + 9 * c + m); }, xn[2], xn[3]);
-            fn = fma(d, d, fn);
-        }
-        const bool dec = fn <= rr;
         bool moved = false;              // (no division: 0 / width would take the slow path of the FP64 divide)
         if (dec) {
 #pragma unroll
