@@ -111,11 +111,11 @@ __device__ __forceinline__ void np_flush_counters(DcScalars *S, const NpCounters
 
 // ------------------------------------------------------------------------------------------
 // Stage: one thread per (band element, boundary patch).  ecoef [b][6][28] (27 monomial coefficients [coord][9] + the
-// higher-order constant K), pbox [b][6][6] (Bezier box of each boundary patch).  (best[b], dmin[b] and the seed item
+// higher-order constant K), pbox [b][6][8] floats (Bezier box of each boundary patch, rounded outward).  (best[b], dmin[b] and the seed item
 // are written by k_pairs, which meets every candidate pair anyway.)
 __global__ void __launch_bounds__(128) k_np_stage(const DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
                                                   const int *__restrict__ band_elem, double *__restrict__ ecoef,
-                                                  double *__restrict__ pbox)
+                                                  float *__restrict__ pbox)
 {
     const int n_band = min(S->n_band, S->max_band);
     const long long n = (long long)n_band * 6;
@@ -149,9 +149,10 @@ __global__ void __launch_bounds__(128) k_np_stage(const DcScalars *S, const doub
         double2 *out = reinterpret_cast<double2 *>(ecoef + (size_t)i * 28);
 #pragma unroll
         for (int m = 0; m < 14; ++m) out[m] = make_double2(A[2 * m], A[2 * m + 1]);
-        double2 *ob = reinterpret_cast<double2 *>(pbox + (size_t)i * 6);
-#pragma unroll
-        for (int m = 0; m < 3; ++m) ob[m] = make_double2(box[2 * m], box[2 * m + 1]);
+        // the patch's box in single precision, rounded OUTWARD (it only feeds k_np_roots' filter)
+        float4 *ob = reinterpret_cast<float4 *>(pbox + (size_t)i * 8);
+        ob[0] = make_float4(__double2float_rd(box[0]), __double2float_rd(box[1]), __double2float_rd(box[2]), 0.f);
+        ob[1] = make_float4(__double2float_ru(box[3]), __double2float_ru(box[4]), __double2float_ru(box[5]), 0.f);
     }
 }
 
@@ -405,7 +406,7 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
 // the patch's Bezier box and the face's Bezier box is within best + t_tie; survivors become the items of round 0
 // (warp-aggregated append: a scan of the lanes' counts, one atomic per warp).
 __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__restrict__ pair_band, const int *__restrict__ pair_face,
-                                                  const double *__restrict__ fbox, const double *__restrict__ pbox,
+                                                  const float *__restrict__ fbox, const float *__restrict__ pbox,
                                                   const unsigned long long *__restrict__ best, long long max_pairs,
                                                   NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
 {
@@ -423,21 +424,18 @@ __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__res
             b = __ldg(pair_band + p);
             const double bst = u2d(__ldg(best + b));
             if (bst > tau_exit) {                                   // (else: already CUT)
-                const double cut = bst + t_tie, cut2 = cut * cut;
-                const double2 *fp = reinterpret_cast<const double2 *>(fbox + (size_t)__ldg(pair_face + p) * 6);
-                const double2 f0 = __ldg(fp), f1 = __ldg(fp + 1), f2 = __ldg(fp + 2);
-                const double fb[6] = { f0.x, f0.y, f1.x, f1.y, f2.x, f2.y };
-                const double2 *pb = reinterpret_cast<const double2 *>(pbox + (size_t)b * 36);
+                // single precision, conservative: boxes rounded outward, gaps and their squares rounded down, the cutoff up
+                const float cutf = __double2float_ru(bst + t_tie), cut2 = __fmul_ru(cutf, cutf);
+                const float4 *fp = reinterpret_cast<const float4 *>(fbox) + (size_t)__ldg(pair_face + p) * 2;
+                const float4 flo = __ldg(fp), fhi = __ldg(fp + 1);
+                const float4 *pb = reinterpret_cast<const float4 *>(pbox) + (size_t)b * 12;
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
-                    const double2 b0 = __ldg(pb + 3 * k), b1 = __ldg(pb + 3 * k + 1), b2 = __ldg(pb + 3 * k + 2);
-                    const double bb[6] = { b0.x, b0.y, b1.x, b1.y, b2.x, b2.y };
-                    double d2 = 0.0;
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        const double g = dmax2(0.0, dmax2(fb[c] - bb[3 + c], bb[c] - fb[3 + c]));
-                        d2 = fma(g, g, d2);
-                    }
+                    const float4 plo = __ldg(pb + 2 * k), phi = __ldg(pb + 2 * k + 1);
+                    const float gx = fmaxf(0.f, fmaxf(__fsub_rd(flo.x, phi.x), __fsub_rd(plo.x, fhi.x)));
+                    const float gy = fmaxf(0.f, fmaxf(__fsub_rd(flo.y, phi.y), __fsub_rd(plo.y, fhi.y)));
+                    const float gz = fmaxf(0.f, fmaxf(__fsub_rd(flo.z, phi.z), __fsub_rd(plo.z, fhi.z)));
+                    const float d2 = __fadd_rd(__fadd_rd(__fmul_rd(gx, gx), __fmul_rd(gy, gy)), __fmul_rd(gz, gz));
                     if (d2 <= cut2) mask |= 1u << k;
                 }
             }
