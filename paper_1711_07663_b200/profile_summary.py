@@ -69,7 +69,7 @@ def do_full(path: str, cfg: int, tag: str):
            BENCH_CMD % cfg + " > gpurun_out/plain.log 2>&1 &&",
            "ncu --set full --metrics smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,"
            "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum \\",
-           "    --clock-control none --import-source on -k regex:'k_' --launch-skip 105 -c 35 \\",
+           "    --clock-control none --import-source on -k regex:'k_' --launch-skip 106 -c 35 \\",
            "    -f -o gpurun_out/prof_%s " % tag + BENCH_CMD % cfg,
            "ncu -i gpurun_out/prof_%s.ncu-rep --page raw --csv > raw.csv" % tag,
            "python -m paper_1711_07663_b200.profile_summary full raw.csv %d %s" % (cfg, tag), "```", "",
