@@ -53,9 +53,9 @@ METRIC = "element_face_pair_tests_per_s"
 UNIT = "pair tests/s"
 
 # algorithmic fp64 flops per operation of the narrow phase (FMA = 2)
-FLOP_PER_BNB_NODE = 850.0       # centre evals with first derivatives 183, norms + leaf rule 45, model closest pair 250, true patches there 120,
+FLOP_PER_BNB_NODE = 920.0       # centre evals with first derivatives 183, norms + leaf rule 45, model closest pair 320 (4 sweeps), true patches there 120,
 #                                 2 x 8 projected coefficients 80, 2 Bernstein ranges 170
-FLOP_PER_BNB_ROOT = 585.0       # a whole patch pair (round 0): no centre evaluation (-180), no re-centring in the two ranges (-85)
+FLOP_PER_BNB_ROOT = 655.0       # a whole patch pair (round 0): no centre evaluation (-180), no re-centring in the two ranges (-85)
 FLOP_PER_NEWTON_EVAL = 560.0    # 6 jets x 36 + (r, g, H) 3 x 43 + LDL^T 4x4 ~75 + trial point and its value 6 x 16 + 17 + tests ~35
 FLOP_PER_NEWTON_FINISH = 40.0   # normal, cosine, distance of a finished solve
 # S2 algorithmic bytes: every conn row (108 B) and every node (24 B) read once, one box (48 B) written per element
