@@ -84,6 +84,17 @@ extern "C" {
                                        those of that method (its linearisation error included): for comparison with the exact
                                        mode, not for parity with the exact oracle.  S4 and S7 are unchanged. */
 
+#define DC_FLAG_EXACT_FAR 4         /* exact distance EVERYWHERE (reading A5's alternative, "d_band = infinity"; SURVEY.md 8(f)
+                                       NEXT-4): after the banded cut and the flood fill, every element still clamped at
+                                       +-d_band gets sdist = +-d_e -- the magnitude from the same narrow phase (S5) run on the
+                                       faces whose box is within an attained upper bound of the element (nearest-bin walk
+                                       over an octree of the face bins, so no N_e x N_f pair list), the sign from S7.  Labels
+                                       are unchanged.  Runs in passes sized to the workspace and SYNCHRONISES the stream
+                                       after each; dc_get_pairs is not available afterwards.  Costs about 20-40 x the banded
+                                       cut on the configs of BASELINE.json.  Ignored with DC_FLAG_PAPER_MODE.
+                                       A pass holds max_pairs / 6 pairs: DC_ERR_WORKSPACE (dc_get_stats) when ONE element
+                                       has more candidate faces than that (pairs_needed says what max_pairs would do). */
+
 typedef struct dc_ctx dc_ctx;
 
 typedef struct {
@@ -116,6 +127,11 @@ typedef struct {
     long long band_needed;       /* elements with candidate pairs (> the band capacity on DC_STATUS_BAND_OVERFLOW) */
     long long queue_needed;      /* largest narrow-phase queue any round wanted (> the capacity max(2^20, max_pairs) on
                                     DC_STATUS_QUEUE_OVERFLOW: size max_pairs >= queue_needed) */
+    long long n_far;             /* DC_FLAG_EXACT_FAR: elements the banded cut left clamped at +-d_band ... */
+    long long n_far_done;        /* ... of which got their exact distance (= n_far unless the pass failed) */
+    long long n_far_unresolved;  /* ... and for which the narrow phase solved no leaf (0; they keep the clamp) */
+    long long far_pairs;         /* candidate pairs of the far pass, all chunks */
+    long long far_chunks;        /* passes the far pass ran in (each ends with a stream synchronisation) */
     double l_ref, tau_cut, d_band;
     float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
                                     4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface,
@@ -126,7 +142,9 @@ typedef struct {
                                     4 k_np_compact, 5 k_np_solve leaf passes 1-3, 6 overflow rounds (2 x bound + solve),
                                     7 k_np_decide */
     int status;                  /* DC_STATUS_* bits */
-    int n_launches;              /* kernels launched by the last dc_set_cut_surface + dc_classify */
+    int n_launches;              /* kernels launched by the last dc_set_cut_surface + dc_classify (far pass not counted) */
+    float ms_far;                /* the exact far pass, host synchronisations included (CUDA events) */
+    int reserved;
 } dc_stats;
 
 /* Bytes of device scratch dc_create_grid needs for a grid of this size, up to max_faces
@@ -163,7 +181,9 @@ int dc_set_cut_surface(dc_ctx *ctx, long long n_face, const double *face_nodes_d
  * One direct cut (S4 candidate pairs, S5 narrow phase, S6 decide, S7 flood fill; S2 too with
  * DC_FLAG_RECOMPUTE_BOXES).  params may be NULL (all defaults).
  *   labels_dev [n_elem] int8 dev  out    DC_HOLE / DC_NORMAL / DC_CUT   (L217 "blanking status ... saved to memory")
- *   sdist_dev  [n_elem] f64  dev  out    signed min distance, clamped to +-d_band, 0 for CUT
+ *   sdist_dev  [n_elem] f64  dev  out    signed min distance, clamped to +-d_band (not clamped with
+ *                                        DC_FLAG_EXACT_FAR), 0 for CUT
+ * Asynchronous on `stream`, except with DC_FLAG_EXACT_FAR.
  */
 int dc_classify(dc_ctx *ctx, const dc_params *params, signed char *labels_dev, double *sdist_dev,
                 void *stream);

@@ -7,7 +7,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(_HERE, "csrc", "dc_kernels.cu")]
-DEPS = SRC + [os.path.join(_HERE, "csrc", h) for h in ("dc_geom.cuh", "dc_narrow.cuh", "dc_newton.cuh", "dc_blank.cuh", "dc_paper.cuh", "dc_donor.cuh")] + [
+DEPS = SRC + [os.path.join(_HERE, "csrc", h) for h in ("dc_geom.cuh", "dc_narrow.cuh", "dc_newton.cuh", "dc_blank.cuh", "dc_paper.cuh", "dc_donor.cuh", "dc_far.cuh")] + [
               os.path.join(os.path.dirname(_HERE), "include", "dc.h")]
 LIB = os.path.join(_HERE, "libdc.so")
 

@@ -19,6 +19,7 @@ DC_STATUS_PAIR_OVERFLOW, DC_STATUS_QUEUE_OVERFLOW, DC_STATUS_FILL_CONFLICT, DC_S
 DC_STATUS_BAND_OVERFLOW, DC_STATUS_SURFACE_SMALL = 16, 32
 DC_FLAG_RECOMPUTE_BOXES = 1
 DC_FLAG_PAPER_MODE = 2
+DC_FLAG_EXACT_FAR = 4
 DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
 
 EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify",
@@ -42,8 +43,11 @@ class dc_stats(C.Structure):
                 ("n_seedless_components", C.c_longlong), ("n_fill_conflicts", C.c_longlong),
                 ("pairs_needed", C.c_longlong), ("queue_peak", C.c_longlong),
                 ("n_root_nodes", C.c_longlong), ("band_needed", C.c_longlong), ("queue_needed", C.c_longlong),
+                ("n_far", C.c_longlong), ("n_far_done", C.c_longlong), ("n_far_unresolved", C.c_longlong),
+                ("far_pairs", C.c_longlong), ("far_chunks", C.c_longlong),
                 ("l_ref", C.c_double), ("tau_cut", C.c_double), ("d_band", C.c_double),
-                ("ms_stage", C.c_float * 8), ("ms_kernel", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int)]
+                ("ms_stage", C.c_float * 8), ("ms_kernel", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int),
+                ("ms_far", C.c_float), ("reserved", C.c_int)]
 
     def as_dict(self) -> dict:
         d = {}
@@ -126,12 +130,12 @@ def dc_classify_host(ctx, params: Optional[dc_params], n_face, faces_host_ptr, l
                               labels_host_ptr, sdist_host_ptr, stream or None), "dc_classify_host")
 
 
-def dc_get_stats(ctx, allow_status: bool = False) -> dc_stats:
+def dc_get_stats(ctx, allow_status: bool = False, return_code: bool = False):
     st = dc_stats()
     rc = _lib.dc_get_stats(ctx, C.byref(st))
     if rc != DC_OK and not (allow_status and rc in (DC_ERR_WORKSPACE, DC_ERR_RESULT, DC_ERR_UNSUPPORTED)):
         raise DcError(rc, "dc_get_stats (status=%d, pairs_needed=%d)" % (st.status, st.pairs_needed))
-    return st
+    return (st, rc) if return_code else st
 
 
 def dc_destroy(ctx):
@@ -247,8 +251,8 @@ class DirectCut:
         dc_classify_host(self.ctx, params, int(faces_host.shape[0]), faces_host.data_ptr(),
                          labels_host.data_ptr(), sdist_host.data_ptr(), self._stream())
 
-    def stats(self, allow_status: bool = False) -> dc_stats:
-        return dc_get_stats(self.ctx, allow_status)
+    def stats(self, allow_status: bool = False, return_code: bool = False):
+        return dc_get_stats(self.ctx, allow_status, return_code)
 
     def element_boxes(self):
         out = self.torch.empty((self.n_elem, 6), dtype=self.torch.float64, device=self.xyz.device)

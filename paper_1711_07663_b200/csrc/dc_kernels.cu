@@ -70,6 +70,13 @@ struct DcScalars {
     unsigned long long c_box_tests, c_bnb_nodes, c_newton, c_newton_iters, c_newton_fail,
         c_depth_exceeded, c_cut, c_hole, c_normal, c_ambiguous, c_sign_ambiguous,
         c_fill_conflicts, c_queue_peak, c_seedless_total;
+    // DC_FLAG_EXACT_FAR (dc_far.cuh): the two lists of far elements still to do (ping-pong), the chunk's and the pass's tallies
+    int far_n[2];
+    int far_chunk_done, far_done, far_unresolved, far_pad;
+    unsigned long long far_end;         // end of the pair slots handed out in this chunk
+    unsigned long long far_want;        // most candidates a deferred element asked for
+    unsigned long long far_pairs_total;
+    unsigned long long far_lo[3], far_hi[3];    // box of the far elements' centres (ordered-uint encodings)
 };
 
 __device__ __forceinline__ void atomic_min_d(unsigned long long *addr, double v) { atomicMin(addr, enc_ord(v)); }
@@ -396,6 +403,9 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
     S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
     S->c_depth_exceeded = S->c_cut = S->c_hole = S->c_normal = S->c_ambiguous = 0ull;
     S->c_sign_ambiguous = S->c_fill_conflicts = S->c_queue_peak = S->c_seedless_total = 0ull;
+    S->far_n[0] = S->far_n[1] = 0; S->far_chunk_done = S->far_done = S->far_unresolved = 0;
+    S->far_end = S->far_want = S->far_pairs_total = 0ull;
+    for (int c = 0; c < 3; ++c) { S->far_lo[c] = ~0ull; S->far_hi[c] = 0ull; }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -614,6 +624,7 @@ __constant__ int c_face_node[6][9] = {
 
 #include "dc_narrow.cuh"
 #include "dc_paper.cuh"
+#include "dc_far.cuh"
 
 // ------------------------------------------------------------------------------------------
 // S7: flood fill = connected components of the face-adjacency graph of non-CUT elements
@@ -973,12 +984,17 @@ struct dc_ctx {
     int *pair_face; unsigned long long *pair_key; int *pair_band;
     double *fbox_orig, *fbox, *fcoef; int *fcell, *fperm; float *fboxf;
     int *cell_count, *cell_start, *cell_fill; unsigned char *occ;
+    int *pyr;                 // octree over the face bins (DC_FLAG_EXACT_FAR)
+    float *ffar;              // [max_faces][16]: per-face records of the far pass
+    int *far_sorted, *far_bins;   // the far elements in Morton order; the bins of the counting sort that makes it
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
-    cudaEvent_t ev[12], evk[10];    // evk: boundaries between the kernels of S5/S6
+    cudaEvent_t ev[14], evk[10];    // evk: boundaries between the kernels of S5/S6
     cudaStream_t last_stream;
     bool have_surface, have_cut;
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
     DcScalars *S_host;        // pinned
+    DcScalars *S_band_host;   // pinned: the scalars as the banded cut left them, when a far pass has run since
+    bool far_ran; int far_chunks; long long far_n_total; int far_error;
     const AdtNode *adt; int adt_nodes;   // donor search tree (dc_adt_build), caller's memory
 };
 
@@ -988,7 +1004,7 @@ struct WsLayout {
     size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_tile_flag, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
         off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq, off_nqx,
         off_pair_face, off_pair_key, off_pair_band, off_fbox_orig, off_fbox, off_fboxf, off_fcoef, off_fcell, off_fperm,
-        off_cell_count, off_cell_start, off_cell_fill, off_occ, off_hfaces, off_hlabels, off_hsdist, total;
+        off_cell_count, off_cell_start, off_cell_fill, off_occ, off_pyr, off_ffar, off_far_sorted, off_far_bins, off_hfaces, off_hlabels, off_hsdist, total;
     long long max_band, qcap;
 };
 
@@ -1041,6 +1057,10 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_cell_start = take((size_t)(DC_NCELL + 1) * 4);
     L.off_cell_fill = take((size_t)(DC_NCELL + 8 + SCAN_NCHUNK) * 4);   // + the scan's chunk sums
     L.off_occ = take((size_t)DC_OCC * DC_OCC * DC_OCC);
+    L.off_pyr = take((size_t)DC_PYR_TOTAL * 4);
+    L.off_ffar = take((size_t)max_faces * 16 * 4);
+    L.off_far_sorted = take((size_t)n_elem * 4);
+    L.off_far_bins = take((size_t)(3 * (DC_NCELL + 8) + SCAN_NCHUNK) * 4);
     L.off_hfaces = take((size_t)max_faces * 27 * 8);
     L.off_hlabels = take((size_t)n_elem);
     L.off_hsdist = take((size_t)n_elem * 8);
@@ -1112,13 +1132,18 @@ static int create_grid_body(dc_ctx *c, int num_sms, int device, long long n_node
     c->cell_start = (int *)(c->ws + L.off_cell_start);
     c->cell_fill = (int *)(c->ws + L.off_cell_fill);
     c->occ = c->ws + L.off_occ;
+    c->pyr = (int *)(c->ws + L.off_pyr);
+    c->ffar = (float *)(c->ws + L.off_ffar);
+    c->far_sorted = (int *)(c->ws + L.off_far_sorted);
+    c->far_bins = (int *)(c->ws + L.off_far_bins);
     c->h_faces_dev = (double *)(c->ws + L.off_hfaces);
     c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
     c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
     c->last_stream = st;
-    for (int i = 0; i < 12; ++i) CK(cudaEventCreate(&c->ev[i]));
+    for (int i = 0; i < 14; ++i) CK(cudaEventCreate(&c->ev[i]));
     for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->evk[i]));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
+    CK(cudaMallocHost((void **)&c->S_band_host, sizeof(DcScalars)));
     CK(cudaMemsetAsync(c->S, 0, sizeof(DcScalars), st));
     CK(cudaMemsetAsync(c->tile_flag, 0, (size_t)(n_elem / UF_TILE + 2) * 4, st));
     int rc = run_elem_boxes(c, st);
@@ -1189,6 +1214,137 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
     return DC_OK;
 }
 
+// S5 as a launch sequence (dc_narrow.cuh).  part 0: the band's narrow phase, with the events that time it.  The exact far
+// pass (dc_far.cuh) runs the same kernels on its own elements: part 1 = stage + seed solves (once per slice), part 2 = roots
+// to the last solve (once per pass, after the pass's candidate pairs have been written).
+#define EVREC(ev_, st_) do { if (part == 0) CK(cudaEventRecord(ev_, st_)); } while (0)
+static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds, int part)
+{
+    // ---- S5: wavefront narrow phase (dc_narrow.cuh)
+    const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
+    DcScalars *S = c->S;
+    if (part != 2) k_np_stage<<<gw, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox);
+    // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
+    // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
+    const int gs = c->num_sms * 2 * 4;     // solve grids: grid-stride, 2 resident CTAs of 128 threads per SM
+    EVREC(c->ev[7], st);
+    if (part != 2)
+        k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                                 c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT);
+    if (part == 1) { CK(cudaGetLastError()); return DC_OK; }
+    EVREC(c->ev[10], st);
+    k_np_roots<<<c->num_sms * 8, 256, 0, st>>>(S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
+                                               c->q[0], &S->qn[0], c->qcap);
+    // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
+    // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
+    EVREC(c->evk[0], st);
+    k_np_bound<true><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                 c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
+    for (int r = 1; r < grid_rounds; ++r)
+        k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                      c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
+    if (rounds > grid_rounds)
+        k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                       c->nq, c->nqx, &S->nn[0], c->qcap);
+    // all leaves: first dropped if their element's best distance has fallen below their lower bound meanwhile (the two
+    // bound queues are free by now and take the compacted leaf queue), then three solve passes (the old leaf queue's
+    // memory holds the continuations and the overflow queue of sub-leaves)
+    EVREC(c->ev[5], st);
+    NItem *lq = c->q[0]; NLeafX *lqx = (NLeafX *)c->q[1];
+    NCont *contA = (NCont *)c->nq, *contB = (NCont *)c->nqx;
+    const long long capA = c->qcap / 4, capB = c->qcap / 8;
+    NItem *ovf1 = (NItem *)c->nqx + c->qcap / 2;
+    const long long cap_ovf1 = c->qcap / 2;
+    k_np_compact<<<c->num_sms * 8, 256, 0, st>>>(S, &S->nn[0], c->qcap, c->nq, c->nqx, c->best, lq, lqx, &S->nn[5]);
+    EVREC(c->evk[1], st);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[5], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, contA, &S->nh[0], capA, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET1, NW_MAXIT);
+    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[0], capA, nullptr, nullptr, contA, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, contB, &S->nh[1], capB, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET2, NW_MAXIT);
+    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[1], capB, nullptr, nullptr, contB, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, ovf1, &S->nn[1], cap_ovf1, 0, NW_MAXIT);
+    EVREC(c->evk[2], st);
+    // The sub-leaves of unconverged solves come back through one bound pass (best[b] is final or nearly so: most of them
+    // are pruned) and one solve launch, twice; the last launch finishes whatever still fails on the lane that held it.
+    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[2], c->qcap, 1);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[2], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, c->nq, &S->nn[3], c->qcap, 0, NW_OVF_MAXIT);
+    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[4], c->qcap, 1);
+    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[4], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_OVF_MAXIT);
+    EVREC(c->ev[6], st);
+    CK(cudaGetLastError());
+    return DC_OK;
+}
+#undef EVREC
+
+// DC_FLAG_EXACT_FAR: the exact distance of the elements the banded cut left clamped (dc_far.cuh).  Slices of at most
+// max_band elements (the narrow phase keeps 1.3 KB of patch coefficients per element), passes sized to the pair list within a
+// slice.  Synchronises the stream (two counters are read back per pass).
+static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_dev, double *sdist_dev, int rounds, int grid_rounds)
+{
+    DcScalars *S = c->S;
+    const long long ne = c->n_elem;
+    unsigned char *pmask = (unsigned char *)c->pyr;
+    CK(cudaEventRecord(c->ev[11], st));
+    k_far_pyramid<<<nblk(DC_PYR_TOTAL, 128), 128, 0, st>>>(c->cell_start, pmask);
+    k_far_faces<<<nblk(c->n_face, 128), 128, 0, st>>>(S, c->fcoef, c->fbox, (int)c->n_face, c->ffar);
+    k_far_list<<<nblk(ne, 256), 256, 0, st>>>(S, ne, labels_dev, sdist_dev, c->ebox, c->act_elem);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(c->S_band_host, S, sizeof(DcScalars), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    c->far_ran = true; c->far_chunks = 0; c->far_error = 0;
+    long long n_far = c->S_band_host->far_n[0];
+    c->far_n_total = n_far;
+    if (c->S_band_host->status & DC_STATUS_INVALID) n_far = 0;       // (the banded cut itself failed: nothing to refine)
+    // the union-find arrays are free by now: act_elem holds the far elements as found, parent their Morton codes and, once
+    // they are sorted by those, their nearest faces
+    int *list = c->far_sorted, *fstar = c->parent;
+    if (n_far > 0) {
+        int *bin_count = c->far_bins, *bin_start = bin_count + DC_NCELL + 8, *bin_fill = bin_start + DC_NCELL + 8, *chunk = bin_fill + DC_NCELL + 8;
+        CK(cudaMemsetAsync(bin_count, 0, (size_t)(DC_NCELL + 8) * 4, st));
+        CK(cudaMemsetAsync(bin_fill, 0, (size_t)(DC_NCELL + 8) * 4, st));
+        k_far_codes<<<nblk(n_far, 256), 256, 0, st>>>(S, c->act_elem, c->ebox, ne, c->parent, bin_count);
+        k_scan_sums<<<SCAN_NCHUNK, 256, 0, st>>>(bin_count, chunk);
+        k_scan_cells<<<SCAN_NCHUNK, 256, 0, st>>>(bin_count, chunk, bin_start);
+        k_far_sort<<<nblk(n_far, 256), 256, 0, st>>>(S, c->act_elem, c->parent, bin_start, bin_fill, list);
+    }
+    if (n_far > 0)
+        k_far_nearest<<<nblk(n_far, 128), 128, 0, st>>>(S, list, (int)n_far, c->ebox, ne, c->cell_start, pmask, c->ffar, fstar);
+    // pair slots of one pass: a sixth of the list, so that the root items (up to 6 per pair: the patches of a small distant
+    // element are all about as near as each other) fit the queues
+    const long long cap = (c->max_pairs < c->qcap ? c->max_pairs : c->qcap) / 6;
+    for (long long s0 = 0; s0 < n_far && !c->far_error; s0 += c->max_band) {
+        const long long m = n_far - s0 < c->max_band ? n_far - s0 : c->max_band;
+        k_far_reset<<<1, 1, 0, st>>>(S, (int)m, 1);
+        k_far_slots<<<nblk(m, 256), 256, 0, st>>>(list + s0, fstar + s0, (int)m, c->band_elem, c->band_start, c->band_cnt, c->pair_face,
+                                                   c->pair_key, c->pair_band, c->nq, c->best, c->dmin);
+        { const int rc = launch_narrow(c, st, rounds, grid_rounds, 1); if (rc) return rc; }
+        k_far_count<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_cnt, c->best);
+        long long pending = m;
+        while (pending > 0 && !c->far_error) {
+            k_far_reset<<<1, 1, 0, st>>>(S, (int)m, 0);
+            k_far_pairs<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_start, c->band_cnt,
+                                                       c->pair_face, c->pair_key, c->pair_band, c->best, cap);
+            k_far_fix<<<1, 1, 0, st>>>(S);
+            { const int rc = launch_narrow(c, st, rounds, grid_rounds, 2); if (rc) return rc; }
+            k_far_decide<<<nblk(m, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->dmin, labels_dev, sdist_dev);
+            CK(cudaGetLastError());
+            CK(cudaMemcpyAsync(c->S_host, S, sizeof(DcScalars), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            ++c->far_chunks;
+            const int done = c->S_host->far_chunk_done;
+            if (c->S_host->status & DC_STATUS_INVALID) c->far_error = 1;          // (a queue of the narrow phase overflowed)
+            else if (done == 0) c->far_error = 2;                                    // (an element's candidates exceed a pass)
+            pending -= done;
+        }
+    }
+    CK(cudaEventRecord(c->ev[12], st));
+    return DC_OK;
+}
+
 extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labels_dev, double *sdist_dev, void *stream)
 {
     if (!c || !labels_dev || !sdist_dev) return DC_ERR_ARG;
@@ -1232,59 +1388,8 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
         k_pm_decide<<<g, 128, 0, st>>>(S, c->band_elem, c->face_nodes, W, labels_dev, sdist_dev);
         CK(cudaEventRecord(c->ev[3], st));
     } else {
-    // ---- S5: wavefront narrow phase (dc_narrow.cuh)
-    const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
+    { const int rc = launch_narrow(c, st, rounds, grid_rounds, 0); if (rc) return rc; }
     DcScalars *S = c->S;
-    k_np_stage<<<gw, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox);
-    // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
-    // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
-    const int gs = c->num_sms * 2 * 4;     // solve grids: grid-stride, 2 resident CTAs of 128 threads per SM
-    CK(cudaEventRecord(c->ev[7], st));
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT);
-    CK(cudaEventRecord(c->ev[10], st));
-    k_np_roots<<<c->num_sms * 8, 256, 0, st>>>(S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
-                                               c->q[0], &S->qn[0], c->qcap);
-    // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
-    // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
-    CK(cudaEventRecord(c->evk[0], st));
-    k_np_bound<true><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                 c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
-    for (int r = 1; r < grid_rounds; ++r)
-        k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                      c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
-    if (rounds > grid_rounds)
-        k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                       c->nq, c->nqx, &S->nn[0], c->qcap);
-    // all leaves: first dropped if their element's best distance has fallen below their lower bound meanwhile (the two
-    // bound queues are free by now and take the compacted leaf queue), then three solve passes (the old leaf queue's
-    // memory holds the continuations and the overflow queue of sub-leaves)
-    CK(cudaEventRecord(c->ev[5], st));
-    NItem *lq = c->q[0]; NLeafX *lqx = (NLeafX *)c->q[1];
-    NCont *contA = (NCont *)c->nq, *contB = (NCont *)c->nqx;
-    const long long capA = c->qcap / 4, capB = c->qcap / 8;
-    NItem *ovf1 = (NItem *)c->nqx + c->qcap / 2;
-    const long long cap_ovf1 = c->qcap / 2;
-    k_np_compact<<<c->num_sms * 8, 256, 0, st>>>(S, &S->nn[0], c->qcap, c->nq, c->nqx, c->best, lq, lqx, &S->nn[5]);
-    CK(cudaEventRecord(c->evk[1], st));
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[5], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, contA, &S->nh[0], capA, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET1, NW_MAXIT);
-    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[0], capA, nullptr, nullptr, contA, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, contB, &S->nh[1], capB, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET2, NW_MAXIT);
-    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[1], capB, nullptr, nullptr, contB, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, ovf1, &S->nn[1], cap_ovf1, 0, NW_MAXIT);
-    CK(cudaEventRecord(c->evk[2], st));
-    // The sub-leaves of unconverged solves come back through one bound pass (best[b] is final or nearly so: most of them
-    // are pruned) and one solve launch, twice; the last launch finishes whatever still fails on the lane that held it.
-    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
-                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[2], c->qcap, 1);
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[2], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, c->nq, &S->nn[3], c->qcap, 0, NW_OVF_MAXIT);
-    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
-                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[4], c->qcap, 1);
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[4], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_OVF_MAXIT);
-    CK(cudaEventRecord(c->ev[6], st));
     k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
     CK(cudaEventRecord(c->ev[3], st));
@@ -1298,6 +1403,11 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     k_uf_fix<<<c->num_sms * 4, 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev[4], st));
+    c->far_ran = false;
+    if ((P.flags & DC_FLAG_EXACT_FAR) && !(P.flags & DC_FLAG_PAPER_MODE)) {
+        const int rc = run_exact_far(c, st, labels_dev, sdist_dev, rounds, grid_rounds);
+        if (rc) return rc;
+    }
     c->launches_classify = ((P.flags & DC_FLAG_PAPER_MODE) ? 13 : 21 + grid_rounds + (rounds > grid_rounds ? 1 : 0)) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
     return DC_OK;
@@ -1340,7 +1450,7 @@ extern "C" int dc_get_adjacency(dc_ctx *c, int *out_dev, void *stream)
 extern "C" long long dc_get_pairs(dc_ctx *c, int *elem_host, int *face_host, long long cap)
 {
     if (!c || !elem_host || !face_host) return DC_ERR_ARG;
-    if (!c->have_cut) return DC_ERR_STATE;
+    if (!c->have_cut || c->far_ran) return DC_ERR_STATE;     // (the chunks of an exact far pass have overwritten the band's lists)
     CK(cudaStreamSynchronize(c->last_stream));
     CK(cudaMemcpy(c->S_host, c->S, sizeof(DcScalars), cudaMemcpyDeviceToHost));
     const int na = c->S_host->n_band < (int)c->max_band ? c->S_host->n_band : (int)c->max_band;
@@ -1374,8 +1484,22 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
     CK(cudaSetDevice(c->device));
     CK(cudaStreamSynchronize(c->last_stream));
     CK(cudaMemcpy(c->S_host, c->S, sizeof(DcScalars), cudaMemcpyDeviceToHost));
-    const DcScalars &S = *c->S_host;
+    // after an exact far pass the band's counters are the ones saved before it (its chunks reuse the band's lists)
+    const bool far = c->have_cut && c->far_ran;
+    DcScalars &S = far ? *c->S_band_host : *c->S_host;
     memset(o, 0, sizeof *o);
+    if (far) {
+        const DcScalars &F = *c->S_host;
+        S.status |= F.status;
+        o->n_far = c->far_n_total; o->n_far_done = F.far_done; o->n_far_unresolved = F.far_unresolved;
+        o->far_pairs = (long long)F.far_pairs_total; o->far_chunks = c->far_chunks;
+        if (c->far_error == 2) {            // one element's candidates do not fit a chunk (a third of max_pairs)
+            S.status |= DC_STATUS_PAIR_OVERFLOW;
+            S.n_pairs = 6ull * (F.far_want + 1ull) + 16ull;
+        }
+        float ms;
+        if (cudaEventElapsedTime(&ms, c->ev[11], c->ev[12]) == cudaSuccess) o->ms_far = ms;
+    }
     o->n_elem = c->n_elem; o->n_face = c->n_face;
     o->n_active = S.n_active; o->n_box_tests = (long long)S.c_box_tests;
     o->n_pairs = (long long)S.n_pairs > c->max_pairs ? c->max_pairs : (long long)S.n_pairs;
@@ -1389,6 +1513,11 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
     o->queue_peak = (long long)S.c_queue_peak;
     o->n_root_nodes = S.qn[0]; o->band_needed = S.n_band;
     for (int i = 0; i < DC_NQN; ++i) { if (S.qn[i] > o->queue_needed) o->queue_needed = S.qn[i]; if (S.nn[i] > o->queue_needed) o->queue_needed = S.nn[i]; }
+    if (far)        // (the last pass of the far pass: on DC_STATUS_QUEUE_OVERFLOW, what its largest queue wanted)
+        for (int i = 0; i < DC_NQN; ++i) {
+            if (c->S_host->qn[i] > o->queue_needed) o->queue_needed = c->S_host->qn[i];
+            if (c->S_host->nn[i] > o->queue_needed) o->queue_needed = c->S_host->nn[i];
+        }
     o->l_ref = S.l_ref; o->tau_cut = S.tau; o->d_band = S.d_band;
     o->status = S.status;
     o->n_launches = (c->have_surface ? c->launches_surface : 0) + (c->have_cut ? c->launches_classify : 0);
@@ -1427,9 +1556,10 @@ extern "C" void dc_destroy(dc_ctx *c)
     if (!c) return;
     cudaSetDevice(c->device);
     if (c->last_stream || true) cudaStreamSynchronize(c->last_stream);
-    for (int i = 0; i < 12; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 14; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 10; ++i) if (c->evk[i]) cudaEventDestroy(c->evk[i]);
     if (c->S_host) cudaFreeHost(c->S_host);
+    if (c->S_band_host) cudaFreeHost(c->S_band_host);
     delete c;
 }
 

@@ -57,7 +57,7 @@ def test_struct_layouts_match_header():
     # sizes the binding assumes == what the header implies (doubles then ints, natural alignment)
     from paper_1711_07663_b200 import binding
     assert ctypes.sizeof(binding.dc_params) == 4 * 8 + 2 * 4
-    assert ctypes.sizeof(binding.dc_stats) == 22 * 8 + 3 * 8 + 8 * 4 + 8 * 4 + 2 * 4
+    assert ctypes.sizeof(binding.dc_stats) == 27 * 8 + 3 * 8 + 8 * 4 + 8 * 4 + 4 * 4
 
 
 def test_null_arguments_are_rejected_without_a_gpu(lib):
