@@ -60,6 +60,7 @@ __global__ void k_far_pyramid(const int *__restrict__ cell_start, unsigned char 
 struct FarLane {
     float lo[3], hi[3];     // the element box in units of cells relative to the grid origin (from the doubles), rounded outward
     float cen[3], half[3];  // a centre and half-edges that hold the box about it (rounded up)
+    float glo[3], ghi[3];   // the box grown by what a face may overhang its cell (faces are binned by box centre: at most fhalf)
     bool on;
 };
 
@@ -67,12 +68,14 @@ __device__ __forceinline__ FarLane far_lane(const DcScalars *S, const double *__
 {
     FarLane q; q.on = on;
     const double inv = S->inv_cell;
+    const float infl = __double2float_ru(S->fhalf * S->inv_cell + 1e-6);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         q.lo[c] = on ? __double2float_rd((ebox[(size_t)c * n_elem + e] - S->origin[c]) * inv - 1e-9) : 0.f;
         q.hi[c] = on ? __double2float_ru((ebox[(size_t)(3 + c) * n_elem + e] - S->origin[c]) * inv + 1e-9) : 0.f;
         q.cen[c] = 0.5f * (q.lo[c] + q.hi[c]);
         q.half[c] = fmaxf(__fsub_ru(q.hi[c], q.cen[c]), __fsub_ru(q.cen[c], q.lo[c]));
+        q.glo[c] = __fsub_rd(q.lo[c], infl); q.ghi[c] = __fadd_ru(q.hi[c], infl);
     }
     return q;
 }
@@ -90,28 +93,19 @@ __device__ __forceinline__ float warp_max_f(float v) {
     return v;
 }
 
-// the box of the warp's elements, grown by what a face may overhang its cell (faces are binned by box centre: at most
-// fhalf) and rounded outward
-struct FarGroup { float lo[3], hi[3], cen[3]; };
+// the centre of the warp's elements (the octant order of the nearest-first walk)
+struct FarGroup { float cen[3]; };
 
-__device__ __forceinline__ FarGroup far_group(const DcScalars *S, const FarLane &q)
+__device__ __forceinline__ FarGroup far_group(const FarLane &q)
 {
     FarGroup g;
-    const float infl = __double2float_ru(S->fhalf * S->inv_cell + 1e-6);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        g.lo[c] = __fsub_rd(warp_min_f(q.on ? q.lo[c] : INFINITY), infl);
-        g.hi[c] = __fadd_ru(warp_max_f(q.on ? q.hi[c] : -INFINITY), infl);
-        g.cen[c] = 0.5f * (g.lo[c] + g.hi[c]);
-    }
+    for (int c = 0; c < 3; ++c) g.cen[c] = 0.5f * (warp_min_f(q.on ? q.lo[c] : INFINITY) + warp_max_f(q.on ? q.hi[c] : -INFINITY));
     return g;
 }
-// the group's cutoff for the cubes from the largest of its lanes' squared cutoffs (+ a hair: a lane's own nearest cube
-// must not be lost to the rounding of two distances against each other)
-__device__ __forceinline__ float far_group_cut(float lane_cut2) { return warp_max_f(lane_cut2) * 1.0001f + 1e-6f; }
 
-// squared distance (cell units, never overestimated) between the group's grown box and the cube (x, y, z) of level L
-__device__ __forceinline__ float far_lb2(const FarGroup &g, int L, int x, int y, int z)
+// squared distance (cell units, never overestimated) between the lane's grown box and the cube (x, y, z) of level L
+__device__ __forceinline__ float far_lb2(const FarLane &q, int L, int x, int y, int z)
 {
     const float s = (float)(1 << L);
     const int xi[3] = { x, y, z };
@@ -119,7 +113,7 @@ __device__ __forceinline__ float far_lb2(const FarGroup &g, int L, int x, int y,
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const float nlo = (float)xi[c] * s, nhi = nlo + s;            // (exact)
-        const float gp = fmaxf(0.f, fmaxf(__fsub_rd(nlo, g.hi[c]), __fsub_rd(g.lo[c], nhi)));
+        const float gp = fmaxf(0.f, fmaxf(__fsub_rd(nlo, q.ghi[c]), __fsub_rd(q.glo[c], nhi)));
         d2 = __fadd_rd(d2, __fmul_rd(gp, gp));
     }
     return d2;
@@ -156,11 +150,15 @@ __device__ __forceinline__ float far_dir_lb(const FarLane &q, float cx, float cy
     return D - se - sf - 1e-5f * (D + se + sf) - 1e-4f;
 }
 
-// Depth-first walk, uniform over the warp, of the cubes that hold faces and whose box is within cut2 (cell units) of
-// the group's box; cell(p0, p1) is called (by all lanes) for every such cell with the range of its faces and returns the
-// cutoff to go on with.  ORDERED: nearest octant first, strict test (a cube no nearer than the cutoff is skipped).
+// Depth-first walk, uniform over the warp, of the cubes that hold faces and are within the cutoff of AT LEAST ONE lane
+// (each lane tests the cube against its own box and its own squared cutoff cut2, cell units; one vote): the cubes walked
+// are the union of what the 32 elements would walk alone.  cell(p0, p1) is called (by all lanes) for every such cell with
+// the range of its faces; it returns true (uniformly) to end the walk, and may switch lanes off (q.on).  ORDERED: nearest
+// octant first, strict test, and the lanes' cutoffs may shrink on the way.
+// (Fetching for 32 cubes at a time, lane by lane, with the face records prefetched into L1, was tried: no gain -- a step
+// costs what its hundred dependent instructions cost a lone warp, not its loads; the throughput comes from the warps.)
 template <bool ORDERED, class F>
-__device__ __forceinline__ void far_walk(const FarGroup &g, float cut2, const int *__restrict__ cell_start,
+__device__ __forceinline__ void far_walk(const FarLane &q, const FarGroup &g, const float &cut2, const int *__restrict__ cell_start,
                                          const unsigned char *__restrict__ pmask, unsigned *stack, F &&cell)
 {
     int top = 0;
@@ -168,10 +166,10 @@ __device__ __forceinline__ void far_walk(const FarGroup &g, float cut2, const in
     while (top > 0) {
         const unsigned nd = stack[--top];
         const int L = (int)(nd >> 18), x = (int)(nd & 63u), y = (int)((nd >> 6) & 63u), z = (int)((nd >> 12) & 63u);
-        if (ORDERED && !(far_lb2(g, L, x, y, z) < cut2)) continue;          // (the cutoff has shrunk since the push)
+        if (ORDERED && !__any_sync(0xffffffffu, q.on && far_lb2(q, L, x, y, z) < cut2)) continue;   // (the cutoffs have shrunk since the push)
         if (L == 0) {
             const int c = cell_code(x, y, z);
-            cut2 = cell(__ldg(cell_start + c), __ldg(cell_start + c + 1));
+            if (cell(__ldg(cell_start + c), __ldg(cell_start + c + 1))) break;      // (the caller has seen enough)
             continue;
         }
         const unsigned mask = __ldg(pmask + pyr_off(L) + x + (DC_GRID_MAX >> L) * (y + (DC_GRID_MAX >> L) * z));
@@ -184,8 +182,8 @@ __device__ __forceinline__ void far_walk(const FarGroup &g, float cut2, const in
             const int k = ORDERED ? (j ^ oct) : j;
             if (!((mask >> k) & 1u)) continue;
             const int cx = 2 * x + (k & 1), cy = 2 * y + ((k >> 1) & 1), cz = 2 * z + (k >> 2);
-            const float lb2 = far_lb2(g, L - 1, cx, cy, cz);
-            if (ORDERED ? !(lb2 < cut2) : !(lb2 <= cut2)) continue;
+            const float lb2 = far_lb2(q, L - 1, cx, cy, cz);
+            if (!__any_sync(0xffffffffu, q.on && (ORDERED ? lb2 < cut2 : lb2 <= cut2))) continue;
             if (top < DC_FAR_STACK) stack[top++] = ((unsigned)(L - 1) << 18) | ((unsigned)cz << 12) | ((unsigned)cy << 6) | (unsigned)cx;
         }
     }
@@ -301,7 +299,15 @@ __global__ void k_far_sort(const DcScalars *S, const int *__restrict__ list, con
 
 // every far element at once: the face with the nearest box (one warp per 32 elements of the list)
 #define FAR_WARPS 4
-__global__ void __launch_bounds__(FAR_WARPS * 32) k_far_nearest(const DcScalars *S, const int *__restrict__ list, int n,
+#define FAR_NEAREST_CAP 1024        /* faces a warp looks at for its 32 seeds */
+#ifndef FAR_HEAVY
+#define FAR_HEAVY 128               /* candidates beyond which an element leaves the walk for the brute-force kernels */
+#endif
+#ifndef FAR_WARP_CAP
+#define FAR_WARP_CAP 2048           /* faces a warp may visit before the elements it still walks for leave too */
+#endif
+#define FAR_HEAVY_BIT (1 << 30)
+__global__ void __launch_bounds__(FAR_WARPS * 32) k_far_nearest(DcScalars *S, const int *__restrict__ list, int n,
                                                                 const double *__restrict__ ebox, long long n_elem,
                                                                 const int *__restrict__ cell_start, const unsigned char *__restrict__ pmask,
                                                                 const float *__restrict__ ffar, int *__restrict__ fstar)
@@ -311,16 +317,21 @@ __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_nearest(const DcScalars 
     if ((i & ~31) >= n) return;                         // (whole warps only)
     const bool on = i < n;
     const FarLane q = far_lane(S, ebox, n_elem, on ? list[i] : 0, on);
-    const FarGroup g = far_group(S, q);
+    const FarGroup g = far_group(q);
     float best = on ? INFINITY : 0.f;                   // squared box distance of the nearest face box so far
+    float cut2 = best;                                  // (+ a hair: a lane's nearest cube must not be lost to rounding)
     int f = 0;
-    far_walk<true>(g, INFINITY, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
+    // (the seed only has to be near: where every face is about as near as the next one -- deep inside a round body -- the
+    // walk would visit them all; the nearest octant comes first, so what FAR_NEAREST_CAP faces have shown is near enough)
+    int seen = 0;
+    far_walk<true>(q, g, cut2, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
         for (int p = p0; p < p1; ++p) {
             const float4 *fp = reinterpret_cast<const float4 *>(ffar) + (size_t)p * 4;
             const float d2 = far_box_d2(q, __ldg(fp), __ldg(fp + 1));
-            if (d2 < best) { best = d2; f = p; }
+            if (d2 < best) { best = d2; f = p; cut2 = best * 1.0001f + 1e-6f; }
         }
-        return far_group_cut(best);
+        seen += p1 - p0;
+        return seen >= FAR_NEAREST_CAP;
     });
     if (on) fstar[i] = f;
 }
@@ -335,6 +346,8 @@ __global__ void k_far_reset(DcScalars *S, int m, int first)
     for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; S->nh[i] = 0; }
     S->nh[DC_NQN] = 0;
     S->far_chunk_done = 0;
+    if (first) S->far_nheavy = 0;
+    S->far_nheavy_pass = 0;
 }
 
 __global__ void k_far_slots(const int *__restrict__ list, const int *__restrict__ fstar, int m,
@@ -363,25 +376,97 @@ __device__ __forceinline__ bool far_hit(const FarLane &q, float cutf, float cut2
     return far_dir_lb(q, blo.w, bhi.w, ax.w, ax, __ldg(fp + 3)) <= cutf;
 }
 
-__global__ void __launch_bounds__(FAR_WARPS * 32) k_far_count(const DcScalars *S, const double *__restrict__ ebox, long long n_elem,
+__global__ void __launch_bounds__(FAR_WARPS * 32) k_far_count(DcScalars *S, const double *__restrict__ ebox, long long n_elem,
                                                               const int *__restrict__ cell_start, const unsigned char *__restrict__ pmask,
                                                               const float *__restrict__ ffar, const int *__restrict__ band_elem,
-                                                              int *__restrict__ band_cnt, const unsigned long long *__restrict__ best)
+                                                              int *__restrict__ band_cnt, const unsigned long long *__restrict__ best,
+                                                              int *__restrict__ heavy_list)
 {
     __shared__ unsigned s_stack[FAR_WARPS][DC_FAR_STACK];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, n = S->n_band;
     if ((i & ~31) >= n) return;
     const bool on = i < n;
-    const FarLane q = far_lane(S, ebox, n_elem, on ? band_elem[i] : 0, on);
-    const FarGroup g = far_group(S, q);
+    FarLane q = far_lane(S, ebox, n_elem, on ? band_elem[i] : 0, on);
+    const FarGroup g = far_group(q);
     const float cutf = on ? far_cut(S, u2d(best[i]) + S->t_tie) : 0.f, cut2f = __fmul_ru(cutf, cutf);
-    const float cutg = far_group_cut(cut2f);
+    const float cutg = cut2f * 1.0001f + 1e-6f;        // (for the cubes: + a hair against the rounding of two distances)
     int cnt = 0;
-    far_walk<false>(g, cutg, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
-        for (int p = p0; p < p1; ++p) if (on && far_hit(q, cutf, cut2f, ffar, p)) ++cnt;
-        return cutg;
+    // An element with more than FAR_HEAVY candidates (deep inside a round body every face is about as near as the next
+    // one) leaves the walk -- it would drag its whole warp over most of the surface -- and is counted, and later listed,
+    // by the brute-force kernels below, a CTA per element over all faces.  So do the elements a warp is still walking
+    // for after FAR_WARP_CAP faces: a pass lasts as long as its slowest warp.
+    int seen = 0;
+    far_walk<false>(q, g, cutg, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
+        for (int p = p0; p < p1; ++p) if (q.on && far_hit(q, cutf, cut2f, ffar, p) && ++cnt > FAR_HEAVY) q.on = false;
+        seen += p1 - p0;
+        if (seen > FAR_WARP_CAP && q.on) { cnt = FAR_HEAVY + 1; q.on = false; }
+        return !__any_sync(0xffffffffu, q.on);
     });
-    if (on) band_cnt[i] = cnt;
+    if (on) {
+        const bool heavy = cnt > FAR_HEAVY;
+        band_cnt[i] = heavy ? FAR_HEAVY_BIT : cnt;
+        if (heavy) heavy_list[atomicAdd(&S->far_nheavy, 1)] = i;
+    }
+}
+
+// brute force for the heavy elements: a CTA per element, a thread per face
+#define FAR_HEAVY_THREADS 256
+__global__ void __launch_bounds__(FAR_HEAVY_THREADS) k_far_heavy_count(const DcScalars *S, const double *__restrict__ ebox, long long n_elem,
+                                                                       const float *__restrict__ ffar, const int *__restrict__ band_elem,
+                                                                       int *__restrict__ band_cnt, const unsigned long long *__restrict__ best,
+                                                                       const int *__restrict__ heavy_list)
+{
+    __shared__ int s_warp[FAR_HEAVY_THREADS / 32];
+    const int nh = S->far_nheavy, nf = S->n_face;
+    for (int h = blockIdx.x; h < nh; h += gridDim.x) {
+        const int i = heavy_list[h];
+        const FarLane q = far_lane(S, ebox, n_elem, band_elem[i], true);
+        const float cutf = far_cut(S, u2d(best[i]) + S->t_tie), cut2f = __fmul_ru(cutf, cutf);
+        int cnt = 0;
+        for (int p = threadIdx.x; p < nf; p += FAR_HEAVY_THREADS) cnt += far_hit(q, cutf, cut2f, ffar, p) ? 1 : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = cnt;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int t = 0;
+            for (int w = 0; w < FAR_HEAVY_THREADS / 32; ++w) t += s_warp[w];
+            band_cnt[i] = t | FAR_HEAVY_BIT;
+        }
+        __syncthreads();
+    }
+}
+// ... and the pairs of the heavy elements that got their slots in this pass (k_far_pairs lists them): faces in order
+__global__ void __launch_bounds__(FAR_HEAVY_THREADS) k_far_heavy_pairs(const DcScalars *S, const double *__restrict__ ebox, long long n_elem,
+                                                                       const float *__restrict__ ffar, const int *__restrict__ band_elem,
+                                                                       const long long *__restrict__ band_start,
+                                                                       const unsigned long long *__restrict__ best,
+                                                                       const int *__restrict__ pass_list,
+                                                                       int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key,
+                                                                       int *__restrict__ pair_band)
+{
+    __shared__ int s_warp[FAR_HEAVY_THREADS / 32];
+    const int nh = S->far_nheavy_pass, nf = S->n_face;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int h = blockIdx.x; h < nh; h += gridDim.x) {
+        const int i = pass_list[h];
+        const FarLane q = far_lane(S, ebox, n_elem, band_elem[i], true);
+        const float cutf = far_cut(S, u2d(best[i]) + S->t_tie), cut2f = __fmul_ru(cutf, cutf);
+        long long j = band_start[i];
+        for (int p0 = 0; p0 < nf; p0 += FAR_HEAVY_THREADS) {
+            const int p = p0 + threadIdx.x;
+            const bool hit = p < nf && far_hit(q, cutf, cut2f, ffar, p);
+            const unsigned hm = __ballot_sync(0xffffffffu, hit);
+            if (lane == 0) s_warp[wid] = __popc(hm);
+            __syncthreads();
+            int before = 0, total = 0;
+#pragma unroll
+            for (int w = 0; w < FAR_HEAVY_THREADS / 32; ++w) { const int v = s_warp[w]; if (w < wid) before += v; total += v; }
+            if (hit) { const long long w = j + before + __popc(hm & ((1u << lane) - 1u)); pair_face[w] = p; pair_key[w] = 0x7ff0000000000000ull; pair_band[w] = i; }
+            j += total;
+            __syncthreads();
+        }
+    }
 }
 
 // One pass: every waiting element (band_cnt > 0) asks for its pair slots at ONE counter that is never wound back -- the
@@ -395,33 +480,70 @@ __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_pairs(DcScalars *S, cons
                                                               long long *__restrict__ band_start, const int *__restrict__ band_cnt,
                                                               int *__restrict__ pair_face, unsigned long long *__restrict__ pair_key,
                                                               int *__restrict__ pair_band, const unsigned long long *__restrict__ best,
-                                                              long long cap_pairs)
+                                                              long long cap_pairs, int *__restrict__ pass_list)
 {
     __shared__ unsigned s_stack[FAR_WARPS][DC_FAR_STACK];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, n = S->n_band;
     if ((i & ~31) >= n) return;
-    const int cnt = i < n ? band_cnt[i] : 0;          // (<= 0: done in an earlier pass, or nothing)
-    bool on = false;
-    long long j = 0;
-    if (cnt > cap_pairs) atomicMax(&S->far_want, (unsigned long long)cnt);
-    else if (cnt > 0) {
-        const unsigned long long old = atomicAdd(&S->n_pairs, (unsigned long long)cnt);
-        if (old + (unsigned long long)cnt <= (unsigned long long)cap_pairs) {
-            atomicMax(&S->far_end, old + (unsigned long long)cnt);
-            band_start[i] = (long long)old;
-            j = (long long)old; on = true;
-        }
+    const int raw = i < n ? band_cnt[i] : -1;         // (-1: done in an earlier pass)
+    bool heavy = raw >= 0 && (raw & FAR_HEAVY_BIT) != 0;
+    int cnt = raw >= 0 ? (raw & ~FAR_HEAVY_BIT) : 0;
+    if (cnt > cap_pairs) { atomicMax(&S->far_want, (unsigned long long)cnt); cnt = 0; }
+    // the warp asks for the slots of all its waiting lanes at once, all or nothing: the lanes of a pass are whole warps
+    // (a walk costs the same for one lane as for 32), and the counter sees one atomic per warp.  The warp's range holds
+    // first the pairs of its light lanes, in the order the walk meets them, then a range per heavy lane.
+    const int lane = threadIdx.x & 31;
+    int incl_h = heavy ? cnt : 0, light = heavy ? 0 : cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl_h, o); if (lane >= o) incl_h += v; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) light += __shfl_xor_sync(0xffffffffu, light, o);
+    const int total = light + __shfl_sync(0xffffffffu, incl_h, 31);
+    if (total == 0) return;
+    unsigned long long old = 0;
+    if (lane == 0) {
+        old = total <= cap_pairs ? atomicAdd(&S->n_pairs, (unsigned long long)total) : ~0ull;
+        if (old != ~0ull && old + (unsigned long long)total > (unsigned long long)cap_pairs) old = ~0ull;
+        if (old != ~0ull) atomicMax(&S->far_end, old + (unsigned long long)total);
     }
+    old = __shfl_sync(0xffffffffu, old, 0);
+    long long hbase = 0;
+    if (old == ~0ull) {
+        // (a warp whose lanes together exceed a pass, though none does alone: one lane per pass, the first that waits)
+        if (total <= cap_pairs) return;
+        const unsigned waiting = __ballot_sync(0xffffffffu, cnt > 0);
+        const int leader = __ffs(waiting) - 1;
+        if (lane == leader) {
+            old = atomicAdd(&S->n_pairs, (unsigned long long)cnt);
+            if (old + (unsigned long long)cnt > (unsigned long long)cap_pairs) old = ~0ull;
+            else atomicMax(&S->far_end, old + (unsigned long long)cnt);
+        } else cnt = 0;
+        old = __shfl_sync(0xffffffffu, old, leader);
+        if (old == ~0ull) return;
+        hbase = (long long)old;
+    } else hbase = (long long)old + light + incl_h - cnt;
+    if (cnt == 0) heavy = false;
+    if (heavy) { band_start[i] = hbase; pass_list[atomicAdd(&S->far_nheavy_pass, 1)] = i; }
+    const bool on = cnt > 0 && !heavy;
+    if (on) band_start[i] = (long long)old;           // (>= 0: this element's pairs are in the list of this pass)
     if (!__any_sync(0xffffffffu, on)) return;
     const FarLane q = far_lane(S, ebox, n_elem, on ? band_elem[i] : 0, on);
-    const FarGroup g = far_group(S, q);
+    const FarGroup g = far_group(q);
     // (best[i] has not moved since k_far_count: same candidates)
     const float cutf = on ? far_cut(S, u2d(best[i]) + S->t_tie) : 0.f, cut2f = __fmul_ru(cutf, cutf);
-    const float cutg = far_group_cut(cut2f);
-    far_walk<false>(g, cutg, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
-        for (int p = p0; p < p1; ++p)
-            if (on && far_hit(q, cutf, cut2f, ffar, p)) { pair_face[j] = p; pair_key[j] = 0x7ff0000000000000ull; pair_band[j] = i; ++j; }
-        return cutg;
+    const float cutg = cut2f * 1.0001f + 1e-6f;
+    // the warp's pairs fill its range in the order the walk meets them: the lanes that hit a face write neighbouring
+    // entries (the narrow phase goes by pair_band, not by ranges per element)
+    long long j = (long long)old;
+    const unsigned lt = (1u << (threadIdx.x & 31)) - 1u;
+    far_walk<false>(q, g, cutg, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
+        for (int p = p0; p < p1; ++p) {
+            const bool hit = on && far_hit(q, cutf, cut2f, ffar, p);
+            const unsigned hm = __ballot_sync(0xffffffffu, hit);
+            if (hit) { const long long w = j + __popc(hm & lt); pair_face[w] = p; pair_key[w] = 0x7ff0000000000000ull; pair_band[w] = i; }
+            j += __popc(hm);
+        }
+        return false;
     });
 }
 

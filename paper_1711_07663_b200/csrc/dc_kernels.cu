@@ -73,6 +73,7 @@ struct DcScalars {
     // DC_FLAG_EXACT_FAR (dc_far.cuh): the two lists of far elements still to do (ping-pong), the chunk's and the pass's tallies
     int far_n[2];
     int far_chunk_done, far_done, far_unresolved, far_pad;
+    int far_nheavy, far_nheavy_pass;   // heavy elements of the slice / of those, the ones served in this pass
     unsigned long long far_end;         // end of the pair slots handed out in this chunk
     unsigned long long far_want;        // most candidates a deferred element asked for
     unsigned long long far_pairs_total;
@@ -987,6 +988,7 @@ struct dc_ctx {
     int *pyr;                 // octree over the face bins (DC_FLAG_EXACT_FAR)
     float *ffar;              // [max_faces][16]: per-face records of the far pass
     int *far_sorted, *far_bins;   // the far elements in Morton order; the bins of the counting sort that makes it
+    int *far_heavy;               // [n_elem]: the heavy elements served in a pass (the slice's are listed in act_elem)
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
     cudaEvent_t ev[14], evk[10];    // evk: boundaries between the kernels of S5/S6
     cudaStream_t last_stream;
@@ -1004,7 +1006,7 @@ struct WsLayout {
     size_t off_S, off_ebox, off_adj, off_parent, off_comp, off_tile_flag, off_act_elem, off_band_elem, off_band_start, off_band_cnt,
         off_ecoef, off_pbox, off_best, off_dmin, off_q0, off_q1, off_nq, off_nqx,
         off_pair_face, off_pair_key, off_pair_band, off_fbox_orig, off_fbox, off_fboxf, off_fcoef, off_fcell, off_fperm,
-        off_cell_count, off_cell_start, off_cell_fill, off_occ, off_pyr, off_ffar, off_far_sorted, off_far_bins, off_hfaces, off_hlabels, off_hsdist, total;
+        off_cell_count, off_cell_start, off_cell_fill, off_occ, off_pyr, off_ffar, off_far_sorted, off_far_bins, off_far_heavy, off_hfaces, off_hlabels, off_hsdist, total;
     long long max_band, qcap;
 };
 
@@ -1060,6 +1062,7 @@ static WsLayout ws_layout(long long n_nodes, long long n_elem, long long max_fac
     L.off_pyr = take((size_t)DC_PYR_TOTAL * 4);
     L.off_ffar = take((size_t)max_faces * 16 * 4);
     L.off_far_sorted = take((size_t)n_elem * 4);
+    L.off_far_heavy = take((size_t)n_elem * 4);
     L.off_far_bins = take((size_t)(3 * (DC_NCELL + 8) + SCAN_NCHUNK) * 4);
     L.off_hfaces = take((size_t)max_faces * 27 * 8);
     L.off_hlabels = take((size_t)n_elem);
@@ -1135,6 +1138,7 @@ static int create_grid_body(dc_ctx *c, int num_sms, int device, long long n_node
     c->pyr = (int *)(c->ws + L.off_pyr);
     c->ffar = (float *)(c->ws + L.off_ffar);
     c->far_sorted = (int *)(c->ws + L.off_far_sorted);
+    c->far_heavy = (int *)(c->ws + L.off_far_heavy);
     c->far_bins = (int *)(c->ws + L.off_far_bins);
     c->h_faces_dev = (double *)(c->ws + L.off_hfaces);
     c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
@@ -1322,12 +1326,15 @@ static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_d
         k_far_slots<<<nblk(m, 256), 256, 0, st>>>(list + s0, fstar + s0, (int)m, c->band_elem, c->band_start, c->band_cnt, c->pair_face,
                                                    c->pair_key, c->pair_band, c->nq, c->best, c->dmin);
         { const int rc = launch_narrow(c, st, rounds, grid_rounds, 1); if (rc) return rc; }
-        k_far_count<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_cnt, c->best);
+        k_far_count<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_cnt, c->best, c->act_elem);
+        k_far_heavy_count<<<c->num_sms * 4, FAR_HEAVY_THREADS, 0, st>>>(S, c->ebox, ne, c->ffar, c->band_elem, c->band_cnt, c->best, c->act_elem);
         long long pending = m;
         while (pending > 0 && !c->far_error) {
             k_far_reset<<<1, 1, 0, st>>>(S, (int)m, 0);
             k_far_pairs<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_start, c->band_cnt,
-                                                       c->pair_face, c->pair_key, c->pair_band, c->best, cap);
+                                                       c->pair_face, c->pair_key, c->pair_band, c->best, cap, c->far_heavy);
+            k_far_heavy_pairs<<<c->num_sms * 4, FAR_HEAVY_THREADS, 0, st>>>(S, c->ebox, ne, c->ffar, c->band_elem, c->band_start, c->best, c->far_heavy,
+                                                                             c->pair_face, c->pair_key, c->pair_band);
             k_far_fix<<<1, 1, 0, st>>>(S);
             { const int rc = launch_narrow(c, st, rounds, grid_rounds, 2); if (rc) return rc; }
             k_far_decide<<<nblk(m, 256), 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->dmin, labels_dev, sdist_dev);
