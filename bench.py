@@ -24,6 +24,8 @@ nodes + connectivity + adjacency, surface faces) are resident in HBM before the 
             uniform sample of the same workload's elements, each against ALL faces; `value` counts the SAME
             candidate pairs as the GPU line (those of the sampled elements), per oracle second.
   paper_mode: the paper's own approximate cut (DC_FLAG_PAPER_MODE) on the same context: ms, labels differing from the exact mode.
+  exact_far: DC_FLAG_EXACT_FAR on the same context (exact distance beyond the band too, "d_band = infinity"): ms of the far pass,
+            far elements, candidate pairs, passes.
   donor_search: the paper's other GPU algorithm (4.3: ADT stack search + Newton point containment), 1 M points.
   per_config: the other BASELINE.json configs (0, 1, 3 incl. the sum over its 32 steps, 4), a few seconds each,
             every one with its own clock record over a timed region of at least 200 ms.
@@ -359,6 +361,38 @@ def measure_paper_mode(dcut, faces, B, stream, torch, np, n_cuts: int = 10):
     return out
 
 
+def measure_exact_far(dcut, faces, B, stream, torch, np, n_cuts: int = 3):
+    """SURVEY.md 8(f) NEXT-4 (second half): DC_FLAG_EXACT_FAR on the same context -- the banded cut, then the exact distance
+    of every element it left clamped.  Wall clock of the far pass (it synchronises after each of its passes), its
+    element and pair counts, and that the labels and the band's distances are those of the banded cut."""
+    p_band = B.dc_params(); p_band.flags = B.DC_FLAG_RECOMPUTE_BOXES
+    p_far = B.dc_params(); p_far.flags = B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_EXACT_FAR
+    dcut.set_cut_surface(faces); dcut.classify(p_band)
+    lab0 = dcut.labels.clone(); sd0 = dcut.sdist.clone()
+    st0 = dcut.stats()
+    ms_far, ms_all = [], []
+    for i in range(n_cuts + 1):
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        dcut.set_cut_surface(faces); dcut.classify(p_far)
+        torch.cuda.synchronize(); t1 = time.perf_counter()
+        st = dcut.stats()
+        if i:
+            ms_far.append(float(st.ms_far)); ms_all.append((t1 - t0) * 1e3)
+    lab1, sd1 = dcut.labels, dcut.sdist
+    inband = sd0.abs() < st0.d_band
+    out = {"ms_far_pass": statistics.median(ms_far), "ms_full_cut_with_far_pass_wall": statistics.median(ms_all),
+           "ms_banded_cut": float(st0.ms_stage[5]) + float(st0.ms_stage[0]),
+           "far_elements": int(st.n_far), "far_elements_done": int(st.n_far_done), "far_pairs": int(st.far_pairs),
+           "passes": int(st.far_passes), "max_pairs": int(dcut.max_pairs),
+           "far_elements_per_s": st.n_far / (statistics.median(ms_far) * 1e-3) if st.n_far else 0.0,
+           "labels_equal_banded": bool((lab1 == lab0).all().item()),
+           "band_sdist_equal_banded": bool((sd1[inband] == sd0[inband]).all().item()),
+           "min_abs_far_sdist_over_d_band": float((sd1[~inband & (lab1 != 2)].abs().min().item() / st0.d_band)) if bool((~inband & (lab1 != 2)).any().item()) else None,
+           "max_abs_sdist": float(sd1.abs().max().item())}
+    dcut.set_cut_surface(faces); dcut.classify(p_band)
+    return out
+
+
 def measure_other_config(cfg: int, B, local_rank: int, torch, np, min_ms: float = 200.0):
     """One of the other BASELINE.json configs: full cut and re-cut, each over a timed region of at least `min_ms` with its
     own clock record; config 3: every one of its 32 steps and their sum (re-cut path: the grid is fixed)."""
@@ -403,6 +437,7 @@ def measure_other_config(cfg: int, B, local_rank: int, torch, np, min_ms: float 
                          "ms_sum_32_steps_step1_full": float(per_step[1:].sum() + first_full)}
     if cfg != 3:
         out["paper_mode"] = measure_paper_mode(dcut, face_sets[0], B, stream, torch, np)
+        out["exact_far"] = measure_exact_far(dcut, face_sets[0], B, stream, torch, np)
     dcut.close()
     del dcut, face_sets
     torch.cuda.empty_cache()
@@ -630,6 +665,7 @@ def main():
                                                      "max_abs_dsdist_over_lref": err / ref.stats["l_ref"]}}
     if rank == 0 and world == 1 and cfg != 3 and not args.no_per_config:
         line["paper_mode"] = measure_paper_mode(dcut, face_sets[0], B, stream, torch, np)
+        line["exact_far"] = measure_exact_far(dcut, face_sets[0], B, stream, torch, np)
         # the paper's other GPU algorithm (4.3): ADT stack search + Newton point containment, 1 M query points
         t0 = time.perf_counter(); dcut.build_adt(); t_build = time.perf_counter() - t0
         q = (torch.rand((1 << 20, 3), dtype=torch.float64, device="cuda:%d" % local_rank) * 1.9 - 0.95)

@@ -90,8 +90,9 @@ extern "C" {
                                        faces whose box is within an attained upper bound of the element (nearest-bin walk
                                        over an octree of the face bins, so no N_e x N_f pair list), the sign from S7.  Labels
                                        are unchanged.  Runs in passes sized to the workspace and SYNCHRONISES the stream
-                                       after each; dc_get_pairs is not available afterwards.  Costs about 20-40 x the banded
-                                       cut on the configs of BASELINE.json.  Ignored with DC_FLAG_PAPER_MODE.
+                                       after each; dc_get_pairs is not available afterwards.  Costs tens of banded cuts
+                                       (most elements are far, and far from a round body a hundred
+                                       faces are about as near as the nearest).  Ignored with DC_FLAG_PAPER_MODE.
                                        A pass holds max_pairs / 6 pairs: DC_ERR_WORKSPACE (dc_get_stats) when ONE element
                                        has more candidate faces than that (pairs_needed says what max_pairs would do). */
 
@@ -131,7 +132,7 @@ typedef struct {
     long long n_far_done;        /* ... of which got their exact distance (= n_far unless the pass failed) */
     long long n_far_unresolved;  /* ... and for which the narrow phase solved no leaf (0; they keep the clamp) */
     long long far_pairs;         /* candidate pairs of the far pass, all chunks */
-    long long far_chunks;        /* passes the far pass ran in (each ends with a stream synchronisation) */
+    long long far_passes;        /* passes the far pass ran in (each ends with a stream synchronisation) */
     double l_ref, tau_cut, d_band;
     float ms_stage[8];           /* 0 S1+S3 faces/bins, 1 S2 boxes, 2 S4 pairs, 3 S5+S6 narrow,
                                     4 S7 fill, 5 total dc_classify, 6 dc_set_cut_surface,

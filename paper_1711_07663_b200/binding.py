@@ -44,7 +44,7 @@ class dc_stats(C.Structure):
                 ("pairs_needed", C.c_longlong), ("queue_peak", C.c_longlong),
                 ("n_root_nodes", C.c_longlong), ("band_needed", C.c_longlong), ("queue_needed", C.c_longlong),
                 ("n_far", C.c_longlong), ("n_far_done", C.c_longlong), ("n_far_unresolved", C.c_longlong),
-                ("far_pairs", C.c_longlong), ("far_chunks", C.c_longlong),
+                ("far_pairs", C.c_longlong), ("far_passes", C.c_longlong),
                 ("l_ref", C.c_double), ("tau_cut", C.c_double), ("d_band", C.c_double),
                 ("ms_stage", C.c_float * 8), ("ms_kernel", C.c_float * 8), ("status", C.c_int), ("n_launches", C.c_int),
                 ("ms_far", C.c_float), ("reserved", C.c_int)]

@@ -17,9 +17,19 @@
 //
 // The candidate pairs then go through the SAME narrow phase as the band's (k_np_roots, k_np_bound, k_np_solve: nothing
 // is pruned below the true minimum because best[] starts at the attained ub, not at the band's reach), and k_far_decide
-// writes sdist = +-d_e with the sign the flood fill gave.  Far elements have many more candidates than band elements
-// (on a sphere every face is about as near as the next one), so the pairs are made and solved in PASSES sized to the
-// workspace: an element whose candidates no longer fit waits for the next pass.  The host reads two counters per pass.
+// writes sdist = +-d_e with the sign the flood fill gave.
+//
+// Far elements have many more candidates than band elements (far from a round body a hundred faces are about as near as
+// the nearest), so the pairs are made and solved in PASSES sized to the workspace: in each pass the warps that still wait
+// ask for the slots of their 32 elements at one counter, all or nothing, until the list is full; the host reads two
+// counters per pass.  Deep inside a round body EVERY face is about as near as the next one: an element with more than
+// FAR_HEAVY candidates, or whose warp has walked past FAR_WARP_CAP faces, leaves the walk and is counted and listed by
+// brute force instead (k_far_heavy_count / k_far_heavy_pairs: a CTA per element, a thread per face) -- a pass lasts as
+// long as its slowest warp.
+//
+// Launch order (run_exact_far): pyramid, faces, list, [codes, scan, sort], nearest; per slice of max_band elements:
+// slots, k_np_stage, k_np_solve(seeds), count, heavy_count; per pass: pairs, heavy_pairs, fix, k_np_roots ... the last
+// k_np_solve, decide.
 #pragma once
 
 #define DC_FAR_STACK 48             /* 7 pushed siblings per level x 6 levels + 1 */
@@ -304,7 +314,7 @@ __global__ void k_far_sort(const DcScalars *S, const int *__restrict__ list, con
 #define FAR_HEAVY 128               /* candidates beyond which an element leaves the walk for the brute-force kernels */
 #endif
 #ifndef FAR_WARP_CAP
-#define FAR_WARP_CAP 2048           /* faces a warp may visit before the elements it still walks for leave too */
+#define FAR_WARP_CAP 1024           /* faces a warp may visit before the elements it still walks for leave too */
 #endif
 #define FAR_HEAVY_BIT (1 << 30)
 __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_nearest(DcScalars *S, const int *__restrict__ list, int n,
@@ -345,7 +355,7 @@ __global__ void k_far_reset(DcScalars *S, int m, int first)
     S->far_end = 0ull;
     for (int i = 0; i < DC_NQN; ++i) { S->qn[i] = 0; S->nn[i] = 0; S->nh[i] = 0; }
     S->nh[DC_NQN] = 0;
-    S->far_chunk_done = 0;
+    S->far_pass_done = 0;
     if (first) S->far_nheavy = 0;
     S->far_nheavy_pass = 0;
 }
@@ -570,7 +580,7 @@ __global__ void k_far_decide(DcScalars *S, const int *__restrict__ band_elem, lo
     }
     const unsigned md = __ballot_sync(0xffffffffu, done), mb = __ballot_sync(0xffffffffu, bad);
     if ((threadIdx.x & 31) == 0) {
-        if (md) { atomicAdd(&S->far_chunk_done, __popc(md)); atomicAdd(&S->far_done, __popc(md)); }
-        if (mb) { atomicAdd(&S->far_chunk_done, __popc(mb)); atomicAdd(&S->far_unresolved, __popc(mb)); }
+        if (md) { atomicAdd(&S->far_pass_done, __popc(md)); atomicAdd(&S->far_done, __popc(md)); }
+        if (mb) { atomicAdd(&S->far_pass_done, __popc(mb)); atomicAdd(&S->far_unresolved, __popc(mb)); }
     }
 }

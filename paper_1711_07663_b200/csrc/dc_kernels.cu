@@ -72,7 +72,7 @@ struct DcScalars {
         c_fill_conflicts, c_queue_peak, c_seedless_total;
     // DC_FLAG_EXACT_FAR (dc_far.cuh): the two lists of far elements still to do (ping-pong), the chunk's and the pass's tallies
     int far_n[2];
-    int far_chunk_done, far_done, far_unresolved, far_pad;
+    int far_pass_done, far_done, far_unresolved, far_pad;
     int far_nheavy, far_nheavy_pass;   // heavy elements of the slice / of those, the ones served in this pass
     unsigned long long far_end;         // end of the pair slots handed out in this chunk
     unsigned long long far_want;        // most candidates a deferred element asked for
@@ -404,7 +404,7 @@ __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
     S->c_box_tests = S->c_bnb_nodes = S->c_newton = S->c_newton_iters = S->c_newton_fail = 0ull;
     S->c_depth_exceeded = S->c_cut = S->c_hole = S->c_normal = S->c_ambiguous = 0ull;
     S->c_sign_ambiguous = S->c_fill_conflicts = S->c_queue_peak = S->c_seedless_total = 0ull;
-    S->far_n[0] = S->far_n[1] = 0; S->far_chunk_done = S->far_done = S->far_unresolved = 0;
+    S->far_n[0] = S->far_n[1] = 0; S->far_pass_done = S->far_done = S->far_unresolved = 0;
     S->far_end = S->far_want = S->far_pairs_total = 0ull;
     for (int c = 0; c < 3; ++c) { S->far_lo[c] = ~0ull; S->far_hi[c] = 0ull; }
 }
@@ -996,7 +996,7 @@ struct dc_ctx {
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
     DcScalars *S_host;        // pinned
     DcScalars *S_band_host;   // pinned: the scalars as the banded cut left them, when a far pass has run since
-    bool far_ran; int far_chunks; long long far_n_total; int far_error;
+    bool far_ran; int far_passes; long long far_n_total; int far_error;
     const AdtNode *adt; int adt_nodes;   // donor search tree (dc_adt_build), caller's memory
 };
 
@@ -1299,7 +1299,7 @@ static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_d
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(c->S_band_host, S, sizeof(DcScalars), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    c->far_ran = true; c->far_chunks = 0; c->far_error = 0;
+    c->far_ran = true; c->far_passes = 0; c->far_error = 0;
     long long n_far = c->S_band_host->far_n[0];
     c->far_n_total = n_far;
     if (c->S_band_host->status & DC_STATUS_INVALID) n_far = 0;       // (the banded cut itself failed: nothing to refine)
@@ -1341,8 +1341,8 @@ static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_d
             CK(cudaGetLastError());
             CK(cudaMemcpyAsync(c->S_host, S, sizeof(DcScalars), cudaMemcpyDeviceToHost, st));
             CK(cudaStreamSynchronize(st));
-            ++c->far_chunks;
-            const int done = c->S_host->far_chunk_done;
+            ++c->far_passes;
+            const int done = c->S_host->far_pass_done;
             if (c->S_host->status & DC_STATUS_INVALID) c->far_error = 1;          // (a queue of the narrow phase overflowed)
             else if (done == 0) c->far_error = 2;                                    // (an element's candidates exceed a pass)
             pending -= done;
@@ -1499,7 +1499,7 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
         const DcScalars &F = *c->S_host;
         S.status |= F.status;
         o->n_far = c->far_n_total; o->n_far_done = F.far_done; o->n_far_unresolved = F.far_unresolved;
-        o->far_pairs = (long long)F.far_pairs_total; o->far_chunks = c->far_chunks;
+        o->far_pairs = (long long)F.far_pairs_total; o->far_passes = c->far_passes;
         if (c->far_error == 2) {            // one element's candidates do not fit a chunk (a third of max_pairs)
             S.status |= DC_STATUS_PAIR_OVERFLOW;
             S.n_pairs = 6ull * (F.far_want + 1ull) + 16ull;

@@ -85,7 +85,7 @@ def test_config1_reduced_exact_everywhere_in_many_chunks(B, nproc):
     labels, sdist, st = exact_cut(B, w)
     check(ref, labels, sdist, st)
     labels2, sdist2, st2 = exact_cut(B, w, max_pairs=32000)
-    assert st2.far_chunks > st.far_chunks and st2.far_chunks >= 3
+    assert st2.far_passes > st.far_passes and st2.far_passes >= 3
     assert np.array_equal(labels2, labels)
     assert np.array_equal(sdist2, sdist)                 # bit for bit: chunk composition must not leak into the values
     assert st2.n_far == st.n_far and st2.far_pairs >= st.n_far
