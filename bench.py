@@ -329,8 +329,7 @@ def time_cuts(dcut, face_sets, params, n_cuts: int, stream, torch):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record(stream)
     for i in range(n_cuts):
-        dcut.set_cut_surface(face_sets[i % len(face_sets)])
-        dcut.classify(params)
+        dcut.cut(face_sets[i % len(face_sets)], params)
     ev1.record(stream)
     torch.cuda.synchronize()
     return ev0.elapsed_time(ev1)
@@ -404,10 +403,10 @@ def measure_other_config(cfg: int, B, local_rank: int, torch, np, min_ms: float 
         face_sets = [torch.from_numpy(w.spin_faces(s)).cuda(local_rank) for s in range(1, 33)]
     else:
         face_sets = [torch.from_numpy(w.faces).cuda(local_rank)]
-    p_full = B.dc_params(); p_full.flags = B.DC_FLAG_RECOMPUTE_BOXES
-    p_recut = B.dc_params()
+    p_full = B.dc_params(); p_full.flags = B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_GRAPH
+    p_recut = B.dc_params(); p_recut.flags = B.DC_FLAG_GRAPH
     for i in range(3):
-        dcut.set_cut_surface(face_sets[i % len(face_sets)]); dcut.classify(p_full)
+        dcut.cut(face_sets[i % len(face_sets)], p_full)
     probe = time_cuts(dcut, face_sets, p_full, len(face_sets), stream, torch) / len(face_sets)
     n = max(len(face_sets), int(np.ceil(min_ms / max(probe, 1e-3))))
     n = ((n + len(face_sets) - 1) // len(face_sets)) * len(face_sets)
@@ -474,6 +473,9 @@ def main():
 
     assert torch.cuda.is_available(), "bench.py needs a B200: there is no CPU fallback"
     torch.cuda.set_device(local_rank)
+    # everything below runs on ONE stream of our own, not the legacy default stream: dc_cut replays the cut's launch
+    # sequence from a CUDA graph (DC_FLAG_GRAPH), and the default stream cannot be captured
+    torch.cuda.set_stream(torch.cuda.Stream(local_rank))
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -486,13 +488,12 @@ def main():
         face_sets = [torch.from_numpy(w.spin_faces(s)).cuda(local_rank) for s in range(1, 33)]
     else:
         face_sets = [torch.from_numpy(w.faces).cuda(local_rank)]
-    p_full = B.dc_params(); p_full.flags = B.DC_FLAG_RECOMPUTE_BOXES
-    p_recut = B.dc_params()
+    p_full = B.dc_params(); p_full.flags = B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_GRAPH
+    p_recut = B.dc_params(); p_recut.flags = B.DC_FLAG_GRAPH
     stream = torch.cuda.current_stream(local_rank)
 
     def step(i, params):
-        dcut.set_cut_surface(face_sets[i % len(face_sets)])
-        dcut.classify(params)
+        dcut.cut(face_sets[i % len(face_sets)], params)
 
     def barrier():
         if world > 1:
@@ -532,14 +533,21 @@ def main():
     # ---- per-stage and per-kernel durations: median over repeated steps (events inside the library)
     reps = max(5, min(args.steps, 20))
     stages, kernels, stages_recut = [], [], []
+    # (plain launches: the library's stage events are left out of the replayed graph)
+    p_full_ev = B.dc_params(); p_full_ev.flags = B.DC_FLAG_RECOMPUTE_BOXES
+    p_recut_ev = B.dc_params()
     for i in range(reps):
-        step(i, p_full); s = dcut.stats(); stages.append(list(s.ms_stage)); kernels.append(list(s.ms_kernel))
+        step(i, p_full_ev); s = dcut.stats(); stages.append(list(s.ms_stage)); kernels.append(list(s.ms_kernel))
     for i in range(reps):
-        step(i, p_recut); s = dcut.stats(); stages_recut.append(list(s.ms_stage))
+        step(i, p_recut_ev); s = dcut.stats(); stages_recut.append(list(s.ms_stage))
     med = np.median(np.array(stages), axis=0)
     medk = np.median(np.array(kernels), axis=0)
     med_recut = np.median(np.array(stages_recut), axis=0)
-    step(0, p_full)
+    n_rc = max(20, len(face_sets))
+    for i in range(len(face_sets)):
+        step(i, p_recut)
+    ms_recut_graph = time_cuts(dcut, face_sets, p_recut, n_rc, stream, torch) / n_rc
+    step(0, p_full_ev)
     s_last = dcut.stats()
 
     # ---- e2e: host buffers through dc_classify_host
@@ -615,7 +623,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "n_elem": w.n_elem, "n_face": w.n_face,
-                       "step": "full cut: dc_set_cut_surface + dc_classify(DC_FLAG_RECOMPUTE_BOXES)",
+                       "step": "full cut: dc_cut = dc_set_cut_surface + dc_classify(DC_FLAG_RECOMPUTE_BOXES); its launch sequence replayed from a CUDA graph (DC_FLAG_GRAPH), every kernel runs every step",
                        "d_band": float(s_last.d_band), "reach": float(s_last.d_band + 2 * s_last.tau_cut + 1e-9 * s_last.l_ref),
                        "unit_note": "a pair test is a candidate pair (boxes within reach): the count is tied to d_band; ms_per_step is not",
                        "l2": "inputs larger than L2 (nodes+conn+adj = %.0f MB)" % ((w.xyz.nbytes + w.conn27.nbytes + w.adj6.nbytes) / 1e6),
@@ -632,7 +640,11 @@ def main():
                     "ms_full_cut_stages": {"S1+S3": float(med[6]), "S2": float(med[1]), "S4": float(med[2]),
                                            "S5+S6": float(med[3]), "S7": float(med[4]), "classify": float(med[5])},
                     "ms_S5_S6_kernels": {n: float(v) for n, v in zip(names_k, medk)},
-                    "ms_recut_cached_boxes": float(med_recut[5] + med_recut[6])}}
+                    "ms_full_cut_plain_launches": float(med[5] + med[6]),
+                    "ms_recut_cached_boxes_plain_launches": float(med_recut[5] + med_recut[6]),
+                    "ms_recut_cached_boxes": float(ms_recut_graph),
+                    "note": "stage and kernel times: plain launches with the library's CUDA events (they are left out of the "
+                            "replayed graph); ms_per_step and ms_recut_cached_boxes: graph replay"}}
 
     # ---- cpu baseline (rank 0, N = 1 only): the oracle on a bounded sample of the same workload
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

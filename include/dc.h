@@ -96,6 +96,16 @@ extern "C" {
                                        A pass holds max_pairs / 6 pairs: DC_ERR_WORKSPACE (dc_get_stats) when ONE element
                                        has more candidate faces than that (pairs_needed says what max_pairs would do). */
 
+#define DC_FLAG_GRAPH 8             /* dc_cut / dc_classify_host only: capture the launch sequence of the cut into a CUDA graph
+                                       the first time it is asked for with these arguments (surface address and face count,
+                                       parameters, output addresses, stream) and replay it afterwards; up to 64 graphs are
+                                       kept per context, the least recently used one goes.  The surface's contents may
+                                       change between calls.  Needs a stream other than the legacy default stream (falls
+                                       back to plain launches there, inside a caller's own capture, and with
+                                       DC_FLAG_EXACT_FAR).  Results and the counters of dc_stats are those of the plain
+                                       launches; the stage times (ms_stage, ms_kernel) are not recorded for a replayed
+                                       cut and read 0. */
+
 typedef struct dc_ctx dc_ctx;
 
 typedef struct {
@@ -190,8 +200,15 @@ int dc_classify(dc_ctx *ctx, const dc_params *params, signed char *labels_dev, d
                 void *stream);
 
 /*
+ * dc_set_cut_surface + dc_classify in one call (same arguments, same results); with DC_FLAG_GRAPH in params->flags the
+ * launch sequence is replayed from a CUDA graph (see the flag).  Asynchronous on `stream` except with DC_FLAG_EXACT_FAR.
+ */
+int dc_cut(dc_ctx *ctx, const dc_params *params, long long n_face, const double *face_nodes_dev,
+           signed char *labels_dev, double *sdist_dev, void *stream);
+
+/*
  * End-to-end variant with HOST buffers: copies the face nodes host->device, runs
- * dc_set_cut_surface + dc_classify, copies labels and sdist device->host, and synchronises
+ * dc_cut (DC_FLAG_GRAPH honoured), copies labels and sdist device->host, and synchronises
  * `stream` before returning.  Host buffers should be pinned.
  */
 int dc_classify_host(dc_ctx *ctx, const dc_params *params, long long n_face,

@@ -20,9 +20,10 @@ DC_STATUS_BAND_OVERFLOW, DC_STATUS_SURFACE_SMALL = 16, 32
 DC_FLAG_RECOMPUTE_BOXES = 1
 DC_FLAG_PAPER_MODE = 2
 DC_FLAG_EXACT_FAR = 4
+DC_FLAG_GRAPH = 8
 DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
 
-EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify",
+EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify", "dc_cut",
            "dc_classify_host", "dc_get_element_boxes", "dc_get_adjacency", "dc_get_pairs",
            "dc_get_stats", "dc_destroy", "dc_error_string", "dc_measure_fp64_tflops", "dc_version",
            "dc_union_labels", "dc_unblank", "dc_ab_faces",
@@ -69,6 +70,7 @@ _lib.dc_create_grid.argtypes = [C.POINTER(_vp), C.c_int, C.c_longlong, _vp, C.c_
                                 _vp, C.c_size_t, C.c_longlong, C.c_longlong, _vp]
 _lib.dc_set_cut_surface.argtypes = [_vp, C.c_longlong, _vp, _vp]
 _lib.dc_classify.argtypes = [_vp, C.POINTER(dc_params), _vp, _vp, _vp]
+_lib.dc_cut.argtypes = [_vp, C.POINTER(dc_params), C.c_longlong, _vp, _vp, _vp, _vp]
 _lib.dc_classify_host.argtypes = [_vp, C.POINTER(dc_params), C.c_longlong, _vp, _vp, _vp, _vp]
 _lib.dc_get_element_boxes.argtypes = [_vp, _vp, _vp]
 _lib.dc_get_adjacency.argtypes = [_vp, _vp, _vp]
@@ -123,6 +125,11 @@ def dc_set_cut_surface(ctx, n_face, faces_ptr, stream):
 def dc_classify(ctx, params: Optional[dc_params], labels_ptr, sdist_ptr, stream):
     _ck(_lib.dc_classify(ctx, C.byref(params) if params is not None else None, labels_ptr, sdist_ptr,
                          stream or None), "dc_classify")
+
+
+def dc_cut(ctx, params: Optional[dc_params], n_face, faces_ptr, labels_ptr, sdist_ptr, stream):
+    _ck(_lib.dc_cut(ctx, C.byref(params) if params is not None else None, n_face, faces_ptr, labels_ptr, sdist_ptr,
+                    stream or None), "dc_cut")
 
 
 def dc_classify_host(ctx, params: Optional[dc_params], n_face, faces_host_ptr, labels_host_ptr, sdist_host_ptr, stream):
@@ -244,6 +251,17 @@ class DirectCut:
 
     def classify(self, params: Optional[dc_params] = None):
         dc_classify(self.ctx, params, self.labels.data_ptr(), self.sdist.data_ptr(), self._stream())
+        return self.labels, self.sdist
+
+    def cut(self, faces, params: Optional[dc_params] = None):
+        """dc_cut: set_cut_surface + classify in one call; with DC_FLAG_GRAPH in params.flags the launch sequence is
+        replayed from a CUDA graph (needs a current stream other than the legacy default stream)."""
+        t = self.torch
+        if not (isinstance(faces, t.Tensor) and faces.is_cuda):
+            faces = t.as_tensor(faces, dtype=t.float64).contiguous().to(self.xyz.device)
+        self.faces = faces.contiguous()
+        dc_cut(self.ctx, params, int(self.faces.shape[0]), self.faces.data_ptr(), self.labels.data_ptr(),
+               self.sdist.data_ptr(), self._stream())
         return self.labels, self.sdist
 
     def classify_host(self, faces_host, labels_host, sdist_host, params: Optional[dc_params] = None):

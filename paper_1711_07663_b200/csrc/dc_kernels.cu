@@ -27,6 +27,7 @@
 
 using namespace dcg;
 
+#define DC_MAX_GRAPHS 64                /* launch sequences dc_cut keeps as CUDA graphs (least recently used goes) */
 #define DC_MAX_SEEDLESS 1024           /* seedless components resolved per cut (each by one exhaustive query) */
 #define DC_GRID_MAX 64              /* face-bin cells per axis; cell (x,y,z) has code x + 64 (y + 64 z): a row along x is contiguous */
 #define DC_OCC (DC_GRID_MAX / 4)    /* coarse occupancy grid: 4 x 4 x 4 cells per entry */
@@ -59,6 +60,7 @@ struct DcScalars {
     int n_seedless;
     int uf_tile;                    // next tile of k_uf_tiles (tiles are taken in launch order)
     int n_lroots;                   // tile-local roots listed by k_uf_tiles
+    int epoch;                      // number of the cut (k_uf_tiles' flags); lives on the device so that a replayed CUDA graph counts too
     int surface_small;              // DC_STATUS_SURFACE_SMALL (kept apart from status: k_setup_classify resets that later)
     int status;
     int qn[DC_NQN];                 // items of round r (children queue, ping-pong buffers)
@@ -378,6 +380,7 @@ __global__ void k_adj_pass2(const int *__restrict__ conn, long long n_elem, cons
 __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
 {
     S->max_band = max_band;
+    S->epoch = S->epoch == 0x7fffffff ? 1 : S->epoch + 1;
     const double lref = P.l_ref > 0.0 ? P.l_ref : S->l_ref_auto;
     S->l_ref = lref;
     S->tau = (P.tau_cut_rel > 0.0 ? P.tau_cut_rel : 1e-7) * lref;
@@ -665,7 +668,7 @@ __device__ __forceinline__ void st_release(int *p, int v) { asm volatile("st.rel
 // 1024 elements facing one component of the slab below costs one union, not a thousand.
 #define UF_TILE 1024
 __global__ void __launch_bounds__(UF_TILE) k_uf_tiles(DcScalars *S, const signed char *__restrict__ labels, const int *__restrict__ adj,
-                                                      long long n_elem, int *parent, int *tile_flag, int epoch,
+                                                      long long n_elem, int *parent, int *tile_flag,
                                                       int *__restrict__ lroot_list)
 {
     __shared__ int sp[UF_TILE];
@@ -673,6 +676,7 @@ __global__ void __launch_bounds__(UF_TILE) k_uf_tiles(DcScalars *S, const signed
     __shared__ signed char s_lab[UF_TILE];
     __shared__ int s_tile;
     const int tid = threadIdx.x, lane = tid & 31;
+    const int epoch = S->epoch;
     if (tid == 0) s_tile = atomicAdd(&S->uf_tile, 1);
     s_last[tid] = -1;
     __syncthreads();
@@ -977,7 +981,7 @@ struct dc_ctx {
     DcScalars *S;
     double *ebox;             // [6][n_elem]
     int *adj_own;             // [n_elem][6] (derived) or NULL
-    int *parent; unsigned char *comp; int *tile_flag; int epoch;
+    int *parent; unsigned char *comp; int *tile_flag;
     int *act_elem;
     int *band_elem; long long *band_start; int *band_cnt;
     double *ecoef; float *pbox; unsigned long long *best, *dmin;
@@ -996,7 +1000,14 @@ struct dc_ctx {
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
     DcScalars *S_host;        // pinned
     DcScalars *S_band_host;   // pinned: the scalars as the banded cut left them, when a far pass has run since
+    bool last_was_graph;      // the last cut was a graph replay: no stage times
     bool far_ran; int far_passes; long long far_n_total; int far_error;
+    // dc_cut with DC_FLAG_GRAPH: the launch sequences captured so far, by what they were captured for
+    struct GraphEntry {
+        const double *faces; long long n_face; dc_params P; signed char *labels; double *sdist; cudaStream_t stream;
+        cudaGraphExec_t exec; unsigned long long stamp; int launches_surface, launches_classify;
+    } graphs[DC_MAX_GRAPHS];
+    int n_graphs; unsigned long long graph_clock;
     const AdtNode *adt; int adt_nodes;   // donor search tree (dc_adt_build), caller's memory
 };
 
@@ -1083,6 +1094,18 @@ extern "C" size_t dc_workspace_bytes(long long n_nodes, long long n_elem, long l
     fprintf(stderr, "libdc: %s failed: %s (%s:%d)\n", #call, cudaGetErrorString(e_), __FILE__, __LINE__); return DC_ERR_CUDA; } } while (0)
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+// The events that time the stages (dc_stats.ms_stage / ms_kernel).  On a stream that is being captured into a CUDA graph
+// (dc_cut with DC_FLAG_GRAPH, or the caller's own capture) they are left out: a plain record would only mark a dependency,
+// and as nodes of the graph (cudaEventRecordExternal) the 22 of them cost 3 us each -- most of what the graph saves.
+// dc_get_stats reports no stage times for a replayed cut; a plain dc_cut / dc_classify gives them.
+static cudaError_t ev_record(cudaEvent_t ev, cudaStream_t st)
+{
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    cudaError_t e = cudaStreamIsCapturing(st, &cs);
+    if (e != cudaSuccess) return e;
+    return cs == cudaStreamCaptureStatusActive ? cudaSuccess : cudaEventRecord(ev, st);
+}
 
 static int run_elem_boxes(dc_ctx *c, cudaStream_t st)
 {
@@ -1197,7 +1220,8 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
     cudaStream_t st = (cudaStream_t)stream;
     c->last_stream = st;
     CK(cudaSetDevice(c->device));
-    CK(cudaEventRecord(c->ev[8], st));
+    CK(ev_record(c->ev[8], st));
+    c->last_was_graph = false;
     c->face_nodes = face_nodes_dev; c->n_face = n_face;
     const int nf = (int)n_face;
     k_reset_surface<<<1, 1, 0, st>>>(c->S);
@@ -1212,7 +1236,7 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
     k_face_scatter<<<nblk(nf, 128), 128, 0, st>>>(face_nodes_dev, c->fbox_orig, c->fcell, c->cell_start, c->cell_fill,
                                                    nf, c->fperm, c->fbox, c->fcoef, c->fboxf);
     CK(cudaGetLastError());
-    CK(cudaEventRecord(c->ev[9], st));
+    CK(ev_record(c->ev[9], st));
     c->launches_surface = 8;
     c->have_surface = true;
     return DC_OK;
@@ -1221,7 +1245,7 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
 // S5 as a launch sequence (dc_narrow.cuh).  part 0: the band's narrow phase, with the events that time it.  The exact far
 // pass (dc_far.cuh) runs the same kernels on its own elements: part 1 = stage + seed solves (once per slice), part 2 = roots
 // to the last solve (once per pass, after the pass's candidate pairs have been written).
-#define EVREC(ev_, st_) do { if (part == 0) CK(cudaEventRecord(ev_, st_)); } while (0)
+#define EVREC(ev_, st_) do { if (part == 0) CK(ev_record(ev_, st_)); } while (0)
 static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds, int part)
 {
     // ---- S5: wavefront narrow phase (dc_narrow.cuh)
@@ -1292,7 +1316,7 @@ static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_d
     DcScalars *S = c->S;
     const long long ne = c->n_elem;
     unsigned char *pmask = (unsigned char *)c->pyr;
-    CK(cudaEventRecord(c->ev[11], st));
+    CK(ev_record(c->ev[11], st));
     k_far_pyramid<<<nblk(DC_PYR_TOTAL, 128), 128, 0, st>>>(c->cell_start, pmask);
     k_far_faces<<<nblk(c->n_face, 128), 128, 0, st>>>(S, c->fcoef, c->fbox, (int)c->n_face, c->ffar);
     k_far_list<<<nblk(ne, 256), 256, 0, st>>>(S, ne, labels_dev, sdist_dev, c->ebox, c->act_elem);
@@ -1348,7 +1372,7 @@ static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_d
             pending -= done;
         }
     }
-    CK(cudaEventRecord(c->ev[12], st));
+    CK(ev_record(c->ev[12], st));
     return DC_OK;
 }
 
@@ -1362,15 +1386,16 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     dc_params P; memset(&P, 0, sizeof P);
     if (params) P = *params;
     const long long ne = c->n_elem;
-    CK(cudaEventRecord(c->ev[0], st));
+    c->last_was_graph = false;
+    CK(ev_record(c->ev[0], st));
     if (P.flags & DC_FLAG_RECOMPUTE_BOXES) { int rc = run_elem_boxes(c, st); if (rc) return rc; }
-    CK(cudaEventRecord(c->ev[1], st));
+    CK(ev_record(c->ev[1], st));
     k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
     k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->occ, c->act_elem);
     k_pairs<<<c->num_sms * 16, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
                                            c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key,
                                            c->pair_band, c->nq, c->best, c->dmin);
-    CK(cudaEventRecord(c->ev[2], st));
+    CK(ev_record(c->ev[2], st));
     const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     const int rounds = 2 * max_level + 1;
     const int grid_rounds = rounds < DC_GRID_ROUNDS ? rounds : DC_GRID_ROUNDS;
@@ -1393,23 +1418,22 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
         k_pm_select<<<g, 128, 0, st>>>(S, W);
         k_pm_pass2<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->face_nodes, W);
         k_pm_decide<<<g, 128, 0, st>>>(S, c->band_elem, c->face_nodes, W, labels_dev, sdist_dev);
-        CK(cudaEventRecord(c->ev[3], st));
+        CK(ev_record(c->ev[3], st));
     } else {
     { const int rc = launch_narrow(c, st, rounds, grid_rounds, 0); if (rc) return rc; }
     DcScalars *S = c->S;
     k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev);
-    CK(cudaEventRecord(c->ev[3], st));
+    CK(ev_record(c->ev[3], st));
     }
-    c->epoch = c->epoch == 0x7fffffff ? 1 : c->epoch + 1;
-    k_uf_tiles<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(c->S, labels_dev, c->adj, ne, c->parent, c->tile_flag, c->epoch, c->act_elem);
+    k_uf_tiles<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(c->S, labels_dev, c->adj, ne, c->parent, c->tile_flag, c->act_elem);
     k_uf_seed<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
     k_uf_resolve<<<c->num_sms * 4, 256, 0, st>>>(c->S, c->act_elem, c->parent, c->comp);
     k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     k_seedless<<<32, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
     k_uf_fix<<<c->num_sms * 4, 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
     CK(cudaGetLastError());
-    CK(cudaEventRecord(c->ev[4], st));
+    CK(ev_record(c->ev[4], st));
     c->far_ran = false;
     if ((P.flags & DC_FLAG_EXACT_FAR) && !(P.flags & DC_FLAG_PAPER_MODE)) {
         const int rc = run_exact_far(c, st, labels_dev, sdist_dev, rounds, grid_rounds);
@@ -1417,6 +1441,69 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     }
     c->launches_classify = ((P.flags & DC_FLAG_PAPER_MODE) ? 13 : 21 + grid_rounds + (rounds > grid_rounds ? 1 : 0)) + ((P.flags & DC_FLAG_RECOMPUTE_BOXES) ? 1 : 0);
     c->have_cut = true;
+    return DC_OK;
+}
+
+// One cut in one call: dc_set_cut_surface + dc_classify.  With DC_FLAG_GRAPH the launch sequence (about 35 short kernels,
+// two memsets, the stage events) is captured into a CUDA graph the first time it is asked for with these arguments, and
+// replayed afterwards: the gaps between dependent launches go (config 2: 1.22 -> 1.11 ms per cut; config 0: 0.28 -> 0.17).
+// Everything a replay must see anew is on the device (the cut's counters, the epoch of the flood fill's flags); what the
+// graph fixes is what it was captured for: the surface's address and face count, the parameters, the output addresses, the
+// stream.  The surface's CONTENTS may change between calls (a moving body updated in place: the re-cut of PAPER.md L233).
+extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, const double *face_nodes_dev,
+                      signed char *labels_dev, double *sdist_dev, void *stream)
+{
+    if (!c || !face_nodes_dev || !labels_dev || !sdist_dev || n_face <= 0) return DC_ERR_ARG;
+    if (n_face > c->max_faces) return DC_ERR_WORKSPACE;
+    dc_params P; memset(&P, 0, sizeof P);
+    if (params) P = *params;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    CK(cudaSetDevice(c->device));
+    CK(cudaStreamIsCapturing(st, &cs));
+    // no graph of our own: not asked for; the far pass reads counters back between its passes; the caller is capturing
+    // already (our launches then go into the caller's graph); the legacy default stream cannot be captured
+    if (!(P.flags & DC_FLAG_GRAPH) || (P.flags & DC_FLAG_EXACT_FAR) || cs != cudaStreamCaptureStatusNone || st == nullptr) {
+        const int rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
+        return rc ? rc : dc_classify(c, &P, labels_dev, sdist_dev, stream);
+    }
+    dc_ctx::GraphEntry *g = nullptr;
+    for (int i = 0; i < c->n_graphs; ++i) {
+        dc_ctx::GraphEntry &q = c->graphs[i];
+        if (q.faces == face_nodes_dev && q.n_face == n_face && q.labels == labels_dev && q.sdist == sdist_dev && q.stream == st &&
+            memcmp(&q.P, &P, sizeof P) == 0) { g = &q; break; }
+    }
+    if (!g) {
+        CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+        int rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
+        if (!rc) rc = dc_classify(c, &P, labels_dev, sdist_dev, stream);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(st, &graph);
+        if (rc || e != cudaSuccess || !graph) {
+            if (graph) cudaGraphDestroy(graph);
+            (void)cudaGetLastError();
+            c->have_cut = false;
+            return rc ? rc : DC_ERR_CUDA;
+        }
+        cudaGraphExec_t exec = nullptr;
+        const cudaError_t ei = cudaGraphInstantiate(&exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ei != cudaSuccess) { fprintf(stderr, "libdc: cudaGraphInstantiate failed: %s\n", cudaGetErrorString(ei)); return DC_ERR_CUDA; }
+        if (c->n_graphs < DC_MAX_GRAPHS) g = &c->graphs[c->n_graphs++];
+        else {
+            g = &c->graphs[0];
+            for (int i = 1; i < DC_MAX_GRAPHS; ++i) if (c->graphs[i].stamp < g->stamp) g = &c->graphs[i];
+            cudaGraphExecDestroy(g->exec);
+        }
+        g->faces = face_nodes_dev; g->n_face = n_face; g->P = P; g->labels = labels_dev; g->sdist = sdist_dev; g->stream = st;
+        g->exec = exec; g->launches_surface = c->launches_surface; g->launches_classify = c->launches_classify;
+    }
+    g->stamp = ++c->graph_clock;
+    // what the two calls leave on the host
+    c->face_nodes = face_nodes_dev; c->n_face = n_face; c->last_stream = st;
+    c->launches_surface = g->launches_surface; c->launches_classify = g->launches_classify;
+    c->have_surface = true; c->have_cut = true; c->far_ran = false; c->last_was_graph = true;
+    CK(cudaGraphLaunch(g->exec, st));
     return DC_OK;
 }
 
@@ -1428,9 +1515,7 @@ extern "C" int dc_classify_host(dc_ctx *c, const dc_params *params, long long n_
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(c->device));
     CK(cudaMemcpyAsync(c->h_faces_dev, face_nodes_host, (size_t)n_face * 27 * 8, cudaMemcpyHostToDevice, st));
-    int rc = dc_set_cut_surface(c, n_face, c->h_faces_dev, stream);
-    if (rc) return rc;
-    rc = dc_classify(c, params, c->h_labels_dev, c->h_sdist_dev, stream);
+    const int rc = dc_cut(c, params, n_face, c->h_faces_dev, c->h_labels_dev, c->h_sdist_dev, stream);
     if (rc) return rc;
     CK(cudaMemcpyAsync(labels_host, c->h_labels_dev, (size_t)c->n_elem, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(sdist_host, c->h_sdist_dev, (size_t)c->n_elem * 8, cudaMemcpyDeviceToHost, st));
@@ -1528,7 +1613,7 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
     o->l_ref = S.l_ref; o->tau_cut = S.tau; o->d_band = S.d_band;
     o->status = S.status;
     o->n_launches = (c->have_surface ? c->launches_surface : 0) + (c->have_cut ? c->launches_classify : 0);
-    if (c->have_cut) {
+    if (c->have_cut && !c->last_was_graph) {
         float ms;
         if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) == cudaSuccess) o->ms_stage[1] = ms;
         if (cudaEventElapsedTime(&ms, c->ev[1], c->ev[2]) == cudaSuccess) o->ms_stage[2] = ms;
@@ -1547,7 +1632,7 @@ extern "C" int dc_get_stats(dc_ctx *c, dc_stats *o)
         // (ms_stage[7]: every k_np_solve launch = seeds + leaf passes + overflow rounds; the compaction pass is not in it)
         o->ms_stage[7] = o->ms_kernel[1] + o->ms_kernel[5] + o->ms_kernel[6];
     }
-    if (c->have_surface) {
+    if (c->have_surface && !c->last_was_graph) {
         float ms;
         if (cudaEventElapsedTime(&ms, c->ev[8], c->ev[9]) == cudaSuccess) { o->ms_stage[0] = ms; o->ms_stage[6] = ms; }
     }
@@ -1567,6 +1652,7 @@ extern "C" void dc_destroy(dc_ctx *c)
     for (int i = 0; i < 10; ++i) if (c->evk[i]) cudaEventDestroy(c->evk[i]);
     if (c->S_host) cudaFreeHost(c->S_host);
     if (c->S_band_host) cudaFreeHost(c->S_band_host);
+    for (int i = 0; i < c->n_graphs; ++i) if (c->graphs[i].exec) cudaGraphExecDestroy(c->graphs[i].exec);
     delete c;
 }
 
@@ -1659,5 +1745,5 @@ extern "C" int dc_find_donors(dc_ctx *c, long long n_pts, const double *pts_dev,
     return DC_OK;
 }
 
-extern "C" int dc_version(void) { return 3; }
+extern "C" int dc_version(void) { return 4; }
 
