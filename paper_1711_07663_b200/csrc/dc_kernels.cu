@@ -82,6 +82,14 @@ struct DcScalars {
     unsigned long long far_lo[3], far_hi[3];    // box of the far elements' centres (ordered-uint encodings)
 };
 
+// first statement of every kernel of a cut (see launch_pdl): let the next kernel start launching, then wait for the previous
+// one (a no-op for a kernel launched the plain way)
+__device__ __forceinline__ void pdl_start()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 __device__ __forceinline__ void atomic_min_d(unsigned long long *addr, double v) { atomicMin(addr, enc_ord(v)); }
 __device__ __forceinline__ void atomic_max_d(unsigned long long *addr, double v) { atomicMax(addr, enc_ord(v)); }
 
@@ -96,6 +104,7 @@ __device__ __forceinline__ double bez_mid(double x0, double x1, double x2) { ret
 __global__ void k_face_boxes(DcScalars *S, const double *__restrict__ face_nodes, int n_face,
                              double *__restrict__ fbox_orig /*[n_face][6]*/)
 {
+    pdl_start();
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
     double lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
     double nlo[3] = { INFINITY, INFINITY, INFINITY }, nhi[3] = { -INFINITY, -INFINITY, -INFINITY };
@@ -142,6 +151,7 @@ __global__ void k_face_boxes(DcScalars *S, const double *__restrict__ face_nodes
 
 __global__ void k_reset_surface(DcScalars *S)
 {
+    pdl_start();
     for (int c = 0; c < 3; ++c) {
         S->node_min[c] = S->fbox_min[c] = ~0ull;
         S->node_max[c] = S->fbox_max[c] = 0ull;
@@ -151,6 +161,7 @@ __global__ void k_reset_surface(DcScalars *S)
 
 __global__ void k_setup_surface(DcScalars *S, int n_face)
 {
+    pdl_start();
     double ext = 0.0, lref = 0.0;
     for (int c = 0; c < 3; ++c) {
         S->smin[c] = dec_ord(S->fbox_min[c]); S->smax[c] = dec_ord(S->fbox_max[c]);
@@ -180,6 +191,7 @@ __device__ __forceinline__ int cell_coord(const DcScalars *S, double x, int c)
 __global__ void k_face_hist(const DcScalars *S, const double *__restrict__ fbox_orig, int n_face,
                             int *__restrict__ fcell, int *cell_count)
 {
+    pdl_start();
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= n_face) return;
     int ic[3];
@@ -209,6 +221,7 @@ __device__ __forceinline__ int block_sum_256(int v, int *s_warp)
 }
 __global__ void __launch_bounds__(256) k_scan_sums(const int *__restrict__ cell_count, int *__restrict__ chunk_sum)
 {
+    pdl_start();
     __shared__ int s_warp[8];
     const int4 v = reinterpret_cast<const int4 *>(cell_count)[blockIdx.x * 256 + threadIdx.x];
     const int t = block_sum_256(v.x + v.y + v.z + v.w, s_warp);
@@ -217,6 +230,7 @@ __global__ void __launch_bounds__(256) k_scan_sums(const int *__restrict__ cell_
 __global__ void __launch_bounds__(256) k_scan_cells(const int *__restrict__ cell_count, const int *__restrict__ chunk_sum,
                                                     int *__restrict__ cell_start)
 {
+    pdl_start();
     __shared__ int s_warp[8];
     __shared__ int s_incl[8];
     // sum of the chunks before this one (SCAN_NCHUNK = 256 values: one per thread)
@@ -242,6 +256,7 @@ __global__ void __launch_bounds__(256) k_scan_cells(const int *__restrict__ cell
 // near the surface's box are in empty space)
 __global__ void k_cell_occ(const int *__restrict__ cell_start, unsigned char *__restrict__ occ)
 {
+    pdl_start();
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= DC_OCC * DC_OCC * DC_OCC) return;
     const int X = t % DC_OCC, Y = (t / DC_OCC) % DC_OCC, Z = t / (DC_OCC * DC_OCC);
@@ -260,6 +275,7 @@ __global__ void k_face_scatter(const double *__restrict__ face_nodes, const doub
                                int *cell_fill, int n_face, int *__restrict__ fperm,
                                double *__restrict__ fbox, double *__restrict__ fcoef, float *__restrict__ fboxf)
 {
+    pdl_start();
     const int f = blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= n_face) return;
     const int code = fcell[f];
@@ -303,6 +319,7 @@ __global__ void __launch_bounds__(EB_THREADS) k_elem_boxes(DcScalars *S, const d
                                                            const int *__restrict__ conn, long long n_elem,
                                                            double *__restrict__ ebox)
 {
+    pdl_start();
     // One (element, coordinate) pair per work item, 3 items per thread: consecutive lanes read CONSECUTIVE
     // doubles of a node (x, y, z of one element, then the next element), so one warp load touches a third
     // of the sectors a lane-per-element gather would, and the Lagrange -> Bezier conversion is per coordinate
@@ -379,6 +396,7 @@ __global__ void k_adj_pass2(const int *__restrict__ conn, long long n_elem, cons
 // per-classify scalar setup
 __global__ void k_setup_classify(DcScalars *S, dc_params P, int max_band)
 {
+    pdl_start();
     S->max_band = max_band;
     S->epoch = S->epoch == 0x7fffffff ? 1 : S->epoch + 1;
     const double lref = P.l_ref > 0.0 ? P.l_ref : S->l_ref_auto;
@@ -451,6 +469,7 @@ __global__ void k_filter(DcScalars *S, const double *__restrict__ ebox, long lon
                          unsigned char *__restrict__ comp, const int *__restrict__ cell_start,
                          const unsigned char *__restrict__ occ, int *__restrict__ act_elem)
 {
+    pdl_start();
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     bool active = false;
     if (e < n_elem) {
@@ -500,6 +519,7 @@ __global__ void __launch_bounds__(PR_WARPS * 32) k_pairs(DcScalars *S, const dou
                                                int *__restrict__ pair_band, NItem *__restrict__ seed_q,
                                                unsigned long long *__restrict__ best, unsigned long long *__restrict__ dmin)
 {
+    pdl_start();
     __shared__ int s_list[PR_GROUPS][PR_CAP];
     __shared__ int s_off[PR_GROUPS][PR_W + 1];
     __shared__ int s_first[PR_GROUPS][PR_W];
@@ -671,6 +691,7 @@ __global__ void __launch_bounds__(UF_TILE) k_uf_tiles(DcScalars *S, const signed
                                                       long long n_elem, int *parent, int *tile_flag,
                                                       int *__restrict__ lroot_list)
 {
+    pdl_start();
     __shared__ int sp[UF_TILE];
     __shared__ int s_last[UF_TILE];
     __shared__ signed char s_lab[UF_TILE];
@@ -754,6 +775,7 @@ __global__ void __launch_bounds__(UF_TILE) k_uf_tiles(DcScalars *S, const signed
 __global__ void k_uf_seed(const DcScalars *S, const int *__restrict__ band_elem, const signed char *__restrict__ labels,
                           int *parent, unsigned char *comp)
 {
+    pdl_start();
     const int n_band = min(S->n_band, S->max_band);
     for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < n_band; b += gridDim.x * blockDim.x) {
         const int e = band_elem[b];
@@ -778,6 +800,7 @@ __global__ void k_uf_seed(const DcScalars *S, const int *__restrict__ band_elem,
 __global__ void __launch_bounds__(SL_THREADS) k_seedless(DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
                                                          const double *__restrict__ fcoef, int n_face, unsigned char *comp)
 {
+    pdl_start();
     __shared__ double s_ecoef[6][28];
     __shared__ double s_nodes[81];
     __shared__ unsigned long long s_best;
@@ -898,6 +921,7 @@ __device__ __forceinline__ void uf_census(DcScalars *S, int lab, bool conflict)
 }
 __global__ void k_uf_resolve(DcScalars *S, const int *__restrict__ lroot_list, int *parent, unsigned char *comp)
 {
+    pdl_start();
     const int n = S->n_lroots;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int r = lroot_list[i];
@@ -915,6 +939,7 @@ __global__ void k_uf_assign(DcScalars *S, long long n_elem, const int *__restric
                             const unsigned char *__restrict__ comp, signed char *__restrict__ labels,
                             double *__restrict__ sdist)
 {
+    pdl_start();
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int lab = -2, out = -2;
     bool conflict = false;
@@ -929,6 +954,7 @@ __global__ void k_uf_assign(DcScalars *S, long long n_elem, const int *__restric
 __global__ void k_uf_fix(DcScalars *S, long long n_elem, int *parent, const unsigned char *__restrict__ comp,
                          signed char *__restrict__ labels, double *__restrict__ sdist)
 {
+    pdl_start();
     if (S->n_seedless == 0) return;
     for (long long e0 = (long long)blockIdx.x * blockDim.x; e0 < n_elem; e0 += (long long)gridDim.x * blockDim.x) {
         const long long e = e0 + threadIdx.x;
@@ -1095,6 +1121,22 @@ extern "C" size_t dc_workspace_bytes(long long n_nodes, long long n_elem, long l
 
 static inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
+// Every kernel of a cut is launched with programmatic stream serialisation: it starts as its predecessor's CTAs drain
+// (each kernel raises griddepcontrol.launch_dependents on entry) and waits at griddepcontrol.wait -- its first
+// instruction after that -- until the predecessor has completed and its writes are visible.  What overlaps is the launch
+// latency and the tail of one kernel with the ramp of the next: a cut is ~38 short dependent kernels.
+template <class... KArgs, class... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args &&... args)
+{
+    cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 // The events that time the stages (dc_stats.ms_stage / ms_kernel).  On a stream that is being captured into a CUDA graph
 // (dc_cut with DC_FLAG_GRAPH, or the caller's own capture) they are left out: a plain record would only mark a dependency,
 // and as nodes of the graph (cudaEventRecordExternal) the 22 of them cost 3 us each -- most of what the graph saves.
@@ -1110,7 +1152,7 @@ static cudaError_t ev_record(cudaEvent_t ev, cudaStream_t st)
 static int run_elem_boxes(dc_ctx *c, cudaStream_t st)
 {
     CK(cudaMemsetAsync(&c->S->grid_max_diag2, 0, 8, st));
-    k_elem_boxes<<<nblk(c->n_elem, EB_THREADS), EB_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->n_elem, c->ebox);
+    CK(launch_pdl(k_elem_boxes, nblk(c->n_elem, EB_THREADS), EB_THREADS, st, c->S, c->xyz, c->conn, c->n_elem, c->ebox));
     CK(cudaGetLastError());
     return DC_OK;
 }
@@ -1224,17 +1266,17 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
     c->last_was_graph = false;
     c->face_nodes = face_nodes_dev; c->n_face = n_face;
     const int nf = (int)n_face;
-    k_reset_surface<<<1, 1, 0, st>>>(c->S);
-    k_face_boxes<<<nblk(nf, 128), 128, 0, st>>>(c->S, face_nodes_dev, nf, c->fbox_orig);
-    k_setup_surface<<<1, 1, 0, st>>>(c->S, nf);
+    CK(launch_pdl(k_reset_surface, 1, 1, st, c->S));
+    CK(launch_pdl(k_face_boxes, nblk(nf, 128), 128, st, c->S, face_nodes_dev, nf, c->fbox_orig));
+    CK(launch_pdl(k_setup_surface, 1, 1, st, c->S, nf));
     CK(cudaMemsetAsync(c->cell_count, 0, (size_t)(DC_NCELL + 1) * 4, st));
     CK(cudaMemsetAsync(c->cell_fill, 0, (size_t)(DC_NCELL + 1) * 4, st));
-    k_face_hist<<<nblk(nf, 128), 128, 0, st>>>(c->S, c->fbox_orig, nf, c->fcell, c->cell_count);
-    k_scan_sums<<<SCAN_NCHUNK, 256, 0, st>>>(c->cell_count, c->cell_fill + DC_NCELL + 8);
-    k_scan_cells<<<SCAN_NCHUNK, 256, 0, st>>>(c->cell_count, c->cell_fill + DC_NCELL + 8, c->cell_start);
-    k_cell_occ<<<(DC_OCC * DC_OCC * DC_OCC + 127) / 128, 128, 0, st>>>(c->cell_start, c->occ);
-    k_face_scatter<<<nblk(nf, 128), 128, 0, st>>>(face_nodes_dev, c->fbox_orig, c->fcell, c->cell_start, c->cell_fill,
-                                                   nf, c->fperm, c->fbox, c->fcoef, c->fboxf);
+    CK(launch_pdl(k_face_hist, nblk(nf, 128), 128, st, c->S, c->fbox_orig, nf, c->fcell, c->cell_count));
+    CK(launch_pdl(k_scan_sums, SCAN_NCHUNK, 256, st, c->cell_count, c->cell_fill + DC_NCELL + 8));
+    CK(launch_pdl(k_scan_cells, SCAN_NCHUNK, 256, st, c->cell_count, c->cell_fill + DC_NCELL + 8, c->cell_start));
+    CK(launch_pdl(k_cell_occ, (DC_OCC * DC_OCC * DC_OCC + 127) / 128, 128, st, c->cell_start, c->occ));
+    CK(launch_pdl(k_face_scatter, nblk(nf, 128), 128, st, face_nodes_dev, c->fbox_orig, c->fcell, c->cell_start, c->cell_fill,
+                                                   nf, c->fperm, c->fbox, c->fcoef, c->fboxf));
     CK(cudaGetLastError());
     CK(ev_record(c->ev[9], st));
     c->launches_surface = 8;
@@ -1251,29 +1293,29 @@ static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds
     // ---- S5: wavefront narrow phase (dc_narrow.cuh)
     const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
     DcScalars *S = c->S;
-    if (part != 2) k_np_stage<<<gw, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox);
+    if (part != 2) CK(launch_pdl(k_np_stage, gw, 128, st, S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox));
     // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
     // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
     const int gs = c->num_sms * 2 * 4;     // solve grids: grid-stride, 2 resident CTAs of 128 threads per SM
     EVREC(c->ev[7], st);
     if (part != 2)
-        k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                                 c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT);
+        CK(launch_pdl(k_np_solve<0>, gs, NW_THREADS, st, S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                                 c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT));
     if (part == 1) { CK(cudaGetLastError()); return DC_OK; }
     EVREC(c->ev[10], st);
-    k_np_roots<<<c->num_sms * 8, 256, 0, st>>>(S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
-                                               c->q[0], &S->qn[0], c->qcap);
+    CK(launch_pdl(k_np_roots, c->num_sms * 8, 256, st, S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
+                                               c->q[0], &S->qn[0], c->qcap));
     // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
     // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
     EVREC(c->evk[0], st);
-    k_np_bound<true><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                 c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
+    CK(launch_pdl(k_np_bound<true>, gw, NPW_THREADS, st, S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                 c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0));
     for (int r = 1; r < grid_rounds; ++r)
-        k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                      c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0);
+        CK(launch_pdl(k_np_bound<false>, gw, NPW_THREADS, st, S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                      c->q[(r + 1) & 1], &S->qn[r + 1], c->nq, c->nqx, &S->nn[0], c->qcap, 0));
     if (rounds > grid_rounds)
-        k_np_bound_tail<<<1, NP_TAIL_THREADS, 0, st>>>(S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
-                                                       c->nq, c->nqx, &S->nn[0], c->qcap);
+        CK(launch_pdl(k_np_bound_tail, 1, NP_TAIL_THREADS, st, S, grid_rounds, rounds, c->q[0], c->q[1], c->pair_face, c->fcoef, c->ecoef, c->best,
+                                                       c->nq, c->nqx, &S->nn[0], c->qcap));
     // all leaves: first dropped if their element's best distance has fallen below their lower bound meanwhile (the two
     // bound queues are free by now and take the compacted leaf queue), then three solve passes (the old leaf queue's
     // memory holds the continuations and the overflow queue of sub-leaves)
@@ -1283,25 +1325,25 @@ static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds
     const long long capA = c->qcap / 4, capB = c->qcap / 8;
     NItem *ovf1 = (NItem *)c->nqx + c->qcap / 2;
     const long long cap_ovf1 = c->qcap / 2;
-    k_np_compact<<<c->num_sms * 8, 256, 0, st>>>(S, &S->nn[0], c->qcap, c->nq, c->nqx, c->best, lq, lqx, &S->nn[5]);
+    CK(launch_pdl(k_np_compact, c->num_sms * 8, 256, st, S, &S->nn[0], c->qcap, c->nq, c->nqx, c->best, lq, lqx, &S->nn[5]));
     EVREC(c->evk[1], st);
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[5], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, contA, &S->nh[0], capA, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET1, NW_MAXIT);
-    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[0], capA, nullptr, nullptr, contA, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, contB, &S->nh[1], capB, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET2, NW_MAXIT);
-    k_np_solve<1><<<gs, NW_THREADS, 0, st>>>(S, &S->nh[1], capB, nullptr, nullptr, contB, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, ovf1, &S->nn[1], cap_ovf1, 0, NW_MAXIT);
+    CK(launch_pdl(k_np_solve<0>, gs, NW_THREADS, st, S, &S->nn[5], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, contA, &S->nh[0], capA, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET1, NW_MAXIT));
+    CK(launch_pdl(k_np_solve<1>, gs, NW_THREADS, st, S, &S->nh[0], capA, nullptr, nullptr, contA, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, contB, &S->nh[1], capB, ovf1, &S->nn[1], cap_ovf1, NW_BUDGET2, NW_MAXIT));
+    CK(launch_pdl(k_np_solve<1>, gs, NW_THREADS, st, S, &S->nh[1], capB, nullptr, nullptr, contB, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, ovf1, &S->nn[1], cap_ovf1, 0, NW_MAXIT));
     EVREC(c->evk[2], st);
     // The sub-leaves of unconverged solves come back through one bound pass (best[b] is final or nearly so: most of them
     // are pruned) and one solve launch, twice; the last launch finishes whatever still fails on the lane that held it.
-    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
-                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[2], c->qcap, 1);
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[2], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, c->nq, &S->nn[3], c->qcap, 0, NW_OVF_MAXIT);
-    k_np_bound<false><<<gw, NPW_THREADS, 0, st>>>(S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
-                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[4], c->qcap, 1);
-    k_np_solve<0><<<gs, NW_THREADS, 0, st>>>(S, &S->nn[4], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
-                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_OVF_MAXIT);
+    CK(launch_pdl(k_np_bound<false>, gw, NPW_THREADS, st, S, &S->nn[1], ovf1, c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[2], c->qcap, 1));
+    CK(launch_pdl(k_np_solve<0>, gs, NW_THREADS, st, S, &S->nn[2], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, c->nq, &S->nn[3], c->qcap, 0, NW_OVF_MAXIT));
+    CK(launch_pdl(k_np_bound<false>, gw, NPW_THREADS, st, S, &S->nn[3], c->nq, c->pair_face, c->fcoef, c->ecoef, c->best,
+                                           nullptr, &S->qn[DC_NQN - 1], lq, lqx, &S->nn[4], c->qcap, 1));
+    CK(launch_pdl(k_np_solve<0>, gs, NW_THREADS, st, S, &S->nn[4], c->qcap, lq, lqx, nullptr, c->pair_face, c->fcoef, c->ecoef,
+                                             c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_OVF_MAXIT));
     EVREC(c->ev[6], st);
     CK(cudaGetLastError());
     return DC_OK;
@@ -1390,11 +1432,11 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     CK(ev_record(c->ev[0], st));
     if (P.flags & DC_FLAG_RECOMPUTE_BOXES) { int rc = run_elem_boxes(c, st); if (rc) return rc; }
     CK(ev_record(c->ev[1], st));
-    k_setup_classify<<<1, 1, 0, st>>>(c->S, P, (int)c->max_band);
-    k_filter<<<nblk(ne, 256), 256, 0, st>>>(c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->occ, c->act_elem);
-    k_pairs<<<c->num_sms * 16, 256, 0, st>>>(c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
+    CK(launch_pdl(k_setup_classify, 1, 1, st, c->S, P, (int)c->max_band));
+    CK(launch_pdl(k_filter, nblk(ne, 256), 256, st, c->S, c->ebox, ne, labels_dev, c->parent, c->comp, c->cell_start, c->occ, c->act_elem));
+    CK(launch_pdl(k_pairs, c->num_sms * 16, 256, st, c->S, c->ebox, ne, c->act_elem, c->cell_start, c->fbox, c->max_pairs,
                                            c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->pair_key,
-                                           c->pair_band, c->nq, c->best, c->dmin);
+                                           c->pair_band, c->nq, c->best, c->dmin));
     CK(ev_record(c->ev[2], st));
     const int max_level = (P.max_level > 0 && P.max_level <= 12) ? P.max_level : 12;
     const int rounds = 2 * max_level + 1;
@@ -1413,25 +1455,25 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
         W.d2 = (double *)base; base += mb * PM_NF2 * 3 * 8;
         W.v2 = (double *)base;
         const int g = c->num_sms * 8;
-        k_pm_rank<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fperm, c->face_nodes, W);
-        k_pm_pass1<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->face_nodes, W);
-        k_pm_select<<<g, 128, 0, st>>>(S, W);
-        k_pm_pass2<<<g, 128, 0, st>>>(S, c->xyz, c->conn, c->band_elem, c->face_nodes, W);
-        k_pm_decide<<<g, 128, 0, st>>>(S, c->band_elem, c->face_nodes, W, labels_dev, sdist_dev);
+        CK(launch_pdl(k_pm_rank, g, 128, st, S, c->xyz, c->conn, c->band_elem, c->band_start, c->band_cnt, c->pair_face, c->fperm, c->face_nodes, W));
+        CK(launch_pdl(k_pm_pass1, g, 128, st, S, c->xyz, c->conn, c->band_elem, c->face_nodes, W));
+        CK(launch_pdl(k_pm_select, g, 128, st, S, W));
+        CK(launch_pdl(k_pm_pass2, g, 128, st, S, c->xyz, c->conn, c->band_elem, c->face_nodes, W));
+        CK(launch_pdl(k_pm_decide, g, 128, st, S, c->band_elem, c->face_nodes, W, labels_dev, sdist_dev));
         CK(ev_record(c->ev[3], st));
     } else {
     { const int rc = launch_narrow(c, st, rounds, grid_rounds, 0); if (rc) return rc; }
     DcScalars *S = c->S;
-    k_np_decide<<<c->num_sms * 8, 256, 0, st>>>(S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
-                                                                              c->pair_key, labels_dev, sdist_dev);
+    CK(launch_pdl(k_np_decide, c->num_sms * 8, 256, st, S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
+                                                                              c->pair_key, labels_dev, sdist_dev));
     CK(ev_record(c->ev[3], st));
     }
-    k_uf_tiles<<<nblk(ne, UF_TILE), UF_TILE, 0, st>>>(c->S, labels_dev, c->adj, ne, c->parent, c->tile_flag, c->act_elem);
-    k_uf_seed<<<c->num_sms * 8, 256, 0, st>>>(c->S, c->band_elem, labels_dev, c->parent, c->comp);
-    k_uf_resolve<<<c->num_sms * 4, 256, 0, st>>>(c->S, c->act_elem, c->parent, c->comp);
-    k_uf_assign<<<nblk(ne, 256), 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
-    k_seedless<<<32, SL_THREADS, 0, st>>>(c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp);
-    k_uf_fix<<<c->num_sms * 4, 256, 0, st>>>(c->S, ne, c->parent, c->comp, labels_dev, sdist_dev);
+    CK(launch_pdl(k_uf_tiles, nblk(ne, UF_TILE), UF_TILE, st, c->S, labels_dev, c->adj, ne, c->parent, c->tile_flag, c->act_elem));
+    CK(launch_pdl(k_uf_seed, c->num_sms * 8, 256, st, c->S, c->band_elem, labels_dev, c->parent, c->comp));
+    CK(launch_pdl(k_uf_resolve, c->num_sms * 4, 256, st, c->S, c->act_elem, c->parent, c->comp));
+    CK(launch_pdl(k_uf_assign, nblk(ne, 256), 256, st, c->S, ne, c->parent, c->comp, labels_dev, sdist_dev));
+    CK(launch_pdl(k_seedless, 32, SL_THREADS, st, c->S, c->xyz, c->conn, c->fcoef, (int)c->n_face, c->comp));
+    CK(launch_pdl(k_uf_fix, c->num_sms * 4, 256, st, c->S, ne, c->parent, c->comp, labels_dev, sdist_dev));
     CK(cudaGetLastError());
     CK(ev_record(c->ev[4], st));
     c->far_ran = false;

@@ -117,6 +117,7 @@ __global__ void __launch_bounds__(128) k_np_stage(const DcScalars *S, const doub
                                                   const int *__restrict__ band_elem, double *__restrict__ ecoef,
                                                   float *__restrict__ pbox)
 {
+    pdl_start();
     const int n_band = min(S->n_band, S->max_band);
     const long long n = (long long)n_band * 6;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
@@ -203,6 +204,7 @@ __global__ void __launch_bounds__(256) k_np_compact(const DcScalars *S, const in
                                                     const unsigned long long *__restrict__ best,
                                                     NItem *__restrict__ nq_out, NLeafX *__restrict__ nqx_out, int *__restrict__ n_out)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     const int n = min(*n_in, (int)min(in_cap, (long long)0x7fffffff));
     const double tau_exit = S->tau_exit, t_tie = S->t_tie;
@@ -243,6 +245,7 @@ __global__ void __launch_bounds__(NW_THREADS, 2) k_np_solve(DcScalars *S, const 
                                                            NItem *__restrict__ ovf, int *__restrict__ ovf_n, long long ovf_cap,
                                                            int budget, int maxit)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     const int n = min(*n_items, (int)min(in_cap, (long long)0x7fffffff));
     const double tau_exit = S->tau_exit, tol_d2 = S->tol_d * S->tol_d, t_tie = S->t_tie;
@@ -410,6 +413,7 @@ __global__ void __launch_bounds__(256) k_np_roots(DcScalars *S, const int *__res
                                                   const unsigned long long *__restrict__ best, long long max_pairs,
                                                   NItem *__restrict__ qout, int *__restrict__ qout_n, long long qcap)
 {
+    pdl_start();
     __shared__ int s_wsum[8];
     __shared__ int s_base, s_total;
     if (S->status & DC_STATUS_INVALID) return;       // an overflow upstream left holes in the lists: nothing here can be trusted (or safely read)
@@ -545,6 +549,7 @@ __global__ void __launch_bounds__(NPW_THREADS, ROOT ? 3 : 2) k_np_bound(DcScalar
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
                                                           NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap, int force_leaf)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     const int n = min(*n_in, (int)min(qcap, (long long)0x7fffffff));
     if (n == 0) return;
@@ -563,6 +568,7 @@ __global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S,
                                                                    const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                                    NItem *__restrict__ nq, NLeafX *__restrict__ nqx, int *__restrict__ nq_n, long long qcap)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     NpCounters cnt = { 0, 0, 0, 0, 0 };
     for (int r = r_begin; r < r_end; ++r) {
@@ -585,6 +591,7 @@ __global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, con
                             const unsigned long long *__restrict__ dmin_arr, const unsigned long long *__restrict__ pair_key,
                             signed char *__restrict__ labels, double *__restrict__ sdist)
 {
+    pdl_start();
     const int n_band = min(S->n_band, S->max_band);
     const double tau = S->tau, tau_exit = S->tau_exit, amb = S->amb, t_tie = S->t_tie, d_band = S->d_band;
     unsigned n_amb = 0, n_samb = 0;

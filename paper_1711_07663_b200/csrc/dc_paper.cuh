@@ -193,6 +193,7 @@ __global__ void __launch_bounds__(128) k_pm_rank(const DcScalars *S, const doubl
                                                  const int *__restrict__ band_cnt, const int *__restrict__ pair_face,
                                                  const int *__restrict__ fperm, const double *__restrict__ face_nodes, PmWork W)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     using namespace dcp;
     const int n_band = min(S->n_band, S->max_band);
@@ -286,6 +287,7 @@ __global__ void __launch_bounds__(128) k_pm_rank(const DcScalars *S, const doubl
 __global__ void __launch_bounds__(128) k_pm_pass1(const DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
                                                   const int *__restrict__ band_elem, const double *__restrict__ face_nodes, PmWork W)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     using namespace dcp;
     const long long n = (long long)min(S->n_band, S->max_band) * PM_NF1;
@@ -325,6 +327,7 @@ __global__ void __launch_bounds__(128) k_pm_pass1(const DcScalars *S, const doub
 
 __global__ void __launch_bounds__(128) k_pm_select(const DcScalars *S, PmWork W)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     const int n_band = min(S->n_band, S->max_band);
     for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < n_band; b += gridDim.x * blockDim.x) {
@@ -350,6 +353,7 @@ __global__ void __launch_bounds__(128) k_pm_select(const DcScalars *S, PmWork W)
 __global__ void __launch_bounds__(128) k_pm_pass2(const DcScalars *S, const double *__restrict__ xyz, const int *__restrict__ conn,
                                                   const int *__restrict__ band_elem, const double *__restrict__ face_nodes, PmWork W)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     using namespace dcp;
     const long long n = (long long)min(S->n_band, S->max_band) * PM_NF2 * 3;
@@ -386,6 +390,7 @@ __global__ void __launch_bounds__(128) k_pm_pass2(const DcScalars *S, const doub
 __global__ void __launch_bounds__(128) k_pm_decide(DcScalars *S, const int *__restrict__ band_elem, const double *__restrict__ face_nodes,
                                                    PmWork W, signed char *__restrict__ labels, double *__restrict__ sdist)
 {
+    pdl_start();
     if (S->status & DC_STATUS_INVALID) return;
     using namespace dcp;
     const int n_band = min(S->n_band, S->max_band);
