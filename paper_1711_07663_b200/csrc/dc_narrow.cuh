@@ -585,7 +585,8 @@ __global__ void __launch_bounds__(NP_TAIL_THREADS) k_np_bound_tail(DcScalars *S,
 
 // ------------------------------------------------------------------------------------------
 // S6 decide (L215: nearest face, dot of the minimal vector with its outward normal; ties L294):
-// one thread per band element.
+// a group of 8 lanes per band element (its ~25 pair keys are one contiguous run: the lanes read it side by side).
+#define ND_W 8
 __global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, const long long *__restrict__ band_start,
                             const int *__restrict__ band_cnt, const unsigned long long *__restrict__ best,
                             const unsigned long long *__restrict__ dmin_arr, const unsigned long long *__restrict__ pair_key,
@@ -595,32 +596,49 @@ __global__ void k_np_decide(DcScalars *S, const int *__restrict__ band_elem, con
     const int n_band = min(S->n_band, S->max_band);
     const double tau = S->tau, tau_exit = S->tau_exit, amb = S->amb, t_tie = S->t_tie, d_band = S->d_band;
     unsigned n_amb = 0, n_samb = 0;
-    for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < n_band; b += gridDim.x * blockDim.x) {   // (n_band is only known on the device)
+    const int sub = threadIdx.x & (ND_W - 1);
+    const unsigned gmask = ((1u << ND_W) - 1u) << ((threadIdx.x & 31) & ~(ND_W - 1));
+    const int ngroups = gridDim.x * blockDim.x / ND_W;
+    const int n_round = (n_band + ngroups - 1) / ngroups * ngroups;          // (uniform trip count: group shuffles below)
+    for (int b = (blockIdx.x * blockDim.x + threadIdx.x) / ND_W; b < n_round; b += ngroups) {   // (n_band is only known on the device)
+        if (b >= n_band) continue;
         const int e = band_elem[b];
         const double dmin = u2d(dmin_arr[b]);
-        if (u2d(best[b]) <= tau_exit) { labels[e] = DC_CUT; sdist[e] = 0.0; }
-        else if (dmin <= tau) { labels[e] = DC_CUT; sdist[e] = 0.0; if (dmin >= tau - amb) ++n_amb; }
+        if (u2d(best[b]) <= tau_exit) { if (sub == 0) { labels[e] = DC_CUT; sdist[e] = 0.0; } }
+        else if (dmin <= tau) { if (sub == 0) { labels[e] = DC_CUT; sdist[e] = 0.0; if (dmin >= tau - amb) ++n_amb; } }
         else if (dmin <= d_band) {
             // (an element whose distance exceeds the band keeps label -1 and takes its sign from the flood fill: beyond
             // best[b] = reach the branch and bound has pruned freely, so the faces it did solve need not include the
             // nearest one, and on a body thinner than the band a far-side face could win the sign)
-            if (dmin <= tau + amb) ++n_amb;
-            int bestmag = -1, neg = 0, npos = 0, nneg = 0;
+            int bestkey = -1, bneg = 0, npos = 0, nneg = 0;   // the largest magnitude wins
             const long long p0 = band_start[b];
             const int cnt = band_cnt[b];
-            for (int p = 0; p < cnt; ++p) {
+            for (int p = sub; p < cnt; p += ND_W) {
                 const unsigned long long key = pair_key[p0 + p];
                 const double dk = u2d(key & ~0xffull);
                 if (dk <= dmin + t_tie) {
                     const int code = (int)(key & 0xff), mag = code & 0x7f, ng = code >> 7;
                     if (ng) ++nneg; else ++npos;
-                    if (mag > bestmag) { bestmag = mag; neg = ng; }
+                    // ties in magnitude go to the first pair of the run, as a single thread walking it would decide:
+                    // (mag, -p) ordered, kept as one integer
+                    const int k2 = (mag << 24) | (0xffffff - min(p, 0xffffff));
+                    if (k2 > bestkey) { bestkey = k2; bneg = ng; }
                 }
             }
-            if (npos && nneg) ++n_samb;
-            labels[e] = neg ? DC_HOLE : DC_NORMAL;
-            const double d = dmin2(dmin, d_band);
-            sdist[e] = neg ? -d : d;
+#pragma unroll
+            for (int o = ND_W / 2; o > 0; o >>= 1) {
+                const int ob = __shfl_xor_sync(gmask, bestkey, o), on = __shfl_xor_sync(gmask, bneg, o);
+                npos += __shfl_xor_sync(gmask, npos, o); nneg += __shfl_xor_sync(gmask, nneg, o);
+                if (ob > bestkey) { bestkey = ob; bneg = on; }
+            }
+            if (sub == 0) {
+                if (dmin <= tau + amb) ++n_amb;
+                if (npos && nneg) ++n_samb;
+                const int neg = bneg;
+                labels[e] = neg ? DC_HOLE : DC_NORMAL;
+                const double d = dmin2(dmin, d_band);
+                sdist[e] = neg ? -d : d;
+            }
         }
     }
 #pragma unroll
