@@ -85,6 +85,8 @@ def do_full(path: str, cfg: int, tag: str):
         if len(r) < len(hdr):
             continue
         name = short(r[ix["Kernel Name"]])
+        if started and name == "k_reset_surface":
+            break                                                # (the next cut begins: one cut only)
         started = started or name == "k_reset_surface"          # (rows before the cut's first kernel belong to the cut before)
         if not started:
             continue
@@ -135,7 +137,8 @@ def do_list(path: str, cfg: int, tag: str):
            "python -m paper_1711_07663_b200.profile_summary list gpurun_out/launches_%s.csv %d %s" % (tag, cfg, tag), "```", "",
            "Per-launch times are cold-cache and serialised: compare SHARES with the CUDA-event times of the bench line "
            "(`cut.ms_full_cut_stages`, `cut.ms_S5_S6_kernels`).  Sources: `src_sha16 = %s`." % source_hash(), "",
-           "One cut (the 4th `dc_set_cut_surface` + `dc_classify(DC_FLAG_RECOMPUTE_BOXES)` of the run): %d launches, %.1f us under ncu." % (len(one), tot), "",
+           "One cut (the 4th `dc_cut` of the run = `dc_set_cut_surface` + `dc_classify(DC_FLAG_RECOMPUTE_BOXES)`, replayed from its CUDA "
+           "graph: ncu profiles the graph's kernel nodes one by one): %d launches, %.1f us under ncu." % (len(one), tot), "",
            "| kernel | launches | sum us | share of the cut |", "|---|---:|---:|---:|"]
     for k, (n, v) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
         out.append("| %s | %d | %.1f | %.1f%% |" % (k, n, v, 100.0 * v / tot))
