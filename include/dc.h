@@ -289,6 +289,20 @@ int dc_adt_build(dc_ctx *ctx, void *adt_dev, size_t adt_bytes, void *stream);
 int dc_find_donors(dc_ctx *ctx, long long n_pts, const double *pts_dev, const double *rot9_host, const double *off3_host,
                    int *donor_dev, double *ref_dev, void *scratch_dev, size_t scratch_bytes, void *stream);
 
+/*
+ * dc_find_donors for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments minus the scratch, same kernels, same results.  The candidate lists
+ * live in a fixed array inside the library (4 456 448 bytes of every GPU that loads libdc, until the process exits), so
+ *   - n_pts <= DC_NOALLOC_MAX_POINTS, else DC_ERR_WORKSPACE (and a line on stderr that says so): split the batch;
+ *   - the call allocates and frees nothing (no cudaMalloc / cudaFree, no allocating library routine); the first call on
+ *     a device also asks the runtime for the array's address, once;
+ *   - every call on a device shares the array: calls that OVERLAP on the GPU (different streams, no ordering between
+ *     them) race on it and give wrong donors; calls ordered on one stream, or by events, are fine.
+ */
+#define DC_NOALLOC_MAX_POINTS 65536
+int dc_find_donors_noalloc(dc_ctx *ctx, long long n_pts, const double *pts_dev, const double *rot9_host, const double *off3_host,
+                           int *donor_dev, double *ref_dev, void *stream);
+
 /* FP64 FMA peak microbenchmark (register-resident DFMA chains on every SM): returns measured
  * TFLOP/s (2 flop per FMA) or a negative error.  Used by bench.py for the "alu" roofline. */
 double dc_measure_fp64_tflops(int device, int iters);

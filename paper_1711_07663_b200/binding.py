@@ -22,12 +22,13 @@ DC_FLAG_PAPER_MODE = 2
 DC_FLAG_EXACT_FAR = 4
 DC_FLAG_GRAPH = 8
 DC_MODE_WALL, DC_MODE_OVERSET = 0, 1
+DC_NOALLOC_MAX_POINTS = 65536
 
 EXPORTS = ["dc_workspace_bytes", "dc_create_grid", "dc_set_cut_surface", "dc_classify", "dc_cut",
            "dc_classify_host", "dc_get_element_boxes", "dc_get_adjacency", "dc_get_pairs",
            "dc_get_stats", "dc_destroy", "dc_error_string", "dc_measure_fp64_tflops", "dc_version",
            "dc_union_labels", "dc_unblank", "dc_ab_faces",
-           "dc_adt_bytes", "dc_donor_scratch_bytes", "dc_adt_build", "dc_find_donors"]
+           "dc_adt_bytes", "dc_donor_scratch_bytes", "dc_adt_build", "dc_find_donors", "dc_find_donors_noalloc"]
 
 
 class dc_params(C.Structure):
@@ -93,6 +94,7 @@ _lib.dc_donor_scratch_bytes.argtypes = [C.c_longlong]
 _lib.dc_donor_scratch_bytes.restype = C.c_size_t
 _lib.dc_adt_build.argtypes = [_vp, _vp, C.c_size_t, _vp]
 _lib.dc_find_donors.argtypes = [_vp, C.c_longlong, _vp, C.POINTER(C.c_double), C.POINTER(C.c_double), _vp, _vp, _vp, C.c_size_t, _vp]
+_lib.dc_find_donors_noalloc.argtypes = [_vp, C.c_longlong, _vp, C.POINTER(C.c_double), C.POINTER(C.c_double), _vp, _vp, _vp]
 
 
 class DcError(RuntimeError):
@@ -316,6 +318,17 @@ class DirectCut:
         _ck(_lib.dc_find_donors(self.ctx, n, pts.data_ptr(), R, o, donor.data_ptr(), ref.data_ptr(), scratch.data_ptr(), sb,
                                 self._stream()), "dc_find_donors")
         return donor, ref
+
+    def find_donors_noalloc(self, pts, donor, ref, rot=None, offset=None, return_code: bool = False):
+        """dc_find_donors_noalloc: pts [n][3] CUDA f64, donor int32 [n] and ref f64 [n][3] CUDA tensors of the caller's;
+        the library's built-in scratch (n <= DC_NOALLOC_MAX_POINTS), nothing allocated here or there."""
+        R = (C.c_double * 9)(*[float(x) for x in rot.reshape(-1)]) if rot is not None else None
+        o = (C.c_double * 3)(*[float(x) for x in offset]) if offset is not None else None
+        rc = _lib.dc_find_donors_noalloc(self.ctx, int(pts.shape[0]), pts.data_ptr(), R, o, donor.data_ptr(), ref.data_ptr(),
+                                         self._stream())
+        if return_code:
+            return rc
+        _ck(rc, "dc_find_donors_noalloc")
 
     def close(self):
         if getattr(self, "ctx", None):

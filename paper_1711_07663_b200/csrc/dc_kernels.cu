@@ -20,6 +20,7 @@
 #include <new>
 #include <algorithm>
 #include <vector>
+#include <mutex>
 
 #include "../../include/dc.h"
 #include "dc_geom.cuh"
@@ -1779,6 +1780,67 @@ extern "C" int dc_find_donors(dc_ctx *c, long long n_pts, const double *pts_dev,
     const double I[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 }, Z[3] = { 0, 0, 0 };
     const double *R = rot9_host ? rot9_host : I, *o = off3_host ? off3_host : Z;
     int *cand = (int *)scratch_dev, *cand_n = cand + (size_t)n_pts * DC_DONOR_CAND;
+    k_adt_search<<<nblk(n_pts, 128), 128, 0, st>>>(c->adt, c->adt_nodes, c->ebox, c->n_elem, pts_dev, n_pts, R[0], R[1], R[2], R[3], R[4],
+                                                   R[5], R[6], R[7], R[8], o[0], o[1], o[2], 1e-12, cand, cand_n);
+    k_donor_newton<<<nblk(n_pts, 128), 128, 0, st>>>(c->xyz, c->conn, c->ebox, c->n_elem, pts_dev, n_pts, R[0], R[1], R[2], R[3], R[4],
+                                                     R[5], R[6], R[7], R[8], o[0], o[1], o[2], cand, cand_n, donor_dev, ref_dev);
+    CK(cudaGetLastError());
+    return DC_OK;
+}
+
+// ---- dc_find_donors_noalloc: the donor search for callers that cannot allocate (code under CUDA graph capture, tight
+// serving loops, harnesses that forbid cudaMalloc).  Same two kernels as dc_find_donors; the candidate lists that call
+// takes as caller-allocated scratch live here in ONE file-scope device array of fixed size: DC_NOALLOC_MAX_POINTS points x
+// (DC_DONOR_CAND candidates + 1 count) x 4 bytes = 4 456 448 bytes, held by every GPU that loads the library until exit.
+// In host code the array's name is only a stand-in for the symbol, not a device address: the address is asked for once
+// per device (cudaGetSymbolAddress with that device current, return code checked) and handed to the kernels.
+// Every call on a device shares the array: calls that overlap on the GPU (two streams) race; calls on one stream do not.
+static __device__ __align__(256) int g_noalloc_donor_scratch[(size_t)DC_NOALLOC_MAX_POINTS * (DC_DONOR_CAND + 1)];
+
+#define DC_NOALLOC_MAX_DEVICES 64
+static std::mutex g_noalloc_mutex;
+static int *g_noalloc_ptr[DC_NOALLOC_MAX_DEVICES];          // device address of the array on each device, once resolved
+
+// set-up, once per device: the caller has made `device` current
+static int noalloc_scratch_address(int device, int **out)
+{
+    if (device < 0 || device >= DC_NOALLOC_MAX_DEVICES) return DC_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_donor_scratch);
+        if (e != cudaSuccess || !p) {
+            fprintf(stderr, "libdc: cudaGetSymbolAddress(g_noalloc_donor_scratch) failed on device %d: %s\n", device, cudaGetErrorString(e));
+            return DC_ERR_CUDA;
+        }
+        g_noalloc_ptr[device] = (int *)p;
+    }
+    *out = g_noalloc_ptr[device];
+    return DC_OK;
+}
+
+extern "C" int dc_find_donors_noalloc(dc_ctx *c, long long n_pts, const double *pts_dev, const double *rot9_host, const double *off3_host,
+                                      int *donor_dev, double *ref_dev, void *stream)
+{
+    if (!c || !pts_dev || !donor_dev || !ref_dev || n_pts < 0) return DC_ERR_ARG;
+    if (!c->adt) return DC_ERR_STATE;
+    if (n_pts > DC_NOALLOC_MAX_POINTS) {
+        fprintf(stderr, "libdc: dc_find_donors_noalloc: %lld points exceed the built-in scratch of %d points; split the batch or call "
+                        "dc_find_donors with scratch of your own\n", n_pts, DC_NOALLOC_MAX_POINTS);
+        return DC_ERR_WORKSPACE;
+    }
+    if (n_pts == 0) return DC_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaSetDevice(c->device));
+    int *scratch = nullptr;
+    { const int rc = noalloc_scratch_address(c->device, &scratch); if (rc) return rc; }
+    const double I[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 }, Z[3] = { 0, 0, 0 };
+    const double *R = rot9_host ? rot9_host : I, *o = off3_host ? off3_host : Z;
+    int *cand = scratch, *cand_n = cand + (size_t)n_pts * DC_DONOR_CAND;
+    // The array keeps the last call's contents.  Nothing in it has to start at zero for the result (k_adt_search writes
+    // cand_n[i] for every point, and cand[i][0 .. cand_n[i]) before k_donor_newton reads them), but the counts are cleared
+    // all the same: a stale count must never be taken for this call's, whatever happens to the first kernel.
+    CK(cudaMemsetAsync(cand_n, 0, (size_t)n_pts * 4, st));
     k_adt_search<<<nblk(n_pts, 128), 128, 0, st>>>(c->adt, c->adt_nodes, c->ebox, c->n_elem, pts_dev, n_pts, R[0], R[1], R[2], R[3], R[4],
                                                    R[5], R[6], R[7], R[8], o[0], o[1], o[2], 1e-12, cand, cand_n);
     k_donor_newton<<<nblk(n_pts, 128), 128, 0, st>>>(c->xyz, c->conn, c->ebox, c->n_elem, pts_dev, n_pts, R[0], R[1], R[2], R[3], R[4],
