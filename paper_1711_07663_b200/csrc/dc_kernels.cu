@@ -1000,6 +1000,7 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double *out, int iters, doubl
 // ==========================================================================================
 struct dc_ctx {
     int device, num_sms;
+    int grid_roots, grid_bound_root, grid_decide;   // grid-stride grids of uniform-work kernels: whole waves of resident CTAs
     long long n_nodes, n_elem, max_faces, max_pairs, n_face, max_band, qcap;
     const double *xyz; const int *conn; const int *adj;
     const double *face_nodes;
@@ -1210,6 +1211,19 @@ static int create_grid_body(dc_ctx *c, int num_sms, int device, long long n_node
     c->h_labels_dev = (signed char *)(c->ws + L.off_hlabels);
     c->h_sdist_dev = (double *)(c->ws + L.off_hsdist);
     c->last_stream = st;
+    {
+        // A grid-stride kernel whose items all cost the same runs as long as its waves of resident CTAs: a grid that is not
+        // a whole number of waves idles part of the GPU through its last one (k_np_roots at 8 CTAs per SM with 6 resident:
+        // 1.33 waves, 0.086 ms; at 6: 0.066 ms).  Resident CTAs per SM from the occupancy calculator, not from a guess at
+        // the register count.
+        int occ = 0;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_np_roots, 256, 0));
+        c->grid_roots = num_sms * (occ > 0 ? occ : 1);
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_np_bound<true>, NPW_THREADS, 0));
+        c->grid_bound_root = num_sms * (occ > 0 ? occ : 1) * 2;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_np_decide, 256, 0));
+        c->grid_decide = num_sms * (occ > 0 ? occ : 1);
+    }
     for (int i = 0; i < 14; ++i) CK(cudaEventCreate(&c->ev[i]));
     for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->evk[i]));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
@@ -1304,12 +1318,12 @@ static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds
                                                  c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT));
     if (part == 1) { CK(cudaGetLastError()); return DC_OK; }
     EVREC(c->ev[10], st);
-    CK(launch_pdl(k_np_roots, c->num_sms * 8, 256, st, S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
+    CK(launch_pdl(k_np_roots, c->grid_roots, 256, st, S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
                                                c->q[0], &S->qn[0], c->qcap));
     // branch and bound, level by level (every item of round r has lP + lQ = r, so 2 max_level + 1 rounds end it):
     // the first rounds as grids, the sparse rest inside one CTA; every round appends its leaves to ONE queue
     EVREC(c->evk[0], st);
-    CK(launch_pdl(k_np_bound<true>, gw, NPW_THREADS, st, S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
+    CK(launch_pdl(k_np_bound<true>, c->grid_bound_root, NPW_THREADS, st, S, &S->qn[0], c->q[0], c->pair_face, c->fcoef, c->ecoef, c->best,
                                                  c->q[1], &S->qn[1], c->nq, c->nqx, &S->nn[0], c->qcap, 0));
     for (int r = 1; r < grid_rounds; ++r)
         CK(launch_pdl(k_np_bound<false>, gw, NPW_THREADS, st, S, &S->qn[r], c->q[r & 1], c->pair_face, c->fcoef, c->ecoef, c->best,
@@ -1465,7 +1479,7 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
     } else {
     { const int rc = launch_narrow(c, st, rounds, grid_rounds, 0); if (rc) return rc; }
     DcScalars *S = c->S;
-    CK(launch_pdl(k_np_decide, c->num_sms * 8, 256, st, S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
+    CK(launch_pdl(k_np_decide, c->grid_decide, 256, st, S, c->band_elem, c->band_start, c->band_cnt, c->best, c->dmin,
                                                                               c->pair_key, labels_dev, sdist_dev));
     CK(ev_record(c->ev[3], st));
     }
