@@ -1022,7 +1022,8 @@ struct dc_ctx {
     int *far_sorted, *far_bins;   // the far elements in Morton order; the bins of the counting sort that makes it
     int *far_heavy;               // [n_elem]: the heavy elements served in a pass (the slice's are listed in act_elem)
     double *h_faces_dev; signed char *h_labels_dev; double *h_sdist_dev;   // staging for dc_classify_host
-    cudaEvent_t ev[14], evk[10];    // evk: boundaries between the kernels of S5/S6
+    cudaEvent_t ev[14], evk[10];
+    cudaStream_t side; cudaEvent_t ev_fork, ev_join;   // second branch of dc_cut's graph (capture only)    // evk: boundaries between the kernels of S5/S6
     cudaStream_t last_stream;
     bool have_surface, have_cut;
     int launches_surface, launches_classify;   // kernels launched by the last dc_set_cut_surface / dc_classify
@@ -1225,6 +1226,9 @@ static int create_grid_body(dc_ctx *c, int num_sms, int device, long long n_node
         c->grid_decide = num_sms * (occ > 0 ? occ : 1);
     }
     for (int i = 0; i < 14; ++i) CK(cudaEventCreate(&c->ev[i]));
+    CK(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
     for (int i = 0; i < 10; ++i) CK(cudaEventCreate(&c->evk[i]));
     CK(cudaMallocHost((void **)&c->S_host, sizeof(DcScalars)));
     CK(cudaMallocHost((void **)&c->S_band_host, sizeof(DcScalars)));
@@ -1532,8 +1536,29 @@ extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, cons
     }
     if (!g) {
         CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
-        int rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
-        if (!rc) rc = dc_classify(c, &P, labels_dev, sdist_dev, stream);
+        // Two branches: the surface's own preparation (S1 + S3: ten short dependent launches over the faces, a few dozen
+        // microseconds that leave most of the GPU idle) does not depend on the element boxes (S2: one pass over the raw
+        // nodes at HBM speed) nor S2 on it, so the graph runs them side by side and joins them in front of S4.
+        int rc = DC_OK;
+        const bool fork = (P.flags & DC_FLAG_RECOMPUTE_BOXES) != 0;
+        if (fork) {
+            cudaError_t e1 = cudaEventRecord(c->ev_fork, st);
+            if (e1 == cudaSuccess) e1 = cudaStreamWaitEvent(c->side, c->ev_fork, 0);
+            if (e1 != cudaSuccess) rc = DC_ERR_CUDA;
+            if (!rc) rc = dc_set_cut_surface(c, n_face, face_nodes_dev, (void *)c->side);
+            if (!rc) rc = run_elem_boxes(c, st);
+            if (!rc) {
+                e1 = cudaEventRecord(c->ev_join, c->side);
+                if (e1 == cudaSuccess) e1 = cudaStreamWaitEvent(st, c->ev_join, 0);
+                if (e1 != cudaSuccess) rc = DC_ERR_CUDA;
+            }
+            dc_params Q = P; Q.flags &= ~DC_FLAG_RECOMPUTE_BOXES;
+            if (!rc) rc = dc_classify(c, &Q, labels_dev, sdist_dev, stream);
+            c->launches_classify += 1;          // (k_elem_boxes)
+        } else {
+            rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
+            if (!rc) rc = dc_classify(c, &P, labels_dev, sdist_dev, stream);
+        }
         cudaGraph_t graph = nullptr;
         const cudaError_t e = cudaStreamEndCapture(st, &graph);
         if (rc || e != cudaSuccess || !graph) {
@@ -1707,6 +1732,9 @@ extern "C" void dc_destroy(dc_ctx *c)
     if (c->last_stream || true) cudaStreamSynchronize(c->last_stream);
     for (int i = 0; i < 14; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 10; ++i) if (c->evk[i]) cudaEventDestroy(c->evk[i]);
+    if (c->side) cudaStreamDestroy(c->side);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->S_host) cudaFreeHost(c->S_host);
     if (c->S_band_host) cudaFreeHost(c->S_band_host);
     for (int i = 0; i < c->n_graphs; ++i) if (c->graphs[i].exec) cudaGraphExecDestroy(c->graphs[i].exec);
