@@ -137,7 +137,10 @@ typedef struct {
     long long n_root_nodes;      /* (pair, patch) items of branch-and-bound round 0 (whole patch pairs) */
     long long band_needed;       /* elements with candidate pairs (> the band capacity on DC_STATUS_BAND_OVERFLOW) */
     long long queue_needed;      /* largest narrow-phase queue any round wanted (> the capacity max(2^20, max_pairs) on
-                                    DC_STATUS_QUEUE_OVERFLOW: size max_pairs >= queue_needed) */
+                                    DC_STATUS_QUEUE_OVERFLOW: size max_pairs >= 1.25 queue_needed -- how many leaves are
+                                    queued depends on the order in which the elements' bounds tighten and differs by a
+                                    few per cent from run to run; the rounds after the one that overflowed are not run,
+                                    so a second, larger need may show up on the next call) */
     long long n_far;             /* DC_FLAG_EXACT_FAR: elements the banded cut left clamped at +-d_band ... */
     long long n_far_done;        /* ... of which got their exact distance (= n_far unless the pass failed) */
     long long n_far_unresolved;  /* ... and for which the narrow phase solved no leaf (0; they keep the clamp) */

@@ -283,9 +283,10 @@ def test_band_overflow_is_reported_with_the_size_needed(B):
     assert st.band_needed > 65536 and st.pairs_needed <= 400000
     # following the sizes reported leads to a valid cut (this workload's whole faces make up to 6 root items per pair:
     # the queues, sized by max_pairs too, are the next thing to fill, and say so the same way; a queue that overflowed
-    # hides what the later rounds would have wanted, hence the loop)
+    # hides what the later rounds would have wanted, hence the loop; the leaf queue's need depends on the order in which the
+    # elements' bounds tighten and differs by a few per cent from run to run, hence the margin dc.h asks for)
     need = 8 * int(st.band_needed)
-    for attempt in range(4):
+    for attempt in range(5):
         dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face, max_pairs=need)
         dcut.set_cut_surface(w.faces); dcut.classify()
         st1 = dcut.stats(allow_status=True)
@@ -294,7 +295,7 @@ def test_band_overflow_is_reported_with_the_size_needed(B):
         if st1.status == 0:
             break
         assert st1.status & B.DC_STATUS_QUEUE_OVERFLOW and st1.queue_needed > max(need, 1 << 20)
-        need = int(st1.queue_needed)
+        need = int(1.25 * st1.queue_needed)
     assert st1.status == 0 and st1.band_needed == st.band_needed and st1.n_cut > 1000
 
 
