@@ -23,9 +23,6 @@
 #pragma once
 
 #define NPW_THREADS 128
-#ifndef NPB_ROOT_OCC
-#define NPB_ROOT_OCC 3
-#endif
 #define DC_STATUS_INVALID (DC_STATUS_PAIR_OVERFLOW | DC_STATUS_QUEUE_OVERFLOW | DC_STATUS_BAND_OVERFLOW)
 #define DC_MAX_ROUNDS 25            /* 2 * 12 + 1 */
 
@@ -546,7 +543,7 @@ __device__ __forceinline__ void np_bound_items(DcScalars *S, int n, const NItem 
 }
 
 template <bool ROOT>
-__global__ void __launch_bounds__(NPW_THREADS, ROOT ? NPB_ROOT_OCC : 2) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
+__global__ void __launch_bounds__(NPW_THREADS, ROOT ? 3 : 2) k_np_bound(DcScalars *S, const int *__restrict__ n_in, const NItem *__restrict__ qin,
                                                           const int *__restrict__ pair_face, const double *__restrict__ fcoef,
                                                           const double *__restrict__ ecoef, unsigned long long *__restrict__ best,
                                                           NItem *__restrict__ qout, int *__restrict__ qout_n,
