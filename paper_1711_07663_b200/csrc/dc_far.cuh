@@ -28,7 +28,7 @@
 // long as its slowest warp.
 //
 // Launch order (run_exact_far): pyramid, faces, list, [codes, scan, sort], nearest; per slice of max_band elements:
-// slots, k_np_stage, k_np_solve(seeds), count, heavy_count; per pass: pairs, heavy_pairs, fix, k_np_roots ... the last
+// slots, k_np_stage, k_np_solve(seeds), count(refine: a better seed face), k_np_solve(seeds), count, heavy_count; per pass: pairs, heavy_pairs, fix, k_np_roots ... the last
 // k_np_solve, decide.
 #pragma once
 
@@ -390,13 +390,20 @@ __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_count(DcScalars *S, cons
                                                               const int *__restrict__ cell_start, const unsigned char *__restrict__ pmask,
                                                               const float *__restrict__ ffar, const int *__restrict__ band_elem,
                                                               int *__restrict__ band_cnt, const unsigned long long *__restrict__ best,
-                                                              int *__restrict__ heavy_list)
+                                                              int *__restrict__ heavy_list, int *__restrict__ pair_face, int refine)
 {
     __shared__ unsigned s_stack[FAR_WARPS][DC_FAR_STACK];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, n = S->n_band;
     if ((i & ~31) >= n) return;
     const bool on = i < n;
     FarLane q = far_lane(S, ebox, n_elem, on ? band_elem[i] : 0, on);
+    // refine: no count -- among the candidates, the face (other than the seed's) whose CENTRE is nearest becomes the pair of a
+    // second seed solve.  The first seed is the face with the nearest box, a bound from below that a tilted face wins for
+    // the wrong reason; among the faces that bound has not excluded, the centre distance (a proxy from above) picks better,
+    // and every bit the attained distance comes down by takes candidates off the list.
+    const int seed_face = (refine && on) ? pair_face[i] : -1;
+    int alt = -1;
+    float alt_d2 = INFINITY;
     const FarGroup g = far_group(q);
     const float cutf = on ? far_cut(S, u2d(best[i]) + S->t_tie) : 0.f, cut2f = __fmul_ru(cutf, cutf);
     const float cutg = cut2f * 1.0001f + 1e-6f;        // (for the cubes: + a hair against the rounding of two distances)
@@ -407,11 +414,23 @@ __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_count(DcScalars *S, cons
     // for after FAR_WARP_CAP faces: a pass lasts as long as its slowest warp.
     int seen = 0;
     far_walk<false>(q, g, cutg, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
+        if (refine) {
+            for (int p = p0; p < p1; ++p)
+                if (q.on && p != seed_face && far_hit(q, cutf, cut2f, ffar, p)) {
+                    const float4 *fp = reinterpret_cast<const float4 *>(ffar) + (size_t)p * 4;
+                    const float ex = __ldg(fp).w - q.cen[0], ey = __ldg(fp + 1).w - q.cen[1], ez = __ldg(fp + 2).w - q.cen[2];
+                    const float d2 = ex * ex + ey * ey + ez * ez;
+                    if (d2 < alt_d2) { alt_d2 = d2; alt = p; }
+                }
+            seen += p1 - p0;
+            return seen > FAR_WARP_CAP;
+        }
         for (int p = p0; p < p1; ++p) if (q.on && far_hit(q, cutf, cut2f, ffar, p) && ++cnt > FAR_HEAVY) q.on = false;
         seen += p1 - p0;
         if (seen > FAR_WARP_CAP && q.on) { cnt = FAR_HEAVY + 1; q.on = false; }
         return !__any_sync(0xffffffffu, q.on);
     });
+    if (refine) { if (on && alt >= 0) pair_face[i] = alt; return; }
     if (on) {
         const bool heavy = cnt > FAR_HEAVY;
         band_cnt[i] = heavy ? FAR_HEAVY_BIT : cnt;

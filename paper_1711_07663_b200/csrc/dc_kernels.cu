@@ -1304,15 +1304,16 @@ extern "C" int dc_set_cut_surface(dc_ctx *c, long long n_face, const double *fac
 }
 
 // S5 as a launch sequence (dc_narrow.cuh).  part 0: the band's narrow phase, with the events that time it.  The exact far
-// pass (dc_far.cuh) runs the same kernels on its own elements: part 1 = stage + seed solves (once per slice), part 2 = roots
-// to the last solve (once per pass, after the pass's candidate pairs have been written).
+// pass (dc_far.cuh) runs the same kernels on its own elements: part 1 = stage + seed solves (once per slice), part 3 = the
+// seed solves again (on better faces), part 2 = roots to the last solve (once per pass, after the pass's candidate pairs
+// have been written).
 #define EVREC(ev_, st_) do { if (part == 0) CK(ev_record(ev_, st_)); } while (0)
 static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds, int part)
 {
     // ---- S5: wavefront narrow phase (dc_narrow.cuh)
     const int gw = c->num_sms * 8;     // grid-stride grids: 8 CTAs of 128 threads per SM
     DcScalars *S = c->S;
-    if (part != 2) CK(launch_pdl(k_np_stage, gw, 128, st, S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox));
+    if (part != 2 && part != 3) CK(launch_pdl(k_np_stage, gw, 128, st, S, c->xyz, c->conn, c->band_elem, c->ecoef, c->pbox));
     // seed solves: one per band element, queue = nq[0 .. n_band); never re-split, and cut short after NW_SEED_MAXIT
     // evaluations (a seed only has to leave an attained upper bound: its pair comes back as a leaf)
     const int gs = c->num_sms * 2 * 4;     // solve grids: grid-stride, 2 resident CTAs of 128 threads per SM
@@ -1320,7 +1321,7 @@ static int launch_narrow(dc_ctx *c, cudaStream_t st, int rounds, int grid_rounds
     if (part != 2)
         CK(launch_pdl(k_np_solve<0>, gs, NW_THREADS, st, S, &S->n_band, c->max_band, c->nq, nullptr, nullptr, c->pair_face, c->fcoef, c->ecoef,
                                                  c->best, c->dmin, c->pair_key, nullptr, nullptr, 0, nullptr, nullptr, 0, 0, NW_SEED_MAXIT));
-    if (part == 1) { CK(cudaGetLastError()); return DC_OK; }
+    if (part == 1 || part == 3) { CK(cudaGetLastError()); return DC_OK; }
     EVREC(c->ev[10], st);
     CK(launch_pdl(k_np_roots, c->grid_roots, 256, st, S, c->pair_band, c->pair_face, c->fboxf, c->pbox, c->best, c->max_pairs,
                                                c->q[0], &S->qn[0], c->qcap));
@@ -1411,7 +1412,9 @@ static int run_exact_far(dc_ctx *c, cudaStream_t st, const signed char *labels_d
         k_far_slots<<<nblk(m, 256), 256, 0, st>>>(list + s0, fstar + s0, (int)m, c->band_elem, c->band_start, c->band_cnt, c->pair_face,
                                                    c->pair_key, c->pair_band, c->nq, c->best, c->dmin);
         { const int rc = launch_narrow(c, st, rounds, grid_rounds, 1); if (rc) return rc; }
-        k_far_count<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_cnt, c->best, c->act_elem);
+        k_far_count<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_cnt, c->best, c->act_elem, c->pair_face, 1);
+        { const int rc = launch_narrow(c, st, rounds, grid_rounds, 3); if (rc) return rc; }      // (second seed solve)
+        k_far_count<<<nblk(m, 128), 128, 0, st>>>(S, c->ebox, ne, c->cell_start, pmask, c->ffar, c->band_elem, c->band_cnt, c->best, c->act_elem, c->pair_face, 0);
         k_far_heavy_count<<<c->num_sms * 4, FAR_HEAVY_THREADS, 0, st>>>(S, c->ebox, ne, c->ffar, c->band_elem, c->band_cnt, c->best, c->act_elem);
         long long pending = m;
         while (pending > 0 && !c->far_error) {
