@@ -23,7 +23,7 @@
 // the nearest), so the pairs are made and solved in PASSES sized to the workspace: in each pass the warps that still wait
 // ask for the slots of their 32 elements at one counter, all or nothing, until the list is full; the host reads two
 // counters per pass.  Deep inside a round body EVERY face is about as near as the next one: an element with more than
-// FAR_HEAVY candidates, or whose warp has walked past FAR_WARP_CAP faces, leaves the walk and is counted and listed by
+// FAR_HEAVY candidates, or whose warp has walked past n_face / 24 faces, leaves the walk and is counted and listed by
 // brute force instead (k_far_heavy_count / k_far_heavy_pairs: a CTA per element, a thread per face) -- a pass lasts as
 // long as its slowest warp.
 //
@@ -313,8 +313,12 @@ __global__ void k_far_sort(const DcScalars *S, const int *__restrict__ list, con
 #ifndef FAR_HEAVY
 #define FAR_HEAVY 128               /* candidates beyond which an element leaves the walk for the brute-force kernels */
 #endif
-#ifndef FAR_WARP_CAP
-#define FAR_WARP_CAP 1024           /* faces a warp may visit before the elements it still walks for leave too */
+#ifndef FAR_WARP_CAP_DIV
+#define FAR_WARP_CAP_DIV 24         /* a warp that has visited n_face / 24 faces (at least 1024) gives up its walk: the elements it still
+                                       walks for go to the brute-force kernels, which cost n_face tests each */
+#endif
+#ifndef FAR_REFINE_CAP_MUL
+#define FAR_REFINE_CAP_MUL 4        /* the walk for a better seed may visit this many times as many */
 #endif
 #define FAR_HEAVY_BIT (1 << 30)
 __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_nearest(DcScalars *S, const int *__restrict__ list, int n,
@@ -411,8 +415,9 @@ __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_count(DcScalars *S, cons
     // An element with more than FAR_HEAVY candidates (deep inside a round body every face is about as near as the next
     // one) leaves the walk -- it would drag its whole warp over most of the surface -- and is counted, and later listed,
     // by the brute-force kernels below, a CTA per element over all faces.  So do the elements a warp is still walking
-    // for after FAR_WARP_CAP faces: a pass lasts as long as its slowest warp.
+    // for after warp_cap faces: a pass lasts as long as its slowest warp.
     int seen = 0;
+    const int warp_cap = max(1024, S->n_face / FAR_WARP_CAP_DIV);
     far_walk<false>(q, g, cutg, cell_start, pmask, s_stack[threadIdx.x >> 5], [&](int p0, int p1) {
         if (refine) {
             for (int p = p0; p < p1; ++p)
@@ -423,11 +428,11 @@ __global__ void __launch_bounds__(FAR_WARPS * 32) k_far_count(DcScalars *S, cons
                     if (d2 < alt_d2) { alt_d2 = d2; alt = p; }
                 }
             seen += p1 - p0;
-            return seen > FAR_WARP_CAP;
+            return seen > warp_cap * FAR_REFINE_CAP_MUL;
         }
         for (int p = p0; p < p1; ++p) if (q.on && far_hit(q, cutf, cut2f, ffar, p) && ++cnt > FAR_HEAVY) q.on = false;
         seen += p1 - p0;
-        if (seen > FAR_WARP_CAP && q.on) { cnt = FAR_HEAVY + 1; q.on = false; }
+        if (seen > warp_cap && q.on) { cnt = FAR_HEAVY + 1; q.on = false; }
         return !__any_sync(0xffffffffu, q.on);
     });
     if (refine) { if (on && alt >= 0) pair_face[i] = alt; return; }
