@@ -211,8 +211,9 @@ int dc_cut(dc_ctx *ctx, const dc_params *params, long long n_face, const double 
 
 /*
  * End-to-end variant with HOST buffers: copies the face nodes host->device, runs
- * dc_cut (DC_FLAG_GRAPH honoured), copies labels and sdist device->host, and synchronises
- * `stream` before returning.  Host buffers should be pinned.
+ * dc_cut, copies labels and sdist device->host, and synchronises `stream` before returning.  Host buffers should be
+ * pinned.  With DC_FLAG_GRAPH and pinned buffers the three copies are nodes of the cut's graph (keyed by the host
+ * addresses too): the faces' upload then runs beside S2, which does not need them.
  */
 int dc_classify_host(dc_ctx *ctx, const dc_params *params, long long n_face,
                      const double *face_nodes_host, signed char *labels_host, double *sdist_host,

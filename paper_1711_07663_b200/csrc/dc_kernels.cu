@@ -1034,6 +1034,7 @@ struct dc_ctx {
     // dc_cut with DC_FLAG_GRAPH: the launch sequences captured so far, by what they were captured for
     struct GraphEntry {
         const double *faces; long long n_face; dc_params P; signed char *labels; double *sdist; cudaStream_t stream;
+        const double *h_faces; signed char *h_labels; double *h_sdist;     // dc_classify_host's buffers (copies inside the graph), else NULL
         cudaGraphExec_t exec; unsigned long long stamp; int launches_surface, launches_classify;
     } graphs[DC_MAX_GRAPHS];
     int n_graphs; unsigned long long graph_clock;
@@ -1514,8 +1515,11 @@ extern "C" int dc_classify(dc_ctx *c, const dc_params *params, signed char *labe
 // Everything a replay must see anew is on the device (the cut's counters, the epoch of the flood fill's flags); what the
 // graph fixes is what it was captured for: the surface's address and face count, the parameters, the output addresses, the
 // stream.  The surface's CONTENTS may change between calls (a moving body updated in place: the re-cut of PAPER.md L233).
-extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, const double *face_nodes_dev,
-                      signed char *labels_dev, double *sdist_dev, void *stream)
+// (h_faces / h_labels / h_sdist: dc_classify_host's pinned host buffers, or all NULL -- the copies then become nodes of the
+// graph: the faces' upload at the head of the surface's branch, next to S2, the results' download at the end)
+static int cut_impl(dc_ctx *c, const dc_params *params, long long n_face, const double *face_nodes_dev,
+                    signed char *labels_dev, double *sdist_dev, void *stream,
+                    const double *h_faces, signed char *h_labels, double *h_sdist)
 {
     if (!c || !face_nodes_dev || !labels_dev || !sdist_dev || n_face <= 0) return DC_ERR_ARG;
     if (n_face > c->max_faces) return DC_ERR_WORKSPACE;
@@ -1528,14 +1532,19 @@ extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, cons
     // no graph of our own: not asked for; the far pass reads counters back between its passes; the caller is capturing
     // already (our launches then go into the caller's graph); the legacy default stream cannot be captured
     if (!(P.flags & DC_FLAG_GRAPH) || (P.flags & DC_FLAG_EXACT_FAR) || cs != cudaStreamCaptureStatusNone || st == nullptr) {
-        const int rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
-        return rc ? rc : dc_classify(c, &P, labels_dev, sdist_dev, stream);
+        if (h_faces) CK(cudaMemcpyAsync((void *)face_nodes_dev, h_faces, (size_t)n_face * 27 * 8, cudaMemcpyHostToDevice, st));
+        int rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
+        if (!rc) rc = dc_classify(c, &P, labels_dev, sdist_dev, stream);
+        if (rc) return rc;
+        if (h_labels) CK(cudaMemcpyAsync(h_labels, labels_dev, (size_t)c->n_elem, cudaMemcpyDeviceToHost, st));
+        if (h_sdist) CK(cudaMemcpyAsync(h_sdist, sdist_dev, (size_t)c->n_elem * 8, cudaMemcpyDeviceToHost, st));
+        return DC_OK;
     }
     dc_ctx::GraphEntry *g = nullptr;
     for (int i = 0; i < c->n_graphs; ++i) {
         dc_ctx::GraphEntry &q = c->graphs[i];
         if (q.faces == face_nodes_dev && q.n_face == n_face && q.labels == labels_dev && q.sdist == sdist_dev && q.stream == st &&
-            memcmp(&q.P, &P, sizeof P) == 0) { g = &q; break; }
+            q.h_faces == h_faces && q.h_labels == h_labels && q.h_sdist == h_sdist && memcmp(&q.P, &P, sizeof P) == 0) { g = &q; break; }
     }
     if (!g) {
         CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
@@ -1547,6 +1556,8 @@ extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, cons
         if (fork) {
             cudaError_t e1 = cudaEventRecord(c->ev_fork, st);
             if (e1 == cudaSuccess) e1 = cudaStreamWaitEvent(c->side, c->ev_fork, 0);
+            if (e1 == cudaSuccess && h_faces)
+                e1 = cudaMemcpyAsync((void *)face_nodes_dev, h_faces, (size_t)n_face * 27 * 8, cudaMemcpyHostToDevice, c->side);
             if (e1 != cudaSuccess) rc = DC_ERR_CUDA;
             if (!rc) rc = dc_set_cut_surface(c, n_face, face_nodes_dev, (void *)c->side);
             if (!rc) rc = run_elem_boxes(c, st);
@@ -1559,9 +1570,12 @@ extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, cons
             if (!rc) rc = dc_classify(c, &Q, labels_dev, sdist_dev, stream);
             c->launches_classify += 1;          // (k_elem_boxes)
         } else {
-            rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
+            if (h_faces && cudaMemcpyAsync((void *)face_nodes_dev, h_faces, (size_t)n_face * 27 * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) rc = DC_ERR_CUDA;
+            if (!rc) rc = dc_set_cut_surface(c, n_face, face_nodes_dev, stream);
             if (!rc) rc = dc_classify(c, &P, labels_dev, sdist_dev, stream);
         }
+        if (!rc && h_labels && cudaMemcpyAsync(h_labels, labels_dev, (size_t)c->n_elem, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = DC_ERR_CUDA;
+        if (!rc && h_sdist && cudaMemcpyAsync(h_sdist, sdist_dev, (size_t)c->n_elem * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = DC_ERR_CUDA;
         cudaGraph_t graph = nullptr;
         const cudaError_t e = cudaStreamEndCapture(st, &graph);
         if (rc || e != cudaSuccess || !graph) {
@@ -1581,6 +1595,7 @@ extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, cons
             cudaGraphExecDestroy(g->exec);
         }
         g->faces = face_nodes_dev; g->n_face = n_face; g->P = P; g->labels = labels_dev; g->sdist = sdist_dev; g->stream = st;
+        g->h_faces = h_faces; g->h_labels = h_labels; g->h_sdist = h_sdist;
         g->exec = exec; g->launches_surface = c->launches_surface; g->launches_classify = c->launches_classify;
     }
     g->stamp = ++c->graph_clock;
@@ -1592,6 +1607,21 @@ extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, cons
     return DC_OK;
 }
 
+extern "C" int dc_cut(dc_ctx *c, const dc_params *params, long long n_face, const double *face_nodes_dev,
+                      signed char *labels_dev, double *sdist_dev, void *stream)
+{
+    return cut_impl(c, params, n_face, face_nodes_dev, labels_dev, sdist_dev, stream, nullptr, nullptr, nullptr);
+}
+
+// is this host pointer page-locked (cudaMallocHost / cudaHostRegister)?  Only then can its copies be nodes of a graph that
+// run asynchronously.
+static bool host_pinned(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeHost;
+}
+
 extern "C" int dc_classify_host(dc_ctx *c, const dc_params *params, long long n_face, const double *face_nodes_host,
                                 signed char *labels_host, double *sdist_host, void *stream)
 {
@@ -1599,6 +1629,14 @@ extern "C" int dc_classify_host(dc_ctx *c, const dc_params *params, long long n_
     if (n_face > c->max_faces) return DC_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     CK(cudaSetDevice(c->device));
+    if (params && (params->flags & DC_FLAG_GRAPH) && host_pinned(face_nodes_host) && host_pinned(labels_host) && host_pinned(sdist_host)) {
+        // copies and cut in ONE graph: the faces' upload runs beside S2, which does not need them
+        const int rc = cut_impl(c, params, n_face, c->h_faces_dev, c->h_labels_dev, c->h_sdist_dev, stream,
+                                face_nodes_host, labels_host, sdist_host);
+        if (rc) return rc;
+        CK(cudaStreamSynchronize(st));
+        return DC_OK;
+    }
     CK(cudaMemcpyAsync(c->h_faces_dev, face_nodes_host, (size_t)n_face * 27 * 8, cudaMemcpyHostToDevice, st));
     const int rc = dc_cut(c, params, n_face, c->h_faces_dev, c->h_labels_dev, c->h_sdist_dev, stream);
     if (rc) return rc;

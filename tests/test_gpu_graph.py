@@ -105,3 +105,32 @@ def test_more_surfaces_than_the_graph_cache_holds(B):
                 lab, sd = dcut.cut(b, p)
             assert np.array_equal(lab.cpu().numpy(), lab0) and np.array_equal(sd.cpu().numpy(), sd0)
         dcut.close()
+
+
+def test_classify_host_with_the_copies_inside_the_graph(B):
+    """dc_classify_host + DC_FLAG_GRAPH with pinned buffers: upload, cut and download are one graph (the upload beside S2);
+    results must be those of the plain path for a surface that changes in place, and pageable buffers must still work."""
+    import torch
+    w = make_config(3, N=20, n=8)
+    steps = [w.spin_faces(s) for s in (0, 5, 9)]
+    want = [plain_cut(B, w, f, B.DC_FLAG_RECOMPUTE_BOXES) for f in steps]
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face)
+        fh = torch.empty((w.n_face, 9, 3), dtype=torch.float64).pin_memory()
+        lh = torch.empty(w.n_elem, dtype=torch.int8).pin_memory()
+        sh = torch.empty(w.n_elem, dtype=torch.float64).pin_memory()
+        for flags in (B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_GRAPH, B.DC_FLAG_GRAPH):
+            p = B.dc_params(); p.flags = flags
+            for rep in range(2):
+                for k, f in enumerate(steps):
+                    fh.copy_(torch.from_numpy(f)); lh.fill_(-9); sh.fill_(99.0)
+                    dcut.classify_host(fh, lh, sh, p)               # (synchronises)
+                    assert np.array_equal(lh.numpy(), want[k][0]) and np.array_equal(sh.numpy(), want[k][1]), (flags, rep, k)
+                    assert dcut.stats().status == 0
+        # pageable host memory: the plain path (copies outside any graph)
+        fp = torch.from_numpy(np.ascontiguousarray(steps[1])); lp = torch.empty(w.n_elem, dtype=torch.int8); sp = torch.empty(w.n_elem, dtype=torch.float64)
+        p = B.dc_params(); p.flags = B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_GRAPH
+        dcut.classify_host(fp, lp, sp, p)
+        assert np.array_equal(lp.numpy(), want[1][0]) and np.array_equal(sp.numpy(), want[1][1])
+        dcut.close()
