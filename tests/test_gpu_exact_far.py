@@ -101,6 +101,21 @@ def test_exact_far_with_recomputed_boxes_and_element_inside_the_body(B, nproc):
     assert (labels == 0).sum() > 0 and (sdist[labels == 0] < 0).all()
 
 
+def test_exact_far_between_several_bodies(B, nproc):
+    """Config 4's eight ellipsoids at reduced size: between bodies the face with the nearest box is often on the wrong
+    body (the second seed solve is for this case), and an element may be equally far from two bodies."""
+    w = make_config(4, N=20, n=5)
+    ref = O.classify(w.xyz, w.conn27, w.faces, nproc=nproc, d_band=WIDE)
+    labels, sdist, st = exact_cut(B, w)
+    far = check(ref, labels, sdist, st, zero_ambiguous=False)
+    assert far.sum() > w.n_elem // 2
+    # the smallest workspace the banded cut itself gets by with: more passes, same values
+    small = max(int(1.3 * st.pairs_needed), 8 * int(st.band_needed))
+    labels2, sdist2, st2 = exact_cut(B, w, max_pairs=small)
+    assert st2.far_passes > st.far_passes, (st.far_passes, st2.far_passes, small, st.far_pairs)
+    assert np.array_equal(labels2, labels) and np.array_equal(sdist2, sdist)
+
+
 def test_one_element_with_more_candidates_than_a_chunk_reports_workspace(B):
     """max_pairs so small that a single far element's candidate faces exceed a chunk: DC_ERR_WORKSPACE, and pairs_needed
     large enough to succeed with."""
