@@ -134,3 +134,29 @@ def test_classify_host_with_the_copies_inside_the_graph(B):
         dcut.classify_host(fp, lp, sp, p)
         assert np.array_equal(lp.numpy(), want[1][0]) and np.array_equal(sp.numpy(), want[1][1])
         dcut.close()
+
+
+def test_cut_inside_the_callers_own_capture(B):
+    """The caller captures the cut into a CUDA graph of its own (here torch's): the library must not start a capture of
+    its own nor record its stage events, and the replayed graph must cut like the plain launches do."""
+    import torch
+    w = make_config(1, N=12, n=4)
+    lab0, sd0, st0 = plain_cut(B, w, w.faces, B.DC_FLAG_RECOMPUTE_BOXES)
+    dcut = B.DirectCut(w.xyz, w.conn27, w.adj6, max_faces=w.n_face)
+    faces = torch.from_numpy(w.faces).cuda()
+    p = B.dc_params(); p.flags = B.DC_FLAG_RECOMPUTE_BOXES | B.DC_FLAG_GRAPH     # (the flag is ignored under a capture)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        dcut.cut(faces, p); torch.cuda.synchronize()                             # (warm-up outside the capture)
+        with torch.cuda.graph(g, stream=s):
+            dcut.cut(faces, p)
+    torch.cuda.synchronize()
+    for rep in range(3):
+        dcut.labels.fill_(-5); dcut.sdist.fill_(7.0)
+        g.replay(); torch.cuda.synchronize()
+        assert np.array_equal(dcut.labels.cpu().numpy(), lab0) and np.array_equal(dcut.sdist.cpu().numpy(), sd0), rep
+        st = dcut.stats()
+        assert st.status == 0 and (st.n_cut, st.n_hole, st.n_normal) == (st0.n_cut, st0.n_hole, st0.n_normal)
+    dcut.close()
